@@ -1,0 +1,24 @@
+import os
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def pytest_configure(config):
+    config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
+
+
+@pytest.fixture(scope="session")
+def cfg1():
+    from paper_2312_05800_b200 import synth
+    return synth.make_config(1)
+
+
+@pytest.fixture(scope="session")
+def omech1(cfg1):
+    from oracle import oracle
+    return oracle.Mech(cfg1[0])
