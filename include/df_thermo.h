@@ -1,0 +1,146 @@
+/* df_thermo.h -- C ABI of libdfthermo.so: the per-cell thermochemistry update of
+ * arXiv 2312.05800 as hand-written sm_100a CUDA.
+ *
+ * Citations: "P:n" = /root/reference/PAPER.md line n; "NS" = BASELINE.json north_star;
+ * "A#" = the reading of that number in DESIGN.md (where the paper is silent or garbled).
+ *
+ *   P:34-36  "the entire computational process is executed on GPU, including machine learning
+ *            chemistry ... and computation of thermal and transport properties"
+ *   P:79     ANN input x = {T, p, F(Y)} (Box-Cox F on mass fractions), output = change of
+ *            mass fractions over the step, Z-score normalisation, hidden layers 1600/800/400, GELU
+ *   P:62     time step of 1 us; mass fractions must sum to unity (also P:86)
+ *   P:44     "Hirschfelder and Curtiss mixture-averaged" transport
+ *   NS       names the rules the paper does not print: Newton on NASA-7, Wilke viscosity,
+ *            combination-rule conductivity, mixture-averaged diffusivities from binary fits.
+ *
+ * Conventions
+ *   - Symbols: n = n_cells, K = species count, R = 8314.46261815324 J/(kmol K), W kg/kmol,
+ *     T K, p Pa, h J/kg, cp J/(kg K), mu Pa s, lambda W/(m K), D m^2/s, omega kg/(m^3 s).
+ *   - Field arrays are DEVICE fp32, structure-of-arrays: Y[k*ld + i], species pitch ld >= n,
+ *     ld % 4 == 0 and every base pointer 16-byte aligned (float4 access).
+ *   - Tables passed to *_create are HOST memory; they are copied and repacked, the caller may
+ *     free them on return.  Handles are immutable afterwards: hot calls on different streams
+ *     may share them.
+ *   - Hot calls validate, enqueue on `stream` (a cudaStream_t passed as void*) and return; they
+ *     never synchronise, allocate or touch host memory.  n_cells == 0 is DF_OK and a no-op.
+ *   - Unless stated, inputs and outputs must not alias.
+ *   - Every function returns DF_OK or an error code; df_last_error() gives the thread-local
+ *     message of the last non-OK return.  No exception crosses this boundary.
+ *   - There is no CPU fallback: without a CUDA device the create calls return DF_ERR_CUDA.
+ */
+#ifndef DF_THERMO_H
+#define DF_THERMO_H
+
+#if defined(__GNUC__)
+#define DF_API __attribute__((visibility("default")))
+#else
+#define DF_API
+#endif
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct df_mech df_mech; /* species tables, opaque */
+typedef struct df_ann df_ann;   /* MLP + normalisation tables, opaque */
+typedef struct df_host_ctx df_host_ctx; /* device staging buffers for df_step_host, opaque */
+
+typedef enum {
+    DF_OK = 0,
+    DF_ERR_INVALID_ARG = 1, /* NULL, negative size, ld < n, misalignment, K mismatch */
+    DF_ERR_UNSUPPORTED = 2, /* shape the kernels are not instantiated for */
+    DF_ERR_ALLOC = 3,       /* host or device allocation failed */
+    DF_ERR_CUDA = 4         /* a CUDA runtime call or launch failed */
+} df_status;
+
+/* ABI version of this header (bumped on any signature change). */
+DF_API int df_abi_version(void);
+DF_API const char* df_last_error(void);
+
+/* ---- species tables (NS (1),(2); A1, A2, A5) ---------------------------------------------
+ * NASA-7, two ranges with one common break T_mid (`hi` applies for T >= T_mid, A2):
+ *   cp_k/R = a1 + a2 T + a3 T^2 + a4 T^3 + a5 T^4
+ *   h_k/(R T) = a1 + a2 T/2 + a3 T^2/3 + a4 T^3/4 + a5 T^4/5 + a6/T        (molar)
+ * Pure-species transport fits, L = ln T (A5):
+ *   sqrt(mu_k) = T^(1/4) sum_{m<5} visc_fit[k][m] L^m
+ *   lambda_k   = T^(1/2) sum_{m<5} cond_fit[k][m] L^m
+ *   p D_jk     = T^(3/2) sum_{m<5} bdiff_fit[j][k][m] L^m   (symmetric; diagonal = self-diffusion)
+ * Supported: 1 <= K <= 64.  T_low/T_high are informative (evaluation extrapolates, A3). */
+DF_API df_status df_mech_create(df_mech** out, int K,
+                         const double* W,        /* [K] */
+                         const double* nasa_lo,  /* [K][7] */
+                         const double* nasa_hi,  /* [K][7] */
+                         double T_low, double T_mid, double T_high,
+                         const double* visc_fit,  /* [K][5] */
+                         const double* cond_fit,  /* [K][5] */
+                         const double* bdiff_fit  /* [K][K][5] */);
+DF_API df_status df_mech_destroy(df_mech* mech);
+DF_API int df_mech_num_species(const df_mech* mech);
+
+/* ---- ANN tables (A8-A11, A13, A14, A16, A19) ------------------------------------------
+ * n_layers linear layers, dims[0] = K+2 inputs (T, p, F(Y_0..K-1)), dims[n_layers] = K outputs,
+ * GELU after every layer but the last.  W[l] is [dims[l+1]][dims[l]] row-major (y = x W^T + b).
+ * precision 0: fp32 FFMA path (any n_layers >= 1, every dims[l] <= 256).
+ * precision 1: bf16 operands / fp32 accumulate on tcgen05 (weights are rounded to bf16 at
+ *              create; n_layers == 4, dims[1..3] multiples of 16 with dims[1] % 64 == 0,
+ *              dims[2] % 32 == 0 and dims[2] <= 1024, dims[3] <= 512, K <= 30).
+ * x_mean/x_std [K+2] and u_mean/u_std [K] are the Z-score statistics; the network output
+ * o is the z-scored change in Box-Cox space (A9): Delta_k = u_std[k] o_k + u_mean[k].
+ * F(y) = (y^lambda - 1)/lambda with lambda = boxcox_lambda > 0 (A10); dt in seconds. */
+DF_API df_status df_ann_create(df_ann** out, int n_layers, const int* dims,
+                        const float* const* W, const float* const* b, int precision,
+                        const double* x_mean, const double* x_std,
+                        const double* u_mean, const double* u_std,
+                        double boxcox_lambda, double dt);
+DF_API df_status df_ann_destroy(df_ann* ann);
+/* Device scratch df_chem_ann_source needs for n_cells cells (0 on the fp32 path).  The bf16
+ * path keeps one layer's activations (bf16) for a bounded chunk of cells, so the value does not
+ * grow with n_cells beyond that chunk. */
+DF_API size_t df_ann_workspace_bytes(const df_ann* ann, long long n_cells);
+
+/* ---- hot call 1: temperature from enthalpy (NS (1); A3, A4) ------------------------------
+ * Solves sum_k Y_k h_k(T)/W_k = h[i] for T by Newton, T <- T - (h(T,Y) - h)/cp(T,Y).
+ * T is in/out: on entry the guess (<= 0, NaN or Inf => T_mid), on exit the root.
+ * cp (optional) receives cp(T_root, Y).  n_unconverged (optional, device int) is atomically
+ * incremented once per cell whose last Newton correction exceeded 1e-2 K. */
+DF_API df_status df_thermo_T_from_h(const df_mech* mech, long long n_cells, long long ld,
+                             const float* h, const float* Y, float* T, float* cp,
+                             int* n_unconverged, void* stream);
+
+/* ---- hot call 2: mixture properties (NS (2); A5-A7) -----------------------------------
+ * cp, h = sum Y_k {cp_k, h_k}(T)/W_k; mu by Wilke; lambda = 1/2 (sum X_k lambda_k +
+ * 1/sum(X_k/lambda_k)); D[k] = sum_{j!=k} Y_j / sum_{j!=k} X_j/D_jk (self-diffusion D_kk when
+ * the denominator is 0).  Any output pointer may be NULL (skipped).  D is [K][ld]. */
+DF_API df_status df_thermo_properties(const df_mech* mech, long long n_cells, long long ld,
+                               const float* T, const float* p, const float* Y,
+                               float* cp, float* h, float* mu, float* lambda, float* D,
+                               void* stream);
+
+/* ---- hot call 3: ANN chemistry source (NS (3); A8-A12, A17) -----------------
+ * features -> MLP -> Delta_k; Y*_k = max(Y_k^lambda + lambda Delta_k, 0)^(1/lambda);
+ * Y'_k = Y*_k / sum_j Y*_j; dY_k = Y'_k - Y_k; rho = p Wbar/(R T); omega_k = rho dY_k / dt.
+ * omega and dY are [K][ld]; either may be NULL.  workspace: device memory of at least
+ * df_ann_workspace_bytes(ann, n_cells) bytes, 1024-byte aligned (may be NULL when that is 0). */
+DF_API df_status df_chem_ann_source(const df_ann* ann, const df_mech* mech, long long n_cells, long long ld,
+                             const float* T, const float* p, const float* Y,
+                             float* omega, float* dY,
+                             void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- host-buffer step (bench.py's e2e leg) ----------------------------------------------
+ * One pass of the whole path over HOST arrays: copies h, p, T_guess, Y host->device, runs
+ * T_from_h -> properties -> ann_source (ann may be NULL: skipped) on the context's stream,
+ * copies the requested outputs device->host and synchronises.  Host arrays should be pinned
+ * for the copies to be asynchronous; pitch of Y, D and omega is ld on both sides.
+ * The context owns device staging for up to max_cells cells. */
+DF_API df_status df_host_ctx_create(df_host_ctx** out, const df_mech* mech, const df_ann* ann, long long max_cells);
+DF_API df_status df_host_ctx_destroy(df_host_ctx* ctx);
+DF_API df_status df_step_host(df_host_ctx* ctx, long long n_cells, long long ld,
+                       const float* h, const float* p, const float* T_guess, const float* Y,
+                       float* T, float* cp, float* mu, float* lambda, float* D, float* omega);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DF_THERMO_H */

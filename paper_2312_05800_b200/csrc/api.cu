@@ -1,0 +1,250 @@
+// api.cu -- the extern "C" boundary of libdfthermo.so (include/df_thermo.h): argument validation,
+// df_ann create/destroy, dispatch to the kernel launchers, and the host-buffer step used by
+// bench.py's e2e leg.  No CPU fallback anywhere: every path ends in a kernel launch or an error.
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "common.cuh"
+
+namespace {
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+df_status check_fields(const char* fn, long long n, long long ld) {
+    if (n < 0) return df_set_error(DF_ERR_INVALID_ARG, "%s: n_cells < 0", fn);
+    if (ld < n) return df_set_error(DF_ERR_INVALID_ARG, "%s: ld (%lld) < n_cells (%lld)", fn, ld, n);
+    if (ld % 4 != 0) return df_set_error(DF_ERR_INVALID_ARG, "%s: ld (%lld) must be a multiple of 4", fn, ld);
+    return DF_OK;
+}
+
+}  // namespace
+
+extern "C" df_status df_ann_create(df_ann** out, int n_layers, const int* dims, const float* const* W,
+                                   const float* const* b, int precision, const double* x_mean, const double* x_std,
+                                   const double* u_mean, const double* u_std, double boxcox_lambda, double dt) {
+    if (!out) return df_set_error(DF_ERR_INVALID_ARG, "df_ann_create: out is NULL");
+    *out = nullptr;
+    if (!dims || !W || !b || !x_mean || !x_std || !u_mean || !u_std)
+        return df_set_error(DF_ERR_INVALID_ARG, "df_ann_create: NULL argument");
+    if (n_layers < 1 || n_layers > 8) return df_set_error(DF_ERR_UNSUPPORTED, "df_ann_create: n_layers=%d", n_layers);
+    if (precision != 0 && precision != 1) return df_set_error(DF_ERR_INVALID_ARG, "df_ann_create: precision=%d", precision);
+    const int K = dims[n_layers];
+    if (K < 1 || K > DF_MAX_K || dims[0] != K + 2)
+        return df_set_error(DF_ERR_INVALID_ARG, "df_ann_create: need dims[0] == dims[n_layers] + 2, K in [1,%d]", DF_MAX_K);
+    if (!(boxcox_lambda > 0.0) || !(dt > 0.0))
+        return df_set_error(DF_ERR_INVALID_ARG, "df_ann_create: boxcox_lambda and dt must be > 0");
+    for (int l = 0; l < n_layers; ++l)
+        if (!W[l] || !b[l] || dims[l + 1] < 1) return df_set_error(DF_ERR_INVALID_ARG, "df_ann_create: layer %d", l);
+    for (int i = 0; i < K + 2; ++i)
+        if (!(x_std[i] > 0.0)) return df_set_error(DF_ERR_INVALID_ARG, "df_ann_create: x_std[%d] <= 0", i);
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+        return df_set_error(DF_ERR_CUDA, "df_ann_create: no CUDA device (there is no CPU fallback)");
+
+    df_ann* a = new (std::nothrow) df_ann;
+    if (!a) return df_set_error(DF_ERR_ALLOC, "df_ann_create: out of host memory");
+    a->n_layers = n_layers;
+    a->dims.assign(dims, dims + n_layers + 1);
+    a->precision = precision;
+    a->K = K;
+    memset(&a->norm, 0, sizeof(a->norm));
+    for (int i = 0; i < K + 2; ++i) {
+        a->norm.x_mean[i] = (float)x_mean[i];
+        a->norm.x_inv_std[i] = (float)(1.0 / x_std[i]);
+    }
+    for (int k = 0; k < K; ++k) {
+        a->norm.u_mean[k] = (float)u_mean[k];
+        a->norm.u_std[k] = (float)u_std[k];
+    }
+    a->norm.lambda = (float)boxcox_lambda;
+    a->norm.inv_lambda = (float)(1.0 / boxcox_lambda);
+    a->norm.inv_dt = (float)(1.0 / dt);
+
+    if (precision == 0) {
+        for (int l = 0; l <= n_layers; ++l)
+            if (dims[l] > 256) {
+                delete a;
+                return df_set_error(DF_ERR_UNSUPPORTED, "df_ann_create: fp32 path supports layer widths <= 256 (got %d)", dims[l]);
+            }
+        std::vector<float> host;
+        for (int l = 0; l < n_layers; ++l) {
+            const int din = dims[l], dout = dims[l + 1], op = (dout + 7) / 8 * 8;
+            a->out_pad.push_back(op);
+            a->w32_off.push_back(host.size());
+            host.resize(host.size() + (size_t)din * op, 0.f);
+            float* wt = host.data() + a->w32_off[l];
+            for (int o = 0; o < dout; ++o)
+                for (int i = 0; i < din; ++i) wt[(size_t)i * op + o] = W[l][(size_t)o * din + i];
+            a->b32_off.push_back(host.size());
+            host.resize(host.size() + op, 0.f);
+            memcpy(host.data() + a->b32_off[l], b[l], sizeof(float) * dout);
+        }
+        if (cudaMalloc((void**)&a->w32, host.size() * sizeof(float)) != cudaSuccess) {
+            delete a;
+            return df_set_error(DF_ERR_ALLOC, "df_ann_create: cudaMalloc failed");
+        }
+        if (cudaMemcpy(a->w32, host.data(), host.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess) {
+            df_ann_destroy(a);
+            return df_set_error(DF_ERR_CUDA, "df_ann_create: cudaMemcpy failed");
+        }
+    } else {
+        const df_status st = ann_bf16_create(a, W, b);
+        if (st != DF_OK) {
+            df_ann_destroy(a);
+            return st;
+        }
+    }
+    *out = a;
+    return DF_OK;
+}
+
+extern "C" df_status df_ann_destroy(df_ann* ann) {
+    if (!ann) return DF_OK;
+    cudaFree(ann->w32);
+    if (ann->bf16) ann_bf16_destroy(ann);
+    delete ann;
+    return DF_OK;
+}
+
+extern "C" size_t df_ann_workspace_bytes(const df_ann* ann, long long n_cells) {
+    if (!ann || n_cells <= 0 || ann->precision == 0) return 0;
+    return ann_bf16_workspace(ann, n_cells);
+}
+
+extern "C" df_status df_thermo_T_from_h(const df_mech* mech, long long n, long long ld, const float* h,
+                                        const float* Y, float* T, float* cp, int* n_unconverged, void* stream) {
+    if (!mech) return df_set_error(DF_ERR_INVALID_ARG, "df_thermo_T_from_h: mech is NULL");
+    df_status st = check_fields("df_thermo_T_from_h", n, ld);
+    if (st != DF_OK) return st;
+    if (n == 0) return DF_OK;
+    if (!h || !Y || !T) return df_set_error(DF_ERR_INVALID_ARG, "df_thermo_T_from_h: NULL field");
+    if (!aligned16(h) || !aligned16(Y) || !aligned16(T) || !aligned16(cp))
+        return df_set_error(DF_ERR_INVALID_ARG, "df_thermo_T_from_h: fields must be 16-byte aligned");
+    return launch_T_from_h(mech, n, ld, h, Y, T, cp, n_unconverged, (cudaStream_t)stream);
+}
+
+extern "C" df_status df_thermo_properties(const df_mech* mech, long long n, long long ld, const float* T,
+                                          const float* p, const float* Y, float* cp, float* h, float* mu,
+                                          float* lambda, float* D, void* stream) {
+    if (!mech) return df_set_error(DF_ERR_INVALID_ARG, "df_thermo_properties: mech is NULL");
+    df_status st = check_fields("df_thermo_properties", n, ld);
+    if (st != DF_OK) return st;
+    if (n == 0) return DF_OK;
+    if (!T || !Y || (D && !p)) return df_set_error(DF_ERR_INVALID_ARG, "df_thermo_properties: NULL input field");
+    if (!cp && !h && !mu && !lambda && !D) return DF_OK;
+    if (!aligned16(T) || !aligned16(p) || !aligned16(Y) || !aligned16(cp) || !aligned16(h) || !aligned16(mu) ||
+        !aligned16(lambda) || !aligned16(D))
+        return df_set_error(DF_ERR_INVALID_ARG, "df_thermo_properties: fields must be 16-byte aligned");
+    return launch_properties(mech, n, ld, T, p, Y, cp, h, mu, lambda, D, (cudaStream_t)stream);
+}
+
+extern "C" df_status df_chem_ann_source(const df_ann* ann, const df_mech* mech, long long n, long long ld,
+                                        const float* T, const float* p, const float* Y, float* omega, float* dY,
+                                        void* workspace, size_t workspace_bytes, void* stream) {
+    if (!ann || !mech) return df_set_error(DF_ERR_INVALID_ARG, "df_chem_ann_source: NULL handle");
+    if (ann->K != mech->K)
+        return df_set_error(DF_ERR_INVALID_ARG, "df_chem_ann_source: ann has K=%d, mech has K=%d", ann->K, mech->K);
+    df_status st = check_fields("df_chem_ann_source", n, ld);
+    if (st != DF_OK) return st;
+    if (n == 0) return DF_OK;
+    if (!T || !p || !Y) return df_set_error(DF_ERR_INVALID_ARG, "df_chem_ann_source: NULL input field");
+    if (!omega && !dY) return DF_OK;
+    if (!aligned16(T) || !aligned16(p) || !aligned16(Y) || !aligned16(omega) || !aligned16(dY))
+        return df_set_error(DF_ERR_INVALID_ARG, "df_chem_ann_source: fields must be 16-byte aligned");
+    if (ann->precision == 0) return launch_ann_fp32(ann, mech, n, ld, T, p, Y, omega, dY, (cudaStream_t)stream);
+    const size_t need = ann_bf16_workspace(ann, n);
+    if (need > 0 && (!workspace || workspace_bytes < need))
+        return df_set_error(DF_ERR_INVALID_ARG, "df_chem_ann_source: workspace of %zu bytes needed, %zu given", need,
+                            workspace ? workspace_bytes : (size_t)0);
+    if (reinterpret_cast<uintptr_t>(workspace) & 1023u)
+        return df_set_error(DF_ERR_INVALID_ARG, "df_chem_ann_source: workspace must be 1024-byte aligned");
+    return launch_ann_bf16(ann, mech, n, ld, T, p, Y, omega, dY, workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
+// ---- host-buffer step ----------------------------------------------------------------------------
+struct df_host_ctx {
+    const df_mech* mech;
+    const df_ann* ann;
+    long long cap;  // cells (pitch of the staging arrays)
+    cudaStream_t stream;
+    float *h, *p, *T, *Y, *cp, *mu, *lam, *D, *omega;
+    void* ws;
+    size_t ws_bytes;
+};
+
+extern "C" df_status df_host_ctx_create(df_host_ctx** out, const df_mech* mech, const df_ann* ann, long long max_cells) {
+    if (!out || !mech || max_cells < 1) return df_set_error(DF_ERR_INVALID_ARG, "df_host_ctx_create: bad argument");
+    *out = nullptr;
+    if (ann && ann->K != mech->K) return df_set_error(DF_ERR_INVALID_ARG, "df_host_ctx_create: K mismatch");
+    df_host_ctx* c = new (std::nothrow) df_host_ctx;
+    if (!c) return df_set_error(DF_ERR_ALLOC, "df_host_ctx_create: out of host memory");
+    memset(c, 0, sizeof(*c));
+    c->mech = mech;
+    c->ann = ann;
+    c->cap = (max_cells + 255) / 256 * 256;
+    const size_t f = (size_t)c->cap * sizeof(float), K = (size_t)mech->K;
+    c->ws_bytes = ann ? df_ann_workspace_bytes(ann, max_cells) : 0;
+    bool ok = cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking) == cudaSuccess;
+    ok = ok && cudaMalloc((void**)&c->h, f) == cudaSuccess && cudaMalloc((void**)&c->p, f) == cudaSuccess &&
+         cudaMalloc((void**)&c->T, f) == cudaSuccess && cudaMalloc((void**)&c->Y, f * K) == cudaSuccess &&
+         cudaMalloc((void**)&c->cp, f) == cudaSuccess && cudaMalloc((void**)&c->mu, f) == cudaSuccess &&
+         cudaMalloc((void**)&c->lam, f) == cudaSuccess && cudaMalloc((void**)&c->D, f * K) == cudaSuccess &&
+         cudaMalloc((void**)&c->omega, f * K) == cudaSuccess;
+    if (ok && c->ws_bytes) ok = cudaMalloc(&c->ws, c->ws_bytes) == cudaSuccess;
+    if (!ok) {
+        df_host_ctx_destroy(c);
+        return df_set_error(DF_ERR_ALLOC, "df_host_ctx_create: device allocation failed: %s",
+                            cudaGetErrorString(cudaGetLastError()));
+    }
+    *out = c;
+    return DF_OK;
+}
+
+extern "C" df_status df_host_ctx_destroy(df_host_ctx* c) {
+    if (!c) return DF_OK;
+    cudaFree(c->h); cudaFree(c->p); cudaFree(c->T); cudaFree(c->Y); cudaFree(c->cp); cudaFree(c->mu);
+    cudaFree(c->lam); cudaFree(c->D); cudaFree(c->omega); cudaFree(c->ws);
+    if (c->stream) cudaStreamDestroy(c->stream);
+    delete c;
+    return DF_OK;
+}
+
+extern "C" df_status df_step_host(df_host_ctx* c, long long n, long long ld, const float* h, const float* p,
+                                  const float* T_guess, const float* Y, float* T, float* cp, float* mu, float* lambda,
+                                  float* D, float* omega) {
+    if (!c) return df_set_error(DF_ERR_INVALID_ARG, "df_step_host: ctx is NULL");
+    if (n < 0 || ld < n || n > c->cap) return df_set_error(DF_ERR_INVALID_ARG, "df_step_host: bad n_cells/ld");
+    if (n == 0) return DF_OK;
+    if (!h || !p || !T_guess || !Y) return df_set_error(DF_ERR_INVALID_ARG, "df_step_host: NULL input");
+    if (omega && !c->ann) return df_set_error(DF_ERR_INVALID_ARG, "df_step_host: omega requested but ctx has no ann");
+    const size_t f = (size_t)n * sizeof(float);
+    const int K = c->mech->K;
+    cudaStream_t s = c->stream;
+    DF_CUDA_TRY(cudaMemcpyAsync(c->h, h, f, cudaMemcpyHostToDevice, s));
+    DF_CUDA_TRY(cudaMemcpyAsync(c->p, p, f, cudaMemcpyHostToDevice, s));
+    DF_CUDA_TRY(cudaMemcpyAsync(c->T, T_guess, f, cudaMemcpyHostToDevice, s));
+    DF_CUDA_TRY(cudaMemcpy2DAsync(c->Y, (size_t)c->cap * sizeof(float), Y, (size_t)ld * sizeof(float), f, K,
+                                  cudaMemcpyHostToDevice, s));
+    df_status st = df_thermo_T_from_h(c->mech, n, c->cap, c->h, c->Y, c->T, nullptr, nullptr, s);
+    if (st != DF_OK) return st;
+    st = df_thermo_properties(c->mech, n, c->cap, c->T, c->p, c->Y, cp ? c->cp : nullptr, nullptr, mu ? c->mu : nullptr,
+                              lambda ? c->lam : nullptr, D ? c->D : nullptr, s);
+    if (st != DF_OK) return st;
+    if (omega) {
+        st = df_chem_ann_source(c->ann, c->mech, n, c->cap, c->T, c->p, c->Y, c->omega, nullptr, c->ws, c->ws_bytes, s);
+        if (st != DF_OK) return st;
+    }
+    if (T) DF_CUDA_TRY(cudaMemcpyAsync(T, c->T, f, cudaMemcpyDeviceToHost, s));
+    if (cp) DF_CUDA_TRY(cudaMemcpyAsync(cp, c->cp, f, cudaMemcpyDeviceToHost, s));
+    if (mu) DF_CUDA_TRY(cudaMemcpyAsync(mu, c->mu, f, cudaMemcpyDeviceToHost, s));
+    if (lambda) DF_CUDA_TRY(cudaMemcpyAsync(lambda, c->lam, f, cudaMemcpyDeviceToHost, s));
+    if (D)
+        DF_CUDA_TRY(cudaMemcpy2DAsync(D, (size_t)ld * sizeof(float), c->D, (size_t)c->cap * sizeof(float), f, K,
+                                      cudaMemcpyDeviceToHost, s));
+    if (omega)
+        DF_CUDA_TRY(cudaMemcpy2DAsync(omega, (size_t)ld * sizeof(float), c->omega, (size_t)c->cap * sizeof(float), f, K,
+                                      cudaMemcpyDeviceToHost, s));
+    DF_CUDA_TRY(cudaStreamSynchronize(s));
+    return DF_OK;
+}

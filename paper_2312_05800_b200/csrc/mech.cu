@@ -1,0 +1,202 @@
+// mech.cu -- df_mech: create-time repacking of the species tables (host, fp64/long double) into
+// the forms the kernels evaluate in fp32 without losing the 1e-5 / 1e-3 K tolerances:
+//   * NASA-7 enthalpy polynomials re-expanded about T_mid in tau = (T - T_mid)/S   (K1)
+//   * ln T fits re-expanded in u = (ln T - Lc)/Ls, |u| <~ 1                        (K2)
+//   * Wilke's mass-ratio factor tabulated as B_kj and W_k^(-1/4) folded into the viscosity fit.
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "common.cuh"
+
+static thread_local char g_err[512] = "";
+
+df_status df_set_error(df_status code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+extern "C" const char* df_last_error(void) { return g_err; }
+extern "C" int df_abi_version(void) { return 1; }
+
+namespace {
+
+// q(x) = p(c + s x): coefficients of the shifted/scaled polynomial, degree n-1.
+void shift_poly(const long double* p, int n, long double c, long double s, long double* q) {
+    for (int m = 0; m < n; ++m) {
+        long double acc = 0.0L, binom = 1.0L, cpow = 1.0L;  // C(i,m) c^(i-m), i = m..n-1
+        for (int i = m; i < n; ++i) {
+            acc += p[i] * binom * cpow;
+            binom = binom * (long double)(i + 1) / (long double)(i + 1 - m);
+            cpow *= c;
+        }
+        q[m] = acc * powl(s, m);
+    }
+}
+
+template <typename T>
+df_status to_device(T** dst, const std::vector<T>& src) {
+    *dst = nullptr;
+    if (src.empty()) return DF_OK;
+    DF_CUDA_TRY(cudaMalloc((void**)dst, src.size() * sizeof(T)));
+    DF_CUDA_TRY(cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return DF_OK;
+}
+
+struct HostTables {
+    int K;
+    MechScalars sc;
+    std::vector<float> th32, invW, sqrtW, visc, cond, ddiag, dfull, wilkeB;
+    std::vector<double> th64;
+};
+
+template <int K>
+PropTables<K>* make_fixed(const HostTables& t) {
+    PropTables<K>* p = new PropTables<K>;
+    memset(p, 0, sizeof(*p));
+    for (int k = 0; k < K; ++k) {
+        for (int r = 0; r < 2; ++r) {
+            p->h0[k][r] = t.th64[(k * 2 + r) * 6];
+            for (int m = 1; m < 6; ++m) p->th[k][r][m - 1] = t.th32[(k * 2 + r) * 6 + m];
+        }
+        p->invW[k] = t.invW[k];
+        p->sqrtW[k] = t.sqrtW[k];
+        for (int m = 0; m < 5; ++m) {
+            p->visc[k][m] = t.visc[k * 5 + m];
+            p->cond[k][m] = t.cond[k * 5 + m];
+            p->ddiag[k][m] = t.ddiag[k * 5 + m];
+        }
+        for (int j = 0; j < K; ++j) p->B[k][j] = t.wilkeB[k * K + j];
+    }
+    int idx = 0;
+    for (int j = 0; j < K; ++j)
+        for (int k = j + 1; k < K; ++k, ++idx)
+            for (int m = 0; m < 5; ++m) p->dpair[idx][m] = t.dfull[(j * K + k) * 5 + m];
+    p->sc = t.sc;
+    return p;
+}
+
+}  // namespace
+
+extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const double* nasa_lo,
+                                    const double* nasa_hi, double T_low, double T_mid, double T_high,
+                                    const double* visc_fit, const double* cond_fit, const double* bdiff_fit) {
+    if (!out) return df_set_error(DF_ERR_INVALID_ARG, "df_mech_create: out is NULL");
+    *out = nullptr;
+    if (!W || !nasa_lo || !nasa_hi || !visc_fit || !cond_fit || !bdiff_fit)
+        return df_set_error(DF_ERR_INVALID_ARG, "df_mech_create: NULL table");
+    if (K < 1 || K > DF_MAX_K) return df_set_error(DF_ERR_UNSUPPORTED, "df_mech_create: K=%d outside [1,%d]", K, DF_MAX_K);
+    if (!(T_low > 0.0) || !(T_mid > T_low) || !(T_high > T_mid))
+        return df_set_error(DF_ERR_INVALID_ARG, "df_mech_create: need 0 < T_low < T_mid < T_high");
+    for (int k = 0; k < K; ++k)
+        if (!(W[k] > 0.0)) return df_set_error(DF_ERR_INVALID_ARG, "df_mech_create: W[%d] <= 0", k);
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+        return df_set_error(DF_ERR_CUDA, "df_mech_create: no CUDA device (there is no CPU fallback)");
+
+    HostTables t;
+    t.K = K;
+    const long double S = 1000.0L;
+    t.sc.T_mid = (float)T_mid;
+    t.sc.S = (float)S;
+    t.sc.inv_S = (float)(1.0L / S);
+    t.sc.tau_min = (float)((50.0L - T_mid) / S);
+    t.sc.tau_max = (float)((6000.0L - T_mid) / S);
+    const long double lnlo = logl((long double)T_low), lnhi = logl((long double)T_high);
+    const long double Lc = 0.5L * (lnlo + lnhi), Ls = 0.55L * (lnhi - lnlo);
+    t.sc.Lc = (float)Lc;
+    t.sc.inv_Ls = (float)(1.0L / Ls);
+    // The kernels compute u = (ln T - (float)Lc) * (float)(1/Ls); re-expand about exactly those fp32 values.
+    const long double Lc_f = (long double)t.sc.Lc, Ls_f = 1.0L / (long double)t.sc.inv_Ls;
+    const long double S_f = 1.0L / (long double)t.sc.inv_S, Tm_f = (long double)t.sc.T_mid;
+
+    t.th32.resize((size_t)K * 12);
+    t.th64.resize((size_t)K * 12);
+    t.invW.resize(K);
+    t.sqrtW.resize(K);
+    t.visc.resize((size_t)K * 5);
+    t.cond.resize((size_t)K * 5);
+    t.ddiag.resize((size_t)K * 5);
+    t.dfull.resize((size_t)K * K * 5);
+    t.wilkeB.resize((size_t)K * K);
+    for (int k = 0; k < K; ++k) {
+        const long double RW = (long double)DF_R_UNIVERSAL / (long double)W[k];
+        for (int r = 0; r < 2; ++r) {
+            const double* a = (r == 0 ? nasa_lo : nasa_hi) + 7 * k;
+            // h_k/W_k = RW (a6 + a1 T + a2 T^2/2 + a3 T^3/3 + a4 T^4/4 + a5 T^5/5)
+            long double p[6] = {(long double)a[5], (long double)a[0], (long double)a[1] / 2, (long double)a[2] / 3,
+                                (long double)a[3] / 4, (long double)a[4] / 5};
+            long double q[6];
+            shift_poly(p, 6, Tm_f, S_f, q);
+            for (int m = 0; m < 6; ++m) {
+                t.th64[(k * 2 + r) * 6 + m] = (double)(RW * q[m]);
+                t.th32[(k * 2 + r) * 6 + m] = (float)(RW * q[m]);
+            }
+        }
+        t.invW[k] = (float)(1.0L / (long double)W[k]);
+        t.sqrtW[k] = (float)sqrtl((long double)W[k]);
+        long double p[5], q[5];
+        const long double w4 = powl((long double)W[k], -0.25L);
+        for (int m = 0; m < 5; ++m) p[m] = (long double)visc_fit[5 * k + m];
+        shift_poly(p, 5, Lc_f, Ls_f, q);
+        for (int m = 0; m < 5; ++m) t.visc[k * 5 + m] = (float)(q[m] * w4);
+        for (int m = 0; m < 5; ++m) p[m] = (long double)cond_fit[5 * k + m];
+        shift_poly(p, 5, Lc_f, Ls_f, q);
+        for (int m = 0; m < 5; ++m) t.cond[k * 5 + m] = (float)q[m];
+        for (int j = 0; j < K; ++j) {
+            // bdiff is declared symmetric; average the two halves so the GPU tables are exactly symmetric.
+            for (int m = 0; m < 5; ++m)
+                p[m] = 0.5L * ((long double)bdiff_fit[5 * ((size_t)j * K + k) + m] +
+                               (long double)bdiff_fit[5 * ((size_t)k * K + j) + m]);
+            shift_poly(p, 5, Lc_f, Ls_f, q);
+            for (int m = 0; m < 5; ++m) t.dfull[((size_t)j * K + k) * 5 + m] = (float)q[m];
+            if (j == k)
+                for (int m = 0; m < 5; ++m) t.ddiag[k * 5 + m] = (float)q[m];
+            t.wilkeB[(size_t)k * K + j] = (float)(1.0L / sqrtl(8.0L * (1.0L + (long double)W[k] / (long double)W[j])));
+        }
+    }
+
+    df_mech* mech = new (std::nothrow) df_mech;
+    if (!mech) return df_set_error(DF_ERR_ALLOC, "df_mech_create: out of host memory");
+    mech->K = K;
+    mech->W_host.assign(W, W + K);
+    MechDev& d = mech->dev;
+    memset(&d, 0, sizeof(d));
+    d.K = K;
+    d.sc = t.sc;
+    df_status st;
+    if ((st = to_device(&d.th32, t.th32)) || (st = to_device(&d.th64, t.th64)) || (st = to_device(&d.invW, t.invW)) ||
+        (st = to_device(&d.sqrtW, t.sqrtW)) || (st = to_device(&d.visc, t.visc)) || (st = to_device(&d.cond, t.cond)) ||
+        (st = to_device(&d.ddiag, t.ddiag)) || (st = to_device(&d.dfull, t.dfull)) ||
+        (st = to_device(&d.wilkeB, t.wilkeB))) {
+        df_mech_destroy(mech);
+        return st;
+    }
+    if (K == 9) mech->t9 = make_fixed<9>(t);
+    if (K == 19) mech->t19 = make_fixed<19>(t);
+    *out = mech;
+    return DF_OK;
+}
+
+extern "C" df_status df_mech_destroy(df_mech* mech) {
+    if (!mech) return DF_OK;
+    MechDev& d = mech->dev;
+    cudaFree(d.th32);
+    cudaFree(d.th64);
+    cudaFree(d.invW);
+    cudaFree(d.sqrtW);
+    cudaFree(d.visc);
+    cudaFree(d.cond);
+    cudaFree(d.ddiag);
+    cudaFree(d.dfull);
+    cudaFree(d.wilkeB);
+    delete mech->t9;
+    delete mech->t19;
+    delete mech;
+    return DF_OK;
+}
+
+extern "C" int df_mech_num_species(const df_mech* mech) { return mech ? mech->K : -1; }

@@ -1,0 +1,189 @@
+"""GPU parity: every hot call through the C ABI vs the fp64 oracle, element by element, on the
+same seeded fp32 inputs (SURVEY 8(c) "same input bits"; tolerances = DESIGN.md A12)."""
+import numpy as np
+import pytest
+
+from tests import helpers
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2312_05800_b200 import binding
+    return binding
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def h_from_T(omech, cells):
+    """fp32 enthalpy field the way a solver would hold it: oracle h(T, Y) rounded once to fp32."""
+    _, h = omech.mixture_cp_h(cells.T, cells.Y[:, :cells.n])
+    return h.astype(np.float32)
+
+
+def make_case(cfg, n, ld=None):
+    from oracle import oracle
+    from paper_2312_05800_b200 import synth
+    mech, ann, cells = synth.make_config(cfg, n=n, ld=ld)
+    return mech, ann, cells, oracle.Mech(mech)
+
+
+# --------------------------------------------------------------------------------------------
+# H1: T from h
+# --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,n,ld", [(1, 4096, None), (5, 20003, 20004), (3, 8190, 8192), (4, 3001, 3004)])
+@pytest.mark.parametrize("guess", ["warm", "cold", "invalid"])
+def test_T_from_h(B, cfg, n, ld, guess):
+    mech, _, cells, om = make_case(cfg, n, ld)
+    h32 = h_from_T(om, cells)
+    if guess == "warm":
+        g = cells.T_guess.copy()
+    elif guess == "cold":
+        g = np.full(n, 1000.0, np.float32)
+    else:
+        g = np.zeros(n, np.float32)
+        g[::3] = np.nan
+        g[1::3] = -5.0
+    T_ref = om.T_from_h(h32, cells.Y[:, :n], np.where(np.isfinite(g) & (g > 0), g, 1000.0))
+    gm = B.Mech(mech)
+    T = dev(g)
+    cp = torch.empty_like(T)
+    cnt = torch.zeros(1, dtype=torch.int32, device="cuda")
+    B.df_thermo_T_from_h(gm, dev(h32), dev(cells.Y), T, cp=cp, n_unconverged=cnt)
+    torch.cuda.synchronize()
+    err = np.abs(T.cpu().numpy().astype(np.float64) - T_ref)
+    assert err.max() <= 1e-3, f"max |dT| = {err.max():.3e} K at {err.argmax()}"
+    assert int(cnt.item()) == 0
+    cp_ref, _ = om.mixture_cp_h(T.cpu().numpy(), cells.Y[:, :n])
+    assert helpers.rel_err(cp.cpu().numpy(), cp_ref).max() <= 1e-5
+
+
+def test_T_from_h_empty_and_errors(B):
+    mech, _, cells, om = make_case(1, 64)
+    gm = B.Mech(mech)
+    Y = dev(cells.Y)
+    T = dev(cells.T_guess)
+    h = dev(h_from_T(om, cells))
+    B.df_thermo_T_from_h(gm, h, Y, T, n_cells=0)  # no-op
+    with pytest.raises(B.DfError) as e:
+        B.df_thermo_T_from_h(gm, h, Y, T, n_cells=65)  # ld < n
+    assert e.value.code == B.DF_ERR_INVALID_ARG
+    with pytest.raises(B.DfError):
+        B.df_thermo_T_from_h(gm, h[1:], Y, T[1:], n_cells=60)  # misaligned
+
+
+# --------------------------------------------------------------------------------------------
+# H2: properties
+# --------------------------------------------------------------------------------------------
+def check_properties(B, mech, cells, om, n):
+    gm = B.Mech(mech)
+    K, ld = cells.Y.shape
+    T, p, Y = dev(cells.T), dev(cells.p), dev(cells.Y)
+    out = {k: torch.empty(n, device="cuda") for k in ("cp", "h", "mu", "lam")}
+    D = torch.zeros(K, ld, device="cuda")
+    B.df_thermo_properties(gm, T, p, Y, D=D, **out)
+    torch.cuda.synchronize()
+    ref = om.properties(cells.T, cells.p, cells.Y[:, :n])
+    for k in ("cp", "mu", "lam"):
+        e = helpers.rel_err(out[k].cpu().numpy(), ref[k])
+        assert e.max() <= 1e-5, f"{k}: max rel err {e.max():.3e} at {e.argmax()}"
+    eh = np.abs(out["h"].cpu().numpy().astype(np.float64) - ref["h"]) / np.maximum(np.abs(ref["h"]), ref["cp"] * cells.T)
+    assert eh.max() <= 1e-5, f"h: {eh.max():.3e}"
+    eD = helpers.rel_err(D.cpu().numpy()[:, :n], ref["D"][:, :n])
+    assert eD.max() <= 1e-5, f"D: max rel err {eD.max():.3e} at {np.unravel_index(eD.argmax(), eD.shape)}"
+
+
+@pytest.mark.parametrize("cfg,n,ld", [(1, 4096, None), (3, 8190, 8192), (5, 20003, 20004), (4, 3001, 3004)])
+def test_properties(B, cfg, n, ld):
+    mech, _, cells, om = make_case(cfg, n, ld)
+    check_properties(B, mech, cells, om, n)
+
+
+@pytest.mark.parametrize("K", [1, 2, 3, 9, 19, 24])
+def test_properties_one_hot_and_generic_K(B, K):
+    """Degenerate cells: pure species (A7 self-diffusion branch) and exact zeros, any K."""
+    from oracle import oracle
+    from paper_2312_05800_b200 import synth
+    mech = synth.make_mechanism(K, 77 + K)
+    n = 4 * K + 8
+    Y = np.zeros((K, n), np.float32)
+    for i in range(n):
+        Y[i % K, i] = 1.0
+    if K > 1:
+        Y[:, -4:] = 0.0
+        Y[0, -4:] = 0.25
+        Y[K - 1, -4:] = 0.75
+    rng = np.random.default_rng(K)
+    cells = synth.Cells(n, rng.uniform(300, 3000, n).astype(np.float32), np.full(n, 2.0e5, np.float32), Y,
+                        np.zeros(n, np.float32))
+    check_properties(B, mech, cells, oracle.Mech(mech), n)
+
+
+def test_properties_subset_outputs(B):
+    mech, _, cells, om = make_case(1, 512)
+    gm = B.Mech(mech)
+    T, p, Y = dev(cells.T), dev(cells.p), dev(cells.Y)
+    cp = torch.empty(512, device="cuda")
+    B.df_thermo_properties(gm, T, p, Y, cp=cp)
+    mu = torch.empty(512, device="cuda")
+    B.df_thermo_properties(gm, T, None, Y, mu=mu)
+    torch.cuda.synchronize()
+    ref = om.properties(cells.T, cells.p, cells.Y)
+    assert helpers.rel_err(cp.cpu().numpy(), ref["cp"]).max() <= 1e-5
+    assert helpers.rel_err(mu.cpu().numpy(), ref["mu"]).max() <= 1e-5
+
+
+# --------------------------------------------------------------------------------------------
+# H3: ANN source, fp32 path
+# --------------------------------------------------------------------------------------------
+def check_source(B, mech, ann, cells, n, tol, sample=None):
+    from oracle import oracle
+    gm, ga = B.Mech(mech), B.Ann(ann)
+    K, ld = cells.Y.shape
+    T, p, Y = dev(cells.T), dev(cells.p), dev(cells.Y)
+    om_g = torch.zeros(K, ld, device="cuda")
+    dY_g = torch.zeros(K, ld, device="cuda")
+    ws = B.alloc_workspace(ga, n)
+    B.df_chem_ann_source(ga, gm, T, p, Y, omega=om_g, dY=dY_g, workspace=ws, n_cells=n)
+    torch.cuda.synchronize()
+    om_g, dY_g = om_g.cpu().numpy(), dY_g.cpu().numpy()
+    # sum_k (Y_k + dY_k) = 1 on every cell (A11 / P:86)
+    s = (cells.Y[:, :n].astype(np.float64) + dY_g[:, :n]).sum(axis=0)
+    assert np.abs(s - 1.0).max() <= 2e-6, np.abs(s - 1.0).max()
+    idx = np.arange(n) if sample is None else sample
+    o_mech, o_ann = oracle.Mech(mech), oracle.Ann(ann)
+    om_r, dY_r = o_ann.source(o_mech, cells.T[idx], cells.p[idx], np.ascontiguousarray(cells.Y[:, idx]))
+    for name, got, ref in (("dY", dY_g[:, idx], dY_r), ("omega", om_g[:, idx], om_r)):
+        mixed, norm = helpers.mixed_err(got, ref[:, :len(idx)])
+        assert mixed <= tol and norm <= tol, f"{name}: mixed {mixed:.3e} normwise {norm:.3e} (tol {tol})"
+    return dY_g, om_g
+
+
+def test_ann_source_fp32_cfg1(B):
+    mech, ann, cells, _ = make_case(1, 4096)
+    check_source(B, mech, ann, cells, 4096, 1e-5)
+
+
+def test_ann_source_fp32_ragged_and_degenerate(B):
+    from paper_2312_05800_b200 import synth
+    mech, ann, cells, _ = make_case(1, 1003, 1004)
+    cells.Y[:, :8] = 0.0
+    cells.Y[np.arange(8), np.arange(8)] = 1.0   # one-hot cells: Y_k = 0 branch of the inverse transform
+    check_source(B, mech, ann, cells, 1003, 1e-5)
+
+
+def test_ann_K_mismatch(B):
+    from paper_2312_05800_b200 import synth
+    mech9 = B.Mech(synth.make_mechanism(9, 1))
+    ann19 = B.Ann(synth.make_ann(19, [32, 32], 0, 1))
+    x = torch.zeros(64, device="cuda")
+    with pytest.raises(B.DfError) as e:
+        B.df_chem_ann_source(ann19, mech9, x, x, torch.zeros(19, 64, device="cuda"), omega=torch.zeros(19, 64, device="cuda"))
+    assert e.value.code == B.DF_ERR_INVALID_ARG
