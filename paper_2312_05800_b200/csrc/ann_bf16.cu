@@ -1,6 +1,709 @@
-// placeholder during bring-up
-#include "common.cuh"
-df_status ann_bf16_create(df_ann*, const float* const*, const float* const*) { return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path not built yet"); }
-void ann_bf16_destroy(df_ann*) {}
-size_t ann_bf16_workspace(const df_ann*, long long) { return 0; }
-df_status launch_ann_bf16(const df_ann*, const df_mech*, long long, long long, const float*, const float*, const float*, float*, float*, void*, size_t, cudaStream_t) { return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path not built yet"); }
+// ann_bf16.cu -- K4: the ANN source term with bf16 operands / fp32 accumulation on the 5th-gen
+// tensor cores (tcgen05.mma, accumulators in TMEM, weights streamed by TMA bulk copies), one
+// persistent warp-specialised kernel for the whole chain (1600-800-400 GELU MLP;
+// DESIGN.md "K4").
+//
+// Per 128-cell tile (UMMA M = 128, one cell per TMEM lane) a CTA runs
+//   prologue   T, p, Y -> Box-Cox + z-score -> bf16 A0 [128 x 32]                    (threads)
+//   phase A    for each half h of layer 2's outputs (N = d2/2 <= 400 TMEM columns):
+//                for each 64-wide chunk j of layer 1:  D1 = A0 W1_j^T  (K = 32)     (tcgen05)
+//                  epilogue warps: +b1, GELU, bf16 -> A1 ring (swizzled smem)       (threads)
+//                  D2 += A1_j W2[h, j]^T                                            (tcgen05)
+//              drain D2: +b2, GELU, bf16 -> this CTA's private H2 scratch (global, L2-resident)
+//   phase B    D3 = H2 W3^T with H2 chunks read back by TMA; drain D3 in 64-wide chunks:
+//              +b3, GELU, bf16 -> H3 ring -> D4 += H3_c W4_c^T; final epilogue: +b4, inverse
+//              Box-Cox, sum-to-one renormalisation, rho, omega -> global (coalesced SoA).
+// Layer 1 is recomputed for each half of layer 2 (K = 32: 2 % of the MMA work) because neither
+// a 128 x 1600 bf16 activation tile (400 KB) nor a 128 x 800 fp32 accumulator (800 TMEM columns)
+// fits on an SM.  All weights are re-tiled at create time into the exact 128B-swizzled K-major
+// shared-memory images the UMMA descriptors expect, in streaming order, so every TMA transfer is
+// one contiguous cp.async.bulk of 8-26 KB.
+//
+// Warp roles (384 threads): 0 = weight-ring TMA producer, 1 = MMA issuer, 2 = TMEM allocator,
+// 3 = auxiliary TMA producer (W1 pairs, H2 chunks, W4), 4..11 = epilogue (8 warps; warp w owns
+// TMEM lanes 32 (w % 4) .. +31 and one half of the columns of every chunk).
+#include <cuda_bf16.h>
+
+#include <cstring>
+#include <new>
+
+#include "ann_common.cuh"
+
+namespace {
+
+// ---- geometry ---------------------------------------------------------------------------------
+constexpr int kTileM = 128;
+constexpr int kThreads = 384;
+constexpr int kWStages = 5;
+constexpr int kChunkBytes = kTileM * 128;  // one [128 x 64] bf16 K-major swizzled operand tile
+constexpr int kW1PairBytes = 64 * 128;     // [64 rows x (2 x 32 K)] bf16
+constexpr int kSmallCol = 448;             // TMEM columns of D1 / D4 (accumulator uses [0, 448))
+constexpr int kTmemCols = 512;
+
+struct NetGeom {
+    int K, K0steps;          // species, k-steps (of 16) of layer 1
+    int d1, d2, d3;          // hidden widths
+    int NC;                  // d1 / 64 chunks of layer 1
+    int NH, na2, nb2;        // half of d2 and its two MMA N pieces
+    int n3a, n3b;            // layer-3 N pieces
+    int NKS;                 // d2 / 32 K-stages of layer 3
+    int NKC;                 // ceil(d2 / 64) H2 chunks
+    int NJ;                  // ceil(d3 / 64) H3 chunks
+    int w2_tile_bytes, w3_tile_bytes, w_slot_bytes, w4_bytes;
+    int smem_bytes;
+    // shared-memory offsets (bytes from the 1024-aligned base)
+    int off_w, off_r1, off_r2, off_w4, off_bar;
+};
+
+struct Bf16Dev {
+    const uint8_t* w1t;  // [ceil(NC/2)][8192]
+    const uint8_t* w2t;  // [2][NC][2][w2_tile_bytes]
+    const uint8_t* w3t;  // [NKS][w3_tile_bytes]
+    const uint8_t* w4t;  // [NJ][4096]
+    const float *b1, *b2, *b3, *b4;
+};
+
+}  // namespace
+
+struct Bf16Plan {
+    NetGeom g;
+    Bf16Dev d;
+    void* blob = nullptr;
+    int num_sms = 0;
+};
+
+namespace {
+
+// ---- PTX wrappers -------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void tma_bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc)
+        : "memory");
+}
+__device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// K-major, 128B-swizzled operand tile: 8-row groups 1024 B apart (SBO), descriptor version 1 (sm_100).
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) |
+           ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
+}
+// kind::f16 instruction descriptor: D = f32, A = B = bf16, both K-major, M = 128.
+__device__ __forceinline__ uint32_t umma_idesc(int N) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
+}
+
+__device__ __forceinline__ float tanh_approx(float x) {
+    float r;
+    asm("tanh.approx.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+// GELU in its tanh form (within 5e-4 of x Phi(x); the bf16 rounding that follows is 4e-3 relative).
+__device__ __forceinline__ float gelu_fast(float v) {
+    const float u = v * fmaf(0.0356774081f, v * v, 0.7978845608f);
+    const float hv = 0.5f * v;
+    return fmaf(hv, tanh_approx(u), hv);
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+    uint32_t r;
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+}
+// byte offset of 16-byte chunk c16 (0..7) of row r inside a 128B-swizzled [rows x 64] bf16 tile
+__device__ __forceinline__ uint32_t swz(int r, int c16) { return (uint32_t)(r * 128 + ((c16 ^ (r & 7)) << 4)); }
+
+// barrier indices
+enum {
+    B_W_FULL = 0, B_W_EMPTY = B_W_FULL + kWStages, B_W1_FULL = B_W_EMPTY + kWStages, B_W1_EMPTY = B_W1_FULL + 2,
+    B_A0_FULL = B_W1_EMPTY + 2, B_SMALL_FULL, B_SMALL_EMPTY, B_A1_FULL, B_A1_EMPTY = B_A1_FULL + 2,
+    B_ACC_FULL = B_A1_EMPTY + 2, B_ACC_EMPTY, B_H2_FULL, B_H2C_FULL, B_H2C_EMPTY = B_H2C_FULL + 2,
+    B_H3_FULL = B_H2C_EMPTY + 2, B_H3_EMPTY = B_H3_FULL + 2, B_TILE_DONE = B_H3_EMPTY + 2, B_W4_FULL, B_COUNT
+};
+
+struct KArgs {
+    NetGeom g;
+    Bf16Dev d;
+    const float* invW;
+    long long n, ld;
+    const float *T, *p, *Y;
+    float *omega, *dY;
+    uint8_t* scratch;  // gridDim.x * NKC * 16384 bytes
+};
+
+__global__ void __launch_bounds__(kThreads, 1)
+ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm nm) {
+    extern __shared__ uint8_t smem_dyn[];
+    const NetGeom& g = a.g;
+    const uint32_t sbase = (smem_u32(smem_dyn) + 1023u) & ~1023u;
+    uint8_t* sgen = smem_dyn + (sbase - smem_u32(smem_dyn));
+    const uint32_t s_w = sbase + g.off_w, s_r1 = sbase + g.off_r1, s_r2 = sbase + g.off_r2, s_w4 = sbase + g.off_w4;
+    const uint32_t s_bar = sbase + g.off_bar;
+    volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(sgen + g.off_bar + B_COUNT * 8);
+    auto bar = [&](int i) { return s_bar + 8u * (uint32_t)i; };
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long num_tiles = (a.n + kTileM - 1) / kTileM;
+
+    if (threadIdx.x == 32) {
+        for (int i = 0; i < B_COUNT; ++i) {
+            uint32_t cnt = 1;
+            if (i == B_A0_FULL || i == B_SMALL_EMPTY || i == B_A1_FULL || i == B_A1_FULL + 1 || i == B_ACC_EMPTY ||
+                i == B_H3_FULL || i == B_H3_FULL + 1)
+                cnt = 8;
+            if (i == B_H2_FULL) cnt = 16;
+            mbar_init(bar(i), cnt);
+        }
+        fence_barrier_init();
+    }
+    if (warp == 2) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
+                         smem_u32((const void*)tmem_slot)),
+                     "n"(kTmemCols));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+
+    if (warp == 0) {
+        // ================= weight-ring TMA producer =================
+        if (lane == 0) {
+            uint32_t cnt = 0;
+            auto load = [&](const uint8_t* src, uint32_t bytes) {
+                const uint32_t slot = cnt % kWStages, par = (cnt / kWStages) & 1;
+                mbar_wait(bar(B_W_EMPTY + slot), par ^ 1);
+                mbar_expect_tx(bar(B_W_FULL + slot), bytes);
+                tma_bulk_g2s(s_w + slot * g.w_slot_bytes, src, bytes, bar(B_W_FULL + slot));
+                ++cnt;
+            };
+            for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+                const int n2 = 2 * g.NC * 2;
+                for (int i = 0; i < n2; ++i) load(a.d.w2t + (size_t)i * g.w2_tile_bytes, g.w2_tile_bytes);
+                for (int ks = 0; ks < g.NKS; ++ks) load(a.d.w3t + (size_t)ks * g.w3_tile_bytes, g.w3_tile_bytes);
+            }
+        }
+    } else if (warp == 3) {
+        // ================= auxiliary TMA producer: W4 (once), W1 pairs, H2 chunks =================
+        if (lane == 0) {
+            mbar_expect_tx(bar(B_W4_FULL), g.w4_bytes);
+            tma_bulk_g2s(s_w4, a.d.w4t, g.w4_bytes, bar(B_W4_FULL));
+            const uint8_t* scratch = a.scratch + (size_t)blockIdx.x * g.NKC * kChunkBytes;
+            const int npairs = (g.NC + 1) / 2;
+            uint32_t w1c = 0, h2c = 0, tc = 0;
+            for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tc) {
+                if (tc > 0) mbar_wait(bar(B_TILE_DONE), (tc - 1) & 1);  // R2 (H3 ring) is free again
+                for (int h = 0; h < 2; ++h)
+                    for (int pr = 0; pr < npairs; ++pr, ++w1c) {
+                        const uint32_t slot = w1c & 1, par = (w1c >> 1) & 1;
+                        mbar_wait(bar(B_W1_EMPTY + slot), par ^ 1);
+                        mbar_expect_tx(bar(B_W1_FULL + slot), kW1PairBytes);
+                        tma_bulk_g2s(s_r2 + kChunkBytes + slot * kW1PairBytes, a.d.w1t + (size_t)pr * kW1PairBytes,
+                                     kW1PairBytes, bar(B_W1_FULL + slot));
+                    }
+                mbar_wait(bar(B_H2_FULL), tc & 1);  // both halves of H2 are in the scratch
+                for (int kc = 0; kc < g.NKC; ++kc, ++h2c) {
+                    const uint32_t slot = h2c & 1, par = (h2c >> 1) & 1;
+                    mbar_wait(bar(B_H2C_EMPTY + slot), par ^ 1);
+                    mbar_expect_tx(bar(B_H2C_FULL + slot), kChunkBytes);
+                    tma_bulk_g2s(s_r1 + slot * kChunkBytes, scratch + (size_t)kc * kChunkBytes, kChunkBytes,
+                                 bar(B_H2C_FULL + slot));
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ================= MMA issuer (one thread) =================
+        if (lane == 0) {
+            const uint32_t id64 = umma_idesc(64), id32 = umma_idesc(32);
+            const uint32_t id2a = umma_idesc(g.na2), id2b = umma_idesc(g.nb2 > 0 ? g.nb2 : 16);
+            const uint32_t id3a = umma_idesc(g.n3a), id3b = umma_idesc(g.n3b > 0 ? g.n3b : 16);
+            const uint32_t d_acc = tmem, d_small = tmem + kSmallCol;
+            uint32_t wc = 0, w1c = 0, se = 0, ae = 0, a1c = 0, h2cc = 0, h3c = 0, tc = 0;
+
+            auto issue_L1 = [&](int jn) {
+                const uint32_t slot = w1c & 1;
+                if ((jn & 1) == 0) mbar_wait(bar(B_W1_FULL + slot), (w1c >> 1) & 1);
+                mbar_wait(bar(B_SMALL_EMPTY), (se & 1) ^ 1);
+                ++se;
+                tc_fence_after();
+                const uint32_t a0 = s_r2, b0 = s_r2 + kChunkBytes + slot * kW1PairBytes + (jn & 1) * 64;
+                for (int kk = 0; kk < g.K0steps; ++kk)
+                    tc_mma(d_small, umma_desc(a0 + kk * 32), umma_desc(b0 + kk * 32), id64, kk > 0);
+                tc_commit(bar(B_SMALL_FULL));
+                if ((jn & 1) == 1 || jn == g.NC - 1) {
+                    tc_commit(bar(B_W1_EMPTY + slot));
+                    ++w1c;
+                }
+            };
+            // one 32-wide K stage of a [128 x N] += A[128 x 32] W^T update, N split into two MMA pieces
+            auto issue_stage = [&](uint32_t a_addr, int na, int nb, uint32_t ida, uint32_t idb, bool first) {
+                const uint32_t slot = wc % kWStages;
+                mbar_wait(bar(B_W_FULL + slot), (wc / kWStages) & 1);
+                ++wc;
+                tc_fence_after();
+                const uint32_t wb = s_w + slot * g.w_slot_bytes;
+                for (int kk = 0; kk < 2; ++kk) {
+                    const uint32_t acc = (!first || kk > 0) ? 1u : 0u;
+                    const uint64_t ad = umma_desc(a_addr + kk * 32);
+                    tc_mma(d_acc, ad, umma_desc(wb + kk * 32), ida, acc);
+                    if (nb > 0) tc_mma(d_acc + na, ad, umma_desc(wb + 64 + kk * 32), idb, acc);
+                }
+                tc_commit(bar(B_W_EMPTY + slot));
+            };
+
+            for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tc) {
+                mbar_wait(bar(B_A0_FULL), tc & 1);
+                // ---- phase A: layers 1+2, one half of layer 2's outputs at a time ----
+                for (int h = 0; h < 2; ++h) {
+                    issue_L1(0);
+                    for (int j = 0; j < g.NC; ++j, ++a1c) {
+                        if (j + 1 < g.NC) issue_L1(j + 1);
+                        const uint32_t slot = a1c & 1;
+                        mbar_wait(bar(B_A1_FULL + slot), (a1c >> 1) & 1);
+                        if (j == 0) {
+                            mbar_wait(bar(B_ACC_EMPTY), (ae & 1) ^ 1);
+                            ++ae;
+                        }
+                        const uint32_t aa = s_r1 + slot * kChunkBytes;
+                        issue_stage(aa, g.na2, g.nb2, id2a, id2b, j == 0);
+                        issue_stage(aa + 64, g.na2, g.nb2, id2a, id2b, false);
+                        tc_commit(bar(B_A1_EMPTY + slot));
+                    }
+                    tc_commit(bar(B_ACC_FULL));
+                }
+                // ---- phase B: layer 3 from the H2 chunks, then layer 4 fed by the D3 drain ----
+                mbar_wait(bar(B_ACC_EMPTY), (ae & 1) ^ 1);
+                ++ae;
+                for (int ks = 0; ks < g.NKS; ++ks) {
+                    const uint32_t slot = h2cc & 1;
+                    if ((ks & 1) == 0) mbar_wait(bar(B_H2C_FULL + slot), (h2cc >> 1) & 1);
+                    issue_stage(s_r1 + slot * kChunkBytes + (ks & 1) * 64, g.n3a, g.n3b, id3a, id3b, ks == 0);
+                    if ((ks & 1) == 1 || ks == g.NKS - 1) {
+                        tc_commit(bar(B_H2C_EMPTY + slot));
+                        ++h2cc;
+                    }
+                }
+                tc_commit(bar(B_ACC_FULL));
+                if (tc == 0) mbar_wait(bar(B_W4_FULL), 0);
+                for (int jj = 0; jj < g.NJ; ++jj, ++h3c) {
+                    const uint32_t slot = h3c & 1;
+                    mbar_wait(bar(B_H3_FULL + slot), (h3c >> 1) & 1);
+                    if (jj == 0) {
+                        mbar_wait(bar(B_SMALL_EMPTY), (se & 1) ^ 1);
+                        ++se;
+                    }
+                    tc_fence_after();
+                    const int cols = min(64, g.d3 - jj * 64);
+                    for (int kk = 0; kk < cols / 16; ++kk)
+                        tc_mma(d_small, umma_desc(s_r2 + slot * kChunkBytes + kk * 32),
+                               umma_desc(s_w4 + jj * 4096 + kk * 32), id32, (jj > 0 || kk > 0) ? 1u : 0u);
+                    tc_commit(bar(B_H3_EMPTY + slot));
+                }
+                tc_commit(bar(B_SMALL_FULL));
+                tc_commit(bar(B_TILE_DONE));
+            }
+        }
+    } else if (warp >= 4) {
+        // ================= epilogue warps (also write the A0 feature tile) =================
+        const int ew = warp - 4, q = ew & 3, ch = ew >> 2;
+        const int row = q * 32 + lane;
+        const uint32_t t_lane = tmem + ((uint32_t)(q * 32) << 16);
+        uint8_t* scratch = a.scratch + (size_t)blockIdx.x * g.NKC * kChunkBytes;
+        uint32_t sf = 0, af = 0, a1c = 0, h3c = 0;
+        const float lam = nm.lambda, inv_lam = nm.inv_lambda;
+
+        // +bias, GELU, pack 16 fp32 accumulators into 8 bf16x2 words
+        auto act16 = [&](const uint32_t (&r)[16], const float* bias, uint32_t (&o)[8]) {
+            const float4* b4 = reinterpret_cast<const float4*>(bias);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const float4 b = __ldg(b4 + i);
+                const float v0 = gelu_fast(__uint_as_float(r[4 * i + 0]) + b.x);
+                const float v1 = gelu_fast(__uint_as_float(r[4 * i + 1]) + b.y);
+                const float v2 = gelu_fast(__uint_as_float(r[4 * i + 2]) + b.z);
+                const float v3 = gelu_fast(__uint_as_float(r[4 * i + 3]) + b.w);
+                o[2 * i] = pack_bf16(v0, v1);
+                o[2 * i + 1] = pack_bf16(v2, v3);
+            }
+        };
+        auto st_shared16 = [&](uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+            asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+        };
+
+        for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+            const long long cell = tile * kTileM + row;
+            const bool valid = cell < a.n;
+            // ---- prologue: features -> bf16 A0; this warp writes feature columns [16 ch, 16 ch + 16) ----
+            {
+                uint32_t o[8];
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    float v[2];
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const int f = ch * 16 + 2 * i + e;
+                        float x = 0.f;
+                        if (valid && f < g.K + 2) {
+                            if (f == 0) x = (__ldg(a.T + cell) - nm.x_mean[0]) * nm.x_inv_std[0];
+                            else if (f == 1) x = (__ldg(a.p + cell) - nm.x_mean[1]) * nm.x_inv_std[1];
+                            else {
+                                const float y = __ldg(a.Y + (size_t)(f - 2) * a.ld + cell);
+                                const float qy = exp2f(lam * __log2f(y));  // y^lambda, 0 -> 0
+                                x = ((qy - 1.0f) * inv_lam - nm.x_mean[f]) * nm.x_inv_std[f];
+                            }
+                        }
+                        v[e] = x;
+                    }
+                    o[i] = pack_bf16(v[0], v[1]);
+                }
+                st_shared16(s_r2 + swz(row, ch * 2), o[0], o[1], o[2], o[3]);
+                st_shared16(s_r2 + swz(row, ch * 2 + 1), o[4], o[5], o[6], o[7]);
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(B_A0_FULL));
+            }
+            // ---- phase A ----
+            for (int h = 0; h < 2; ++h) {
+                for (int j = 0; j < g.NC; ++j, ++a1c) {
+                    mbar_wait(bar(B_SMALL_FULL), sf & 1);
+                    ++sf;
+                    tc_fence_after();
+                    uint32_t r0[16], r1[16];
+                    tc_ld16(t_lane + kSmallCol + ch * 32, r0);
+                    tc_ld16(t_lane + kSmallCol + ch * 32 + 16, r1);
+                    tc_wait_ld();
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar(B_SMALL_EMPTY));
+                    uint32_t o0[8], o1[8];
+                    const float* bias = a.d.b1 + j * 64 + ch * 32;
+                    act16(r0, bias, o0);
+                    act16(r1, bias + 16, o1);
+                    const uint32_t slot = a1c & 1;
+                    mbar_wait(bar(B_A1_EMPTY + slot), ((a1c >> 1) & 1) ^ 1);
+                    const uint32_t base = s_r1 + slot * kChunkBytes;
+                    st_shared16(base + swz(row, ch * 4 + 0), o0[0], o0[1], o0[2], o0[3]);
+                    st_shared16(base + swz(row, ch * 4 + 1), o0[4], o0[5], o0[6], o0[7]);
+                    st_shared16(base + swz(row, ch * 4 + 2), o1[0], o1[1], o1[2], o1[3]);
+                    st_shared16(base + swz(row, ch * 4 + 3), o1[4], o1[5], o1[6], o1[7]);
+                    fence_proxy_async();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar(B_A1_FULL + slot));
+                }
+                // drain D2 (this half): +b2, GELU, bf16 -> H2 scratch in the chunk images phase B loads
+                mbar_wait(bar(B_ACC_FULL), af & 1);
+                ++af;
+                tc_fence_after();
+                const int c_lo = ch ? g.na2 : 0, c_hi = ch ? g.NH : g.na2;
+                for (int c0 = c_lo; c0 < c_hi; c0 += 16) {
+                    uint32_t r[16], o[8];
+                    tc_ld16(t_lane + c0, r);
+                    tc_wait_ld();
+                    const int gc = h * g.NH + c0;
+                    act16(r, a.d.b2 + gc, o);
+                    uint8_t* dst = scratch + (size_t)(gc >> 6) * kChunkBytes;
+                    const int c16 = (gc & 63) >> 3;
+                    *reinterpret_cast<uint4*>(dst + swz(row, c16)) = make_uint4(o[0], o[1], o[2], o[3]);
+                    *reinterpret_cast<uint4*>(dst + swz(row, c16 + 1)) = make_uint4(o[4], o[5], o[6], o[7]);
+                }
+                tc_fence_before();
+                __threadfence();
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) {
+                    mbar_arrive(bar(B_ACC_EMPTY));
+                    mbar_arrive(bar(B_H2_FULL));
+                }
+            }
+            // ---- phase B: drain D3 in 64-wide chunks -> H3 ring (feeds layer 4) ----
+            mbar_wait(bar(B_ACC_FULL), af & 1);
+            ++af;
+            tc_fence_after();
+            for (int jj = 0; jj < g.NJ; ++jj, ++h3c) {
+                uint32_t o[2][8];
+                bool have[2];
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const int c0 = jj * 64 + (ch * 2 + u) * 16;
+                    have[u] = c0 < g.d3;
+                    if (have[u]) {
+                        uint32_t r[16];
+                        tc_ld16(t_lane + c0, r);
+                        tc_wait_ld();
+                        act16(r, a.d.b3 + c0, o[u]);
+                    }
+                }
+                const uint32_t slot = h3c & 1;
+                mbar_wait(bar(B_H3_EMPTY + slot), ((h3c >> 1) & 1) ^ 1);
+                const uint32_t base = s_r2 + slot * kChunkBytes;
+#pragma unroll
+                for (int u = 0; u < 2; ++u)
+                    if (have[u]) {
+                        st_shared16(base + swz(row, (ch * 2 + u) * 2), o[u][0], o[u][1], o[u][2], o[u][3]);
+                        st_shared16(base + swz(row, (ch * 2 + u) * 2 + 1), o[u][4], o[u][5], o[u][6], o[u][7]);
+                    }
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(B_H3_FULL + slot));
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_ACC_EMPTY));
+            // ---- final epilogue: D4 -> Delta -> inverse Box-Cox -> renormalise -> omega (A9-A11, A17) ----
+            mbar_wait(bar(B_SMALL_FULL), sf & 1);
+            ++sf;
+            tc_fence_after();
+            uint32_t r0[16], r1[16];
+            if (ch == 0) {
+                tc_ld16(t_lane + kSmallCol, r0);
+                tc_ld16(t_lane + kSmallCol + 16, r1);
+                tc_wait_ld();
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_SMALL_EMPTY));
+            if (ch == 0 && valid) {
+                const float T = __ldg(a.T + cell), p = __ldg(a.p + cell);
+                float dys[32], yv[32];
+                double sumYm1 = -1.0, sumd = 0.0;
+                float inv_Wbar = 0.f;
+#pragma unroll
+                for (int k = 0; k < 32; ++k) {
+                    if (k < g.K) {
+                        const float ok = __uint_as_float(k < 16 ? r0[k & 15] : r1[k & 15]) + __ldg(a.d.b4 + k);
+                        const float y = __ldg(a.Y + (size_t)k * a.ld + cell);
+                        const float d = ann_dystar(y, fmaf(nm.u_std[k], ok, nm.u_mean[k]), lam, inv_lam);
+                        yv[k] = y;
+                        dys[k] = d;
+                        sumYm1 += (double)y;
+                        sumd += (double)d;
+                        inv_Wbar = fmaf(y, __ldg(a.invW + k), inv_Wbar);
+                    }
+                }
+                const double Sm1 = sumYm1 + sumd, inv_S = 1.0 / (1.0 + Sm1);
+                const float rho_dt = p / (inv_Wbar * (float)DF_R_UNIVERSAL * T) * nm.inv_dt;
+#pragma unroll
+                for (int k = 0; k < 32; ++k) {
+                    if (k < g.K) {
+                        const float d = ann_renorm_dY(dys[k], yv[k], Sm1, inv_S);
+                        if (a.dY) a.dY[(size_t)k * a.ld + cell] = d;
+                        if (a.omega) a.omega[(size_t)k * a.ld + cell] = rho_dt * d;
+                    }
+                }
+            }
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) {
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(kTmemCols));
+    }
+}
+
+}  // namespace
+
+// ---- host side: geometry, weight re-tiling, launch ------------------------------------------------
+namespace {
+
+uint16_t bf16_bits(float x) {  // round to nearest even
+    uint32_t u;
+    memcpy(&u, &x, 4);
+    if ((u & 0x7F800000u) == 0x7F800000u) return (uint16_t)(u >> 16);
+    u += 0x7FFFu + ((u >> 16) & 1u);
+    return (uint16_t)(u >> 16);
+}
+
+// element (row r, column c < 64) of a 128B-swizzled K-major bf16 tile
+inline void put(uint8_t* tile, int r, int c, float v) {
+    const size_t off = (size_t)r * 128 + (size_t)((((c >> 3) ^ (r & 7)) << 4) + (c & 7) * 2);
+    const uint16_t b = bf16_bits(v);
+    memcpy(tile + off, &b, 2);
+}
+
+void split_n(int N, int* na, int* nb) {
+    *na = ((N / 2 + 15) / 16) * 16;
+    if (*na > N) *na = N;
+    *nb = N - *na;
+}
+
+}  // namespace
+
+df_status ann_bf16_create(df_ann* ann, const float* const* W, const float* const* b) {
+    if (ann->n_layers != 4) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: n_layers must be 4 (got %d)", ann->n_layers);
+    const int K = ann->K, d1 = ann->dims[1], d2 = ann->dims[2], d3 = ann->dims[3];
+    if (K > 30) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: K <= 30 (got %d)", K);
+    if (d1 % 64 || d1 < 64) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: dims[1] %% 64 == 0 (got %d)", d1);
+    if (d2 % 32 || d2 < 64 || d2 > 896) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: dims[2] %% 32 == 0, 64..896 (got %d)", d2);
+    if (d3 % 16 || d3 < 32 || d3 > 448) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: dims[3] %% 16 == 0, 32..448 (got %d)", d3);
+
+    Bf16Plan* P = new (std::nothrow) Bf16Plan;
+    if (!P) return df_set_error(DF_ERR_ALLOC, "bf16 path: out of host memory");
+    ann->bf16 = P;
+    NetGeom& g = P->g;
+    g.K = K;
+    g.K0steps = (K + 2 <= 16) ? 1 : 2;
+    g.d1 = d1; g.d2 = d2; g.d3 = d3;
+    g.NC = d1 / 64;
+    g.NH = d2 / 2;
+    split_n(g.NH, &g.na2, &g.nb2);
+    split_n(d3, &g.n3a, &g.n3b);
+    g.NKS = d2 / 32;
+    g.NKC = (d2 + 63) / 64;
+    g.NJ = (d3 + 63) / 64;
+    g.w2_tile_bytes = g.na2 * 128;
+    g.w3_tile_bytes = g.n3a * 128;
+    g.w_slot_bytes = (g.w2_tile_bytes > g.w3_tile_bytes ? g.w2_tile_bytes : g.w3_tile_bytes);
+    g.w_slot_bytes = (g.w_slot_bytes + 1023) / 1024 * 1024;
+    g.w4_bytes = g.NJ * 4096;
+    g.off_w = 0;
+    g.off_r1 = kWStages * g.w_slot_bytes;
+    g.off_r2 = g.off_r1 + 2 * kChunkBytes;
+    g.off_w4 = g.off_r2 + 2 * kChunkBytes;
+    g.off_bar = g.off_w4 + g.w4_bytes;
+    g.smem_bytes = g.off_bar + B_COUNT * 8 + 16 + 1024;
+    if (g.smem_bytes > 227 * 1024) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: layer widths need %d B of shared memory", g.smem_bytes);
+
+    int dev = 0;
+    DF_CUDA_TRY(cudaGetDevice(&dev));
+    DF_CUDA_TRY(cudaDeviceGetAttribute(&P->num_sms, cudaDevAttrMultiProcessorCount, dev));
+
+    const int npairs = (g.NC + 1) / 2;
+    const size_t sz_w1 = (size_t)npairs * kW1PairBytes, sz_w2 = (size_t)2 * g.NC * 2 * g.w2_tile_bytes,
+                 sz_w3 = (size_t)g.NKS * g.w3_tile_bytes, sz_w4 = (size_t)g.w4_bytes;
+    const size_t sz_b = (size_t)(d1 + d2 + d3 + 32) * sizeof(float);
+    const size_t o_w1 = 0, o_w2 = o_w1 + sz_w1, o_w3 = o_w2 + sz_w2, o_w4 = o_w3 + sz_w3, o_b = o_w4 + sz_w4;
+    std::vector<uint8_t> blob(o_b + sz_b, 0);
+    const int din = K + 2;
+    for (int pr = 0; pr < npairs; ++pr)
+        for (int c = 0; c < 2; ++c) {
+            const int chunk = 2 * pr + c;
+            if (chunk >= g.NC) continue;
+            uint8_t* t = blob.data() + o_w1 + (size_t)pr * kW1PairBytes;
+            for (int r = 0; r < 64; ++r)
+                for (int k = 0; k < din; ++k) put(t, r, c * 32 + k, W[0][(size_t)(chunk * 64 + r) * din + k]);
+        }
+    for (int h = 0; h < 2; ++h)
+        for (int j = 0; j < g.NC; ++j)
+            for (int half = 0; half < 2; ++half) {
+                uint8_t* t = blob.data() + o_w2 + (size_t)((h * g.NC + j) * 2 + half) * g.w2_tile_bytes;
+                const int k0 = j * 64 + half * 32;
+                for (int kk = 0; kk < 32; ++kk) {
+                    for (int r = 0; r < g.na2; ++r) put(t, r, kk, W[1][(size_t)(h * g.NH + r) * d1 + k0 + kk]);
+                    for (int r = 0; r < g.nb2; ++r) put(t, r, 32 + kk, W[1][(size_t)(h * g.NH + g.na2 + r) * d1 + k0 + kk]);
+                }
+            }
+    for (int ks = 0; ks < g.NKS; ++ks) {
+        uint8_t* t = blob.data() + o_w3 + (size_t)ks * g.w3_tile_bytes;
+        for (int kk = 0; kk < 32; ++kk) {
+            for (int r = 0; r < g.n3a; ++r) put(t, r, kk, W[2][(size_t)r * d2 + ks * 32 + kk]);
+            for (int r = 0; r < g.n3b; ++r) put(t, r, 32 + kk, W[2][(size_t)(g.n3a + r) * d2 + ks * 32 + kk]);
+        }
+    }
+    for (int jj = 0; jj < g.NJ; ++jj) {
+        uint8_t* t = blob.data() + o_w4 + (size_t)jj * 4096;
+        for (int r = 0; r < K; ++r)
+            for (int c = 0; c < 64 && jj * 64 + c < d3; ++c) put(t, r, c, W[3][(size_t)r * d3 + jj * 64 + c]);
+    }
+    float* hb = reinterpret_cast<float*>(blob.data() + o_b);
+    memcpy(hb, b[0], sizeof(float) * d1);
+    memcpy(hb + d1, b[1], sizeof(float) * d2);
+    memcpy(hb + d1 + d2, b[2], sizeof(float) * d3);
+    memcpy(hb + d1 + d2 + d3, b[3], sizeof(float) * K);
+
+    if (cudaMalloc(&P->blob, blob.size()) != cudaSuccess) return df_set_error(DF_ERR_ALLOC, "bf16 path: cudaMalloc of %zu bytes failed", blob.size());
+    DF_CUDA_TRY(cudaMemcpy(P->blob, blob.data(), blob.size(), cudaMemcpyHostToDevice));
+    const uint8_t* base = static_cast<const uint8_t*>(P->blob);
+    P->d.w1t = base + o_w1;
+    P->d.w2t = base + o_w2;
+    P->d.w3t = base + o_w3;
+    P->d.w4t = base + o_w4;
+    const float* db = reinterpret_cast<const float*>(base + o_b);
+    P->d.b1 = db;
+    P->d.b2 = db + d1;
+    P->d.b3 = db + d1 + d2;
+    P->d.b4 = db + d1 + d2 + d3;
+    DF_CUDA_TRY(cudaFuncSetAttribute(ann_bf16_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, g.smem_bytes));
+    return DF_OK;
+}
+
+void ann_bf16_destroy(df_ann* ann) {
+    if (!ann->bf16) return;
+    cudaFree(ann->bf16->blob);
+    delete ann->bf16;
+    ann->bf16 = nullptr;
+}
+
+static long long bf16_grid(const Bf16Plan* P, long long n) {
+    const long long tiles = (n + kTileM - 1) / kTileM;
+    return tiles < P->num_sms ? tiles : P->num_sms;
+}
+
+size_t ann_bf16_workspace(const df_ann* ann, long long n) {
+    const Bf16Plan* P = ann->bf16;
+    return (size_t)bf16_grid(P, n) * P->g.NKC * kChunkBytes;
+}
+
+df_status launch_ann_bf16(const df_ann* ann, const df_mech* mech, long long n, long long ld, const float* T,
+                          const float* p, const float* Y, float* omega, float* dY, void* ws, size_t ws_bytes,
+                          cudaStream_t s) {
+    const Bf16Plan* P = ann->bf16;
+    KArgs a;
+    a.g = P->g;
+    a.d = P->d;
+    a.invW = mech->dev.invW;
+    a.n = n;
+    a.ld = ld;
+    a.T = T; a.p = p; a.Y = Y;
+    a.omega = omega; a.dY = dY;
+    a.scratch = static_cast<uint8_t*>(ws);
+    (void)ws_bytes;
+    ann_bf16_kernel<<<(unsigned)bf16_grid(P, n), kThreads, P->g.smem_bytes, s>>>(a, ann->norm);
+    DF_CUDA_TRY(cudaGetLastError());
+    return DF_OK;
+}

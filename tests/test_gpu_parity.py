@@ -187,3 +187,31 @@ def test_ann_K_mismatch(B):
     with pytest.raises(B.DfError) as e:
         B.df_chem_ann_source(ann19, mech9, x, x, torch.zeros(19, 64, device="cuda"), omega=torch.zeros(19, 64, device="cuda"))
     assert e.value.code == B.DF_ERR_INVALID_ARG
+
+
+# --------------------------------------------------------------------------------------------
+# H3: ANN source, bf16 / tcgen05 path (tolerance 2e-2, A12)
+# --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("hidden,n,ld", [([128, 64, 32], 1000, 1000), ([64, 64, 48], 131, 132), ([192, 96, 80], 700, 704)])
+def test_ann_source_bf16_small_nets(B, hidden, n, ld):
+    """Small layer widths exercise the chunk/piece bookkeeping of the chain at sizes the oracle does in full."""
+    from paper_2312_05800_b200 import synth
+    mech = synth.make_mechanism(19, synth.config_seed(2))
+    ann = synth.make_ann(19, hidden, 1, synth.config_seed(2))
+    cells = synth.cells_stratified(19, n, synth.config_seed(2), ld=ld)
+    check_source(B, mech, ann, cells, n, 2e-2)
+
+
+@pytest.mark.parametrize("n", [128, 2077])
+def test_ann_source_bf16_paper_net(B, n):
+    """21 -> 1600 -> 800 -> 400 -> 19, every cell against the oracle; 2077 = 16 tiles + ragged tail."""
+    mech, ann, cells, _ = make_case(2, n, (n + 3) // 4 * 4)
+    check_source(B, mech, ann, cells, n, 2e-2)
+
+
+def test_ann_source_bf16_multi_tile_per_cta(B):
+    """More tiles than SMs (each CTA loops) on the paper's net: sampled cells vs oracle, sum-to-one on all."""
+    n = 148 * 128 * 2 + 77
+    mech, ann, cells, _ = make_case(2, n, (n + 3) // 4 * 4)
+    sample = np.unique(np.concatenate([np.arange(0, n, 97), np.arange(n - 130, n)]))
+    check_source(B, mech, ann, cells, n, 2e-2, sample=sample)
