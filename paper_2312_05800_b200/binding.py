@@ -102,7 +102,7 @@ class Mech:
         self.handle = h
 
     def close(self):
-        if getattr(self, "handle", None):
+        if getattr(self, "handle", None) and _lib is not None:
             _lib.df_mech_destroy(self.handle)
             self.handle = None
 
@@ -135,7 +135,7 @@ class Ann:
         return int(_lib.df_ann_workspace_bytes(self.handle, int(n_cells)))
 
     def close(self):
-        if getattr(self, "handle", None):
+        if getattr(self, "handle", None) and _lib is not None:
             _lib.df_ann_destroy(self.handle)
             self.handle = None
 
@@ -190,7 +190,7 @@ class HostCtx:
                                  _dp(cp), _dp(mu), _dp(lam), _dp(D), _dp(omega)))
 
     def close(self):
-        if getattr(self, "handle", None):
+        if getattr(self, "handle", None) and _lib is not None:
             _lib.df_host_ctx_destroy(self.handle)
             self.handle = None
 
