@@ -23,6 +23,9 @@
 // 3 = auxiliary TMA producer (W1 pairs, H2 chunks, W4), 4..11 = epilogue (8 warps; warp w owns
 // TMEM lanes 32 (w % 4) .. +31 and one half of the columns of every chunk).
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
+#include <cstdlib>
 
 #include <cstring>
 #include <new>
@@ -33,17 +36,23 @@ namespace {
 
 // ---- geometry ---------------------------------------------------------------------------------
 constexpr int kTileM = 128;
-constexpr int kThreads = 384;
+#ifndef KGROUPS
+#define KGROUPS 3
+#endif
+constexpr int kGroups = KGROUPS;                  // epilogue groups of 4 warps (one warp per TMEM lane quarter)
+constexpr int kThreads = 128 + kGroups * 128;
 constexpr int kWStages = 5;
 constexpr int kChunkBytes = kTileM * 128;  // one [128 x 64] bf16 K-major swizzled operand tile
-constexpr int kW1PairBytes = 64 * 128;     // [64 rows x (2 x 32 K)] bf16
-constexpr int kSmallCol = 448;             // TMEM columns of D1 / D4 (accumulator uses [0, 448))
+constexpr int kW1QuadBytes = 64 * 128;     // four 32-row layer-1 chunks: [2 x 32 rows] x [2 x 32 K] bf16
+constexpr int kSmallCol = 400;             // TMEM columns [400, 496): three 32-column D1 buffers (D4 reuses the first)
+constexpr int kSmallBufs = 3;
 constexpr int kTmemCols = 512;
 
 struct NetGeom {
-    int K, K0steps;          // species, k-steps (of 16) of layer 1
+    int b_fmt;               // UMMA B (weight) format: 1 = bf16, 0 = fp16
+    int K, K0steps;          // species, k-steps (of 16) over the K+4 layer-1 inputs (features, 2 bias columns)
     int d1, d2, d3;          // hidden widths
-    int NC;                  // d1 / 64 chunks of layer 1
+    int NC;                  // d1 / 32 chunks of layer 1 (one 32-wide K stage of layer 2 each)
     int NH, na2, nb2;        // half of d2 and its two MMA N pieces
     int n3a, n3b;            // layer-3 N pieces
     int NKS;                 // d2 / 32 K-stages of layer 3
@@ -56,8 +65,8 @@ struct NetGeom {
 };
 
 struct Bf16Dev {
-    const uint8_t* w1t;  // [ceil(NC/2)][8192]
-    const uint8_t* w2t;  // [2][NC][2][w2_tile_bytes]
+    const uint8_t* w1t;  // [ceil(NC/4)][8192]
+    const uint8_t* w2t;  // [2][NC][w2_tile_bytes]
     const uint8_t* w3t;  // [NKS][w3_tile_bytes]
     const uint8_t* w4t;  // [NJ][4096]
     const float *b1, *b2, *b3, *b4;
@@ -133,9 +142,30 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
     return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) |
            ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
 }
-// kind::f16 instruction descriptor: D = f32, A = B = bf16, both K-major, M = 128.
-__device__ __forceinline__ uint32_t umma_idesc(int N) {
-    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
+// kind::f16 instruction descriptor: D = f32, A = fp16 activations (format 0), B = bf16 weights (format 1),
+// both K-major, M = 128.
+__device__ __forceinline__ uint32_t umma_idesc(int N, int b_fmt) {
+    return (1u << 4) | (0u << 7) | ((uint32_t)b_fmt << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
+}
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile(
+        "{\n\t.reg .b32 rx;\n\t.reg .pred px;\n\t"
+        "elect.sync rx|px, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, px;\n\t}"
+        : "=r"(pred));
+    return pred != 0;
+}
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return done != 0;
 }
 
 __device__ __forceinline__ float tanh_approx(float x) {
@@ -145,24 +175,41 @@ __device__ __forceinline__ float tanh_approx(float x) {
 }
 // GELU in its tanh form (within 5e-4 of x Phi(x); the bf16 rounding that follows is 4e-3 relative).
 __device__ __forceinline__ float gelu_fast(float v) {
+#ifdef DF_DBG_NO_GELU
+    return v;
+#endif
     const float u = v * fmaf(0.0356774081f, v * v, 0.7978845608f);
     const float hv = 0.5f * v;
     return fmaf(hv, tanh_approx(u), hv);
 }
-__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+// two fp32 -> packed fp16x2 (first argument in the low half = lower K index)
+__device__ __forceinline__ uint32_t pack_act(float lo, float hi) {
     uint32_t r;
-    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
     return r;
 }
 // byte offset of 16-byte chunk c16 (0..7) of row r inside a 128B-swizzled [rows x 64] bf16 tile
 __device__ __forceinline__ uint32_t swz(int r, int c16) { return (uint32_t)(r * 128 + ((c16 ^ (r & 7)) << 4)); }
 
+__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&r)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,"
+        "%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+          "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+          "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr)
+        : "memory");
+}
+
 // barrier indices
 enum {
     B_W_FULL = 0, B_W_EMPTY = B_W_FULL + kWStages, B_W1_FULL = B_W_EMPTY + kWStages, B_W1_EMPTY = B_W1_FULL + 2,
-    B_A0_FULL = B_W1_EMPTY + 2, B_SMALL_FULL, B_SMALL_EMPTY, B_A1_FULL, B_A1_EMPTY = B_A1_FULL + 2,
-    B_ACC_FULL = B_A1_EMPTY + 2, B_ACC_EMPTY, B_H2_FULL, B_H2C_FULL, B_H2C_EMPTY = B_H2C_FULL + 2,
-    B_H3_FULL = B_H2C_EMPTY + 2, B_H3_EMPTY = B_H3_FULL + 2, B_TILE_DONE = B_H3_EMPTY + 2, B_W4_FULL, B_COUNT
+    B_A0_FULL = B_W1_EMPTY + 2, B_SMALL_FULL, B_SMALL_EMPTY = B_SMALL_FULL + kSmallBufs,
+    B_A1_FULL = B_SMALL_EMPTY + kSmallBufs, B_A1_EMPTY = B_A1_FULL + 4, B_ACC_FULL = B_A1_EMPTY + 4, B_ACC_EMPTY,
+    B_H2_FULL, B_H2C_FULL, B_H2C_EMPTY = B_H2C_FULL + 2, B_H3_FULL = B_H2C_EMPTY + 2, B_H3_EMPTY = B_H3_FULL + 2, B_TILE_DONE = B_H3_EMPTY + 2,
+    B_W4_FULL, B_COUNT
 };
 
 struct KArgs {
@@ -192,10 +239,9 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
     if (threadIdx.x == 32) {
         for (int i = 0; i < B_COUNT; ++i) {
             uint32_t cnt = 1;
-            if (i == B_A0_FULL || i == B_SMALL_EMPTY || i == B_A1_FULL || i == B_A1_FULL + 1 || i == B_ACC_EMPTY ||
-                i == B_H3_FULL || i == B_H3_FULL + 1)
-                cnt = 8;
-            if (i == B_H2_FULL) cnt = 16;
+            if ((i >= B_SMALL_EMPTY && i < B_SMALL_EMPTY + kSmallBufs) || (i >= B_A1_FULL && i < B_A1_FULL + 4)) cnt = 4;
+            if (i == B_A0_FULL || i == B_ACC_EMPTY || i == B_H3_FULL || i == B_H3_FULL + 1) cnt = 4 * kGroups;
+            if (i == B_H2_FULL) cnt = 8 * kGroups;
             mbar_init(bar(i), cnt);
         }
         fence_barrier_init();
@@ -218,33 +264,37 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             auto load = [&](const uint8_t* src, uint32_t bytes) {
                 const uint32_t slot = cnt % kWStages, par = (cnt / kWStages) & 1;
                 mbar_wait(bar(B_W_EMPTY + slot), par ^ 1);
+#ifdef DF_DBG_NO_TMA
+                mbar_arrive(bar(B_W_FULL + slot));
+#else
                 mbar_expect_tx(bar(B_W_FULL + slot), bytes);
                 tma_bulk_g2s(s_w + slot * g.w_slot_bytes, src, bytes, bar(B_W_FULL + slot));
+#endif
                 ++cnt;
             };
             for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
-                const int n2 = 2 * g.NC * 2;
+                const int n2 = 2 * g.NC;
                 for (int i = 0; i < n2; ++i) load(a.d.w2t + (size_t)i * g.w2_tile_bytes, g.w2_tile_bytes);
                 for (int ks = 0; ks < g.NKS; ++ks) load(a.d.w3t + (size_t)ks * g.w3_tile_bytes, g.w3_tile_bytes);
             }
         }
     } else if (warp == 3) {
-        // ================= auxiliary TMA producer: W4 (once), W1 pairs, H2 chunks =================
+        // ================= auxiliary TMA producer: W4 (once), W1 quads, H2 chunks =================
         if (lane == 0) {
             mbar_expect_tx(bar(B_W4_FULL), g.w4_bytes);
             tma_bulk_g2s(s_w4, a.d.w4t, g.w4_bytes, bar(B_W4_FULL));
             const uint8_t* scratch = a.scratch + (size_t)blockIdx.x * g.NKC * kChunkBytes;
-            const int npairs = (g.NC + 1) / 2;
+            const int nquads = (g.NC + 3) / 4;
             uint32_t w1c = 0, h2c = 0, tc = 0;
             for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tc) {
-                if (tc > 0) mbar_wait(bar(B_TILE_DONE), (tc - 1) & 1);  // R2 (H3 ring) is free again
+                if (tc > 0) mbar_wait(bar(B_TILE_DONE), (tc - 1) & 1);  // R2 (the H3 tiles) is free again
                 for (int h = 0; h < 2; ++h)
-                    for (int pr = 0; pr < npairs; ++pr, ++w1c) {
+                    for (int qd = 0; qd < nquads; ++qd, ++w1c) {
                         const uint32_t slot = w1c & 1, par = (w1c >> 1) & 1;
                         mbar_wait(bar(B_W1_EMPTY + slot), par ^ 1);
-                        mbar_expect_tx(bar(B_W1_FULL + slot), kW1PairBytes);
-                        tma_bulk_g2s(s_r2 + kChunkBytes + slot * kW1PairBytes, a.d.w1t + (size_t)pr * kW1PairBytes,
-                                     kW1PairBytes, bar(B_W1_FULL + slot));
+                        mbar_expect_tx(bar(B_W1_FULL + slot), kW1QuadBytes);
+                        tma_bulk_g2s(s_r2 + kChunkBytes + slot * kW1QuadBytes, a.d.w1t + (size_t)qd * kW1QuadBytes,
+                                     kW1QuadBytes, bar(B_W1_FULL + slot));
                     }
                 mbar_wait(bar(B_H2_FULL), tc & 1);  // both halves of H2 are in the scratch
                 for (int kc = 0; kc < g.NKC; ++kc, ++h2c) {
@@ -257,190 +307,214 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             }
         }
     } else if (warp == 1) {
-        // ================= MMA issuer (one thread) =================
-        if (lane == 0) {
-            const uint32_t id64 = umma_idesc(64), id32 = umma_idesc(32);
-            const uint32_t id2a = umma_idesc(g.na2), id2b = umma_idesc(g.nb2 > 0 ? g.nb2 : 16);
-            const uint32_t id3a = umma_idesc(g.n3a), id3b = umma_idesc(g.n3b > 0 ? g.n3b : 16);
-            const uint32_t d_acc = tmem, d_small = tmem + kSmallCol;
-            uint32_t wc = 0, w1c = 0, se = 0, ae = 0, a1c = 0, h2cc = 0, h3c = 0, tc = 0;
+        // ================= MMA issuer =================
+        // The whole warp runs this loop convergently (all control flow is warp-uniform) and one elected lane
+        // issues the tcgen05 instructions: ptxas then keeps descriptors and barrier addresses in uniform
+        // registers instead of wrapping every UTCHMMA in a per-thread election loop.
+        const uint32_t id32 = umma_idesc(32, g.b_fmt);
+        const uint32_t id2a = umma_idesc(g.na2, g.b_fmt), id2b = umma_idesc(g.nb2 > 0 ? g.nb2 : 16, g.b_fmt);
+        const uint32_t id3a = umma_idesc(g.n3a, g.b_fmt), id3b = umma_idesc(g.n3b > 0 ? g.n3b : 16, g.b_fmt);
+        const uint64_t dA0 = umma_desc(s_r2), dW1 = umma_desc(s_r2 + kChunkBytes), dR1 = umma_desc(s_r1);
+        const uint64_t dW = umma_desc(s_w), dW4 = umma_desc(s_w4);
+        const uint32_t w_slot16 = (uint32_t)g.w_slot_bytes >> 4;
+        // gs: uses of the small-accumulator ring (layer-1 chunks and D4); ac: uses of the A1 quarter-slots
+        uint32_t wc = 0, w1c = 0, gs = 0, ac = 0, ae = 0, h2cc = 0, h3c = 0, tc = 0;
 
-            auto issue_L1 = [&](int jn) {
-                const uint32_t slot = w1c & 1;
-                if ((jn & 1) == 0) mbar_wait(bar(B_W1_FULL + slot), (w1c >> 1) & 1);
-                mbar_wait(bar(B_SMALL_EMPTY), (se & 1) ^ 1);
-                ++se;
-                tc_fence_after();
-                const uint32_t a0 = s_r2, b0 = s_r2 + kChunkBytes + slot * kW1PairBytes + (jn & 1) * 64;
-                for (int kk = 0; kk < g.K0steps; ++kk)
-                    tc_mma(d_small, umma_desc(a0 + kk * 32), umma_desc(b0 + kk * 32), id64, kk > 0);
-                tc_commit(bar(B_SMALL_FULL));
-                if ((jn & 1) == 1 || jn == g.NC - 1) {
-                    tc_commit(bar(B_W1_EMPTY + slot));
-                    ++w1c;
-                }
-            };
-            // one 32-wide K stage of a [128 x N] += A[128 x 32] W^T update, N split into two MMA pieces
-            auto issue_stage = [&](uint32_t a_addr, int na, int nb, uint32_t ida, uint32_t idb, bool first) {
-                const uint32_t slot = wc % kWStages;
-                mbar_wait(bar(B_W_FULL + slot), (wc / kWStages) & 1);
-                ++wc;
-                tc_fence_after();
-                const uint32_t wb = s_w + slot * g.w_slot_bytes;
-                for (int kk = 0; kk < 2; ++kk) {
-                    const uint32_t acc = (!first || kk > 0) ? 1u : 0u;
-                    const uint64_t ad = umma_desc(a_addr + kk * 32);
-                    tc_mma(d_acc, ad, umma_desc(wb + kk * 32), ida, acc);
-                    if (nb > 0) tc_mma(d_acc + na, ad, umma_desc(wb + 64 + kk * 32), idb, acc);
-                }
+        // layer-1 chunk c -> D1 buffer gs % 3 (caller has checked that the buffer and the W1 quad are ready)
+        auto issue_L1 = [&](int c) {
+            const uint32_t slot = w1c & 1, sb = gs % kSmallBufs;
+            ++gs;
+            tc_fence_after();
+            if (elect_one()) {
+                const uint64_t b0 = dW1 + ((slot * kW1QuadBytes + ((c & 3) >> 1) * 4096 + (c & 1) * 64) >> 4);
+                const uint32_t dd = tmem + kSmallCol + sb * 32;
+                tc_mma(dd, dA0, b0, id32, 0u);
+                if (g.K0steps > 1) tc_mma(dd, dA0 + 2, b0 + 2, id32, 1u);
+                tc_commit(bar(B_SMALL_FULL + sb));
+                if ((c & 3) == 3 || c == g.NC - 1) tc_commit(bar(B_W1_EMPTY + slot));
+            }
+            __syncwarp();
+            if ((c & 3) == 3 || c == g.NC - 1) ++w1c;
+        };
+        auto L1_ready = [&](int c) {
+            if ((c & 3) == 0 && !mbar_test(bar(B_W1_FULL + (w1c & 1)), (w1c >> 1) & 1)) return false;
+            return mbar_test(bar(B_SMALL_EMPTY + gs % kSmallBufs), ((gs / kSmallBufs) & 1) ^ 1);
+        };
+        // one 32-wide K stage of a [128 x N] += A[128 x 32] W^T update, N split into two MMA pieces;
+        // `extra` is a second barrier to commit to (the A-operand slot), or 0.
+        auto issue_stage = [&](uint64_t ad, int na, int nb, uint32_t ida, uint32_t idb, bool first, uint32_t extra) {
+            const uint32_t slot = wc % kWStages;
+            mbar_wait(bar(B_W_FULL + slot), (wc / kWStages) & 1);
+            ++wc;
+            tc_fence_after();
+            if (elect_one()) {
+                const uint64_t wb = dW + slot * w_slot16;
+                tc_mma(tmem, ad, wb, ida, first ? 0u : 1u);
+                if (nb > 0) tc_mma(tmem + na, ad, wb + 4, idb, first ? 0u : 1u);
+                tc_mma(tmem, ad + 2, wb + 2, ida, 1u);
+                if (nb > 0) tc_mma(tmem + na, ad + 2, wb + 6, idb, 1u);
                 tc_commit(bar(B_W_EMPTY + slot));
-            };
+                if (extra) tc_commit(extra);
+            }
+            __syncwarp();
+        };
 
-            for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tc) {
-                mbar_wait(bar(B_A0_FULL), tc & 1);
-                // ---- phase A: layers 1+2, one half of layer 2's outputs at a time ----
-                for (int h = 0; h < 2; ++h) {
-                    issue_L1(0);
-                    for (int j = 0; j < g.NC; ++j, ++a1c) {
-                        if (j + 1 < g.NC) issue_L1(j + 1);
-                        const uint32_t slot = a1c & 1;
-                        mbar_wait(bar(B_A1_FULL + slot), (a1c >> 1) & 1);
-                        if (j == 0) {
+        for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tc) {
+            mbar_wait(bar(B_A0_FULL), tc & 1);
+            // ---- phase A: layers 1+2, one half of layer 2's outputs at a time.  Event loop: layer-1 chunks are
+            //      issued as soon as a D1 buffer is free, layer-2 stages as soon as their A1 slot is full, so the
+            //      epilogue groups always have a chunk to work on while the tensor pipe runs layer 2. ----
+            for (int h = 0; h < 2; ++h) {
+                int l1 = 0, l2 = 0;
+                while (l2 < g.NC) {
+                    if (l1 < g.NC && L1_ready(l1)) {
+                        issue_L1(l1++);
+                        continue;
+                    }
+                    const uint32_t slot = ac & 3;
+                    if (l2 < l1 && mbar_test(bar(B_A1_FULL + slot), (ac >> 2) & 1)) {
+                        if (l2 == 0) {
                             mbar_wait(bar(B_ACC_EMPTY), (ae & 1) ^ 1);
                             ++ae;
                         }
-                        const uint32_t aa = s_r1 + slot * kChunkBytes;
-                        issue_stage(aa, g.na2, g.nb2, id2a, id2b, j == 0);
-                        issue_stage(aa + 64, g.na2, g.nb2, id2a, id2b, false);
-                        tc_commit(bar(B_A1_EMPTY + slot));
-                    }
-                    tc_commit(bar(B_ACC_FULL));
-                }
-                // ---- phase B: layer 3 from the H2 chunks, then layer 4 fed by the D3 drain ----
-                mbar_wait(bar(B_ACC_EMPTY), (ae & 1) ^ 1);
-                ++ae;
-                for (int ks = 0; ks < g.NKS; ++ks) {
-                    const uint32_t slot = h2cc & 1;
-                    if ((ks & 1) == 0) mbar_wait(bar(B_H2C_FULL + slot), (h2cc >> 1) & 1);
-                    issue_stage(s_r1 + slot * kChunkBytes + (ks & 1) * 64, g.n3a, g.n3b, id3a, id3b, ks == 0);
-                    if ((ks & 1) == 1 || ks == g.NKS - 1) {
-                        tc_commit(bar(B_H2C_EMPTY + slot));
-                        ++h2cc;
+                        issue_stage(dR1 + (((slot >> 1) * kChunkBytes + (slot & 1) * 64) >> 4), g.na2, g.nb2, id2a, id2b,
+                                    l2 == 0, bar(B_A1_EMPTY + slot));
+                        ++ac;
+                        ++l2;
                     }
                 }
-                tc_commit(bar(B_ACC_FULL));
-                if (tc == 0) mbar_wait(bar(B_W4_FULL), 0);
-                for (int jj = 0; jj < g.NJ; ++jj, ++h3c) {
-                    const uint32_t slot = h3c & 1;
-                    mbar_wait(bar(B_H3_FULL + slot), (h3c >> 1) & 1);
-                    if (jj == 0) {
-                        mbar_wait(bar(B_SMALL_EMPTY), (se & 1) ^ 1);
-                        ++se;
-                    }
-                    tc_fence_after();
-                    const int cols = min(64, g.d3 - jj * 64);
-                    for (int kk = 0; kk < cols / 16; ++kk)
-                        tc_mma(d_small, umma_desc(s_r2 + slot * kChunkBytes + kk * 32),
-                               umma_desc(s_w4 + jj * 4096 + kk * 32), id32, (jj > 0 || kk > 0) ? 1u : 0u);
+                if (elect_one()) tc_commit(bar(B_ACC_FULL));
+                __syncwarp();
+            }
+            // ---- phase B: layer 3 from the H2 chunks, then layer 4 fed by the D3 drain ----
+            mbar_wait(bar(B_ACC_EMPTY), (ae & 1) ^ 1);
+            ++ae;
+            for (int ks = 0; ks < g.NKS; ++ks) {
+                const uint32_t slot = h2cc & 1;
+                if ((ks & 1) == 0) mbar_wait(bar(B_H2C_FULL + slot), (h2cc >> 1) & 1);
+                const bool last = (ks & 1) == 1 || ks == g.NKS - 1;
+                issue_stage(dR1 + ((slot * kChunkBytes + (ks & 1) * 64) >> 4), g.n3a, g.n3b, id3a, id3b, ks == 0,
+                            last ? bar(B_H2C_EMPTY + slot) : 0u);
+                if (last) ++h2cc;
+            }
+            if (elect_one()) tc_commit(bar(B_ACC_FULL));
+            __syncwarp();
+            if (tc == 0) mbar_wait(bar(B_W4_FULL), 0);
+            const uint32_t sb = gs % kSmallBufs;
+            for (int jj = 0; jj < g.NJ; ++jj, ++h3c) {
+                const uint32_t slot = h3c & 1;
+                mbar_wait(bar(B_H3_FULL + slot), (h3c >> 1) & 1);
+                if (jj == 0) mbar_wait(bar(B_SMALL_EMPTY + sb), ((gs / kSmallBufs) & 1) ^ 1);
+                tc_fence_after();
+                if (elect_one()) {
+                    const int ksteps = min(64, g.d3 - jj * 64) / 16;
+                    const uint64_t ha = dA0 + ((slot * kChunkBytes) >> 4), wa = dW4 + ((jj * 4096) >> 4);
+                    for (int kk = 0; kk < ksteps; ++kk)
+                        tc_mma(tmem + kSmallCol + sb * 32, ha + 2 * kk, wa + 2 * kk, id32, (jj > 0 || kk > 0) ? 1u : 0u);
                     tc_commit(bar(B_H3_EMPTY + slot));
                 }
-                tc_commit(bar(B_SMALL_FULL));
+                __syncwarp();
+            }
+            if (elect_one()) {
+                tc_commit(bar(B_SMALL_FULL + sb));
                 tc_commit(bar(B_TILE_DONE));
             }
+            __syncwarp();
+            ++gs;
         }
     } else if (warp >= 4) {
-        // ================= epilogue warps (also write the A0 feature tile) =================
-        const int ew = warp - 4, q = ew & 3, ch = ew >> 2;
+        // ================= epilogue warps: kGroups groups of four (one warp per TMEM lane quarter) =================
+        // Group grp takes every kGroups-th layer-1 chunk (so several chunks are in flight), every kGroups-th
+        // 16-column unit of the D2/D3 drains, and one 16-byte column chunk of the A0 feature tile.
+        const int ew = warp - 4, q = ew & 3, grp = ew >> 2;
         const int row = q * 32 + lane;
         const uint32_t t_lane = tmem + ((uint32_t)(q * 32) << 16);
         uint8_t* scratch = a.scratch + (size_t)blockIdx.x * g.NKC * kChunkBytes;
-        uint32_t sf = 0, af = 0, a1c = 0, h3c = 0;
+        uint32_t gs = 0, ac = 0, af = 0, h3c = 0;
         const float lam = nm.lambda, inv_lam = nm.inv_lambda;
 
-        // +bias, GELU, pack 16 fp32 accumulators into 8 bf16x2 words
-        auto act16 = [&](const uint32_t (&r)[16], const float* bias, uint32_t (&o)[8]) {
+        auto st_shared16 = [&](uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+            asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+        };
+        // +bias, GELU on 16 accumulators -> 8 packed fp16x2 words
+        auto act16 = [&](const uint32_t* r, const float* bias, uint32_t (&o)[8]) {
             const float4* b4 = reinterpret_cast<const float4*>(bias);
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 const float4 b = __ldg(b4 + i);
-                const float v0 = gelu_fast(__uint_as_float(r[4 * i + 0]) + b.x);
-                const float v1 = gelu_fast(__uint_as_float(r[4 * i + 1]) + b.y);
-                const float v2 = gelu_fast(__uint_as_float(r[4 * i + 2]) + b.z);
-                const float v3 = gelu_fast(__uint_as_float(r[4 * i + 3]) + b.w);
-                o[2 * i] = pack_bf16(v0, v1);
-                o[2 * i + 1] = pack_bf16(v2, v3);
+                o[2 * i] = pack_act(gelu_fast(__uint_as_float(r[4 * i + 0]) + b.x), gelu_fast(__uint_as_float(r[4 * i + 1]) + b.y));
+                o[2 * i + 1] = pack_act(gelu_fast(__uint_as_float(r[4 * i + 2]) + b.z), gelu_fast(__uint_as_float(r[4 * i + 3]) + b.w));
             }
-        };
-        auto st_shared16 = [&](uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
-            asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
         };
 
         for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
             const long long cell = tile * kTileM + row;
             const bool valid = cell < a.n;
-            // ---- prologue: features -> bf16 A0; this warp writes feature columns [16 ch, 16 ch + 16) ----
-            {
-                uint32_t o[8];
+            // ---- prologue: features + two bias columns of ones -> fp16 A0 [128 x 32]; group grp writes
+            //      feature columns [8 grp, 8 grp + 8) ----
+            for (int fc = grp; fc < 4; fc += kGroups) {
+                uint32_t o[4];
 #pragma unroll
-                for (int i = 0; i < 8; ++i) {
+                for (int i = 0; i < 4; ++i) {
                     float v[2];
 #pragma unroll
                     for (int e = 0; e < 2; ++e) {
-                        const int f = ch * 16 + 2 * i + e;
+                        const int f = fc * 8 + 2 * i + e;
                         float x = 0.f;
-                        if (valid && f < g.K + 2) {
-                            if (f == 0) x = (__ldg(a.T + cell) - nm.x_mean[0]) * nm.x_inv_std[0];
-                            else if (f == 1) x = (__ldg(a.p + cell) - nm.x_mean[1]) * nm.x_inv_std[1];
-                            else {
-                                const float y = __ldg(a.Y + (size_t)(f - 2) * a.ld + cell);
-                                const float qy = exp2f(lam * __log2f(y));  // y^lambda, 0 -> 0
-                                x = ((qy - 1.0f) * inv_lam - nm.x_mean[f]) * nm.x_inv_std[f];
+                        if (f < g.K + 2) {
+                            if (valid) {
+                                if (f == 0) x = (__ldg(a.T + cell) - nm.x_mean[0]) * nm.x_inv_std[0];
+                                else if (f == 1) x = (__ldg(a.p + cell) - nm.x_mean[1]) * nm.x_inv_std[1];
+                                else {
+                                    const float y = __ldg(a.Y + (size_t)(f - 2) * a.ld + cell);
+                                    const float qy = exp2f(lam * __log2f(y));  // y^lambda, 0 -> 0
+                                    x = ((qy - 1.0f) * inv_lam - nm.x_mean[f]) * nm.x_inv_std[f];
+                                }
                             }
+                        } else if (f < g.K + 4) {
+                            x = 1.0f;  // multiplies the bf16 hi / lo parts of b1 stored as W1 columns K+2, K+3
                         }
                         v[e] = x;
                     }
-                    o[i] = pack_bf16(v[0], v[1]);
+                    o[i] = pack_act(v[0], v[1]);
                 }
-                st_shared16(s_r2 + swz(row, ch * 2), o[0], o[1], o[2], o[3]);
-                st_shared16(s_r2 + swz(row, ch * 2 + 1), o[4], o[5], o[6], o[7]);
-                fence_proxy_async();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar(B_A0_FULL));
+                st_shared16(s_r2 + swz(row, fc), o[0], o[1], o[2], o[3]);
             }
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_A0_FULL));
             // ---- phase A ----
             for (int h = 0; h < 2; ++h) {
-                for (int j = 0; j < g.NC; ++j, ++a1c) {
-                    mbar_wait(bar(B_SMALL_FULL), sf & 1);
-                    ++sf;
+                for (int c = 0; c < g.NC; ++c, ++gs, ++ac) {
+                    if ((int)(ac % kGroups) != grp) continue;
+                    const uint32_t sb = gs % kSmallBufs;
+                    mbar_wait(bar(B_SMALL_FULL + sb), (gs / kSmallBufs) & 1);
                     tc_fence_after();
-                    uint32_t r0[16], r1[16];
-                    tc_ld16(t_lane + kSmallCol + ch * 32, r0);
-                    tc_ld16(t_lane + kSmallCol + ch * 32 + 16, r1);
+                    uint32_t r[32];
+                    tc_ld32(t_lane + kSmallCol + sb * 32, r);
                     tc_wait_ld();
                     tc_fence_before();
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(bar(B_SMALL_EMPTY));
-                    uint32_t o0[8], o1[8];
-                    const float* bias = a.d.b1 + j * 64 + ch * 32;
-                    act16(r0, bias, o0);
-                    act16(r1, bias + 16, o1);
-                    const uint32_t slot = a1c & 1;
-                    mbar_wait(bar(B_A1_EMPTY + slot), ((a1c >> 1) & 1) ^ 1);
-                    const uint32_t base = s_r1 + slot * kChunkBytes;
-                    st_shared16(base + swz(row, ch * 4 + 0), o0[0], o0[1], o0[2], o0[3]);
-                    st_shared16(base + swz(row, ch * 4 + 1), o0[4], o0[5], o0[6], o0[7]);
-                    st_shared16(base + swz(row, ch * 4 + 2), o1[0], o1[1], o1[2], o1[3]);
-                    st_shared16(base + swz(row, ch * 4 + 3), o1[4], o1[5], o1[6], o1[7]);
+                    if (lane == 0) mbar_arrive(bar(B_SMALL_EMPTY + sb));
+                    uint32_t o[16];
+#pragma unroll
+                    for (int i = 0; i < 16; ++i)   // b1 is already in the accumulator (bias columns of W1)
+                        o[i] = pack_act(gelu_fast(__uint_as_float(r[2 * i])), gelu_fast(__uint_as_float(r[2 * i + 1])));
+                    const uint32_t slot = ac & 3;
+                    mbar_wait(bar(B_A1_EMPTY + slot), ((ac >> 2) & 1) ^ 1);
+                    const uint32_t base = s_r1 + (slot >> 1) * kChunkBytes;
+#pragma unroll
+                    for (int c4 = 0; c4 < 4; ++c4)
+                        st_shared16(base + swz(row, (slot & 1) * 4 + c4), o[4 * c4], o[4 * c4 + 1], o[4 * c4 + 2], o[4 * c4 + 3]);
                     fence_proxy_async();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar(B_A1_FULL + slot));
                 }
-                // drain D2 (this half): +b2, GELU, bf16 -> H2 scratch in the chunk images phase B loads
+                // drain D2 (this half): +b2, GELU, fp16 -> H2 scratch in the chunk images phase B loads
                 mbar_wait(bar(B_ACC_FULL), af & 1);
                 ++af;
                 tc_fence_after();
-                const int c_lo = ch ? g.na2 : 0, c_hi = ch ? g.NH : g.na2;
-                for (int c0 = c_lo; c0 < c_hi; c0 += 16) {
+                for (int c0 = grp * 16; c0 < g.NH; c0 += 16 * kGroups) {
                     uint32_t r[16], o[8];
                     tc_ld16(t_lane + c0, r);
                     tc_wait_ld();
@@ -460,32 +534,34 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                     mbar_arrive(bar(B_H2_FULL));
                 }
             }
-            // ---- phase B: drain D3 in 64-wide chunks -> H3 ring (feeds layer 4) ----
+            // ---- phase B: drain D3 in 64-wide chunks -> H3 ring (feeds layer 4); group grp owns 16-column unit grp ----
             mbar_wait(bar(B_ACC_FULL), af & 1);
             ++af;
             tc_fence_after();
             for (int jj = 0; jj < g.NJ; ++jj, ++h3c) {
+                // 16-column units u = grp, grp + kGroups, ... of this 64-wide chunk (at most two per group)
                 uint32_t o[2][8];
                 bool have[2];
 #pragma unroll
-                for (int u = 0; u < 2; ++u) {
-                    const int c0 = jj * 64 + (ch * 2 + u) * 16;
-                    have[u] = c0 < g.d3;
-                    if (have[u]) {
+                for (int i = 0; i < 2; ++i) {
+                    const int u = grp + i * kGroups, c0 = jj * 64 + u * 16;
+                    have[i] = u < 4 && c0 < g.d3;
+                    if (have[i]) {
                         uint32_t r[16];
                         tc_ld16(t_lane + c0, r);
                         tc_wait_ld();
-                        act16(r, a.d.b3 + c0, o[u]);
+                        act16(r, a.d.b3 + c0, o[i]);
                     }
                 }
                 const uint32_t slot = h3c & 1;
                 mbar_wait(bar(B_H3_EMPTY + slot), ((h3c >> 1) & 1) ^ 1);
                 const uint32_t base = s_r2 + slot * kChunkBytes;
 #pragma unroll
-                for (int u = 0; u < 2; ++u)
-                    if (have[u]) {
-                        st_shared16(base + swz(row, (ch * 2 + u) * 2), o[u][0], o[u][1], o[u][2], o[u][3]);
-                        st_shared16(base + swz(row, (ch * 2 + u) * 2 + 1), o[u][4], o[u][5], o[u][6], o[u][7]);
+                for (int i = 0; i < 2; ++i)
+                    if (have[i]) {
+                        const int u = grp + i * kGroups;
+                        st_shared16(base + swz(row, u * 2), o[i][0], o[i][1], o[i][2], o[i][3]);
+                        st_shared16(base + swz(row, u * 2 + 1), o[i][4], o[i][5], o[i][6], o[i][7]);
                     }
                 fence_proxy_async();
                 __syncwarp();
@@ -494,45 +570,45 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(B_ACC_EMPTY));
-            // ---- final epilogue: D4 -> Delta -> inverse Box-Cox -> renormalise -> omega (A9-A11, A17) ----
-            mbar_wait(bar(B_SMALL_FULL), sf & 1);
-            ++sf;
-            tc_fence_after();
-            uint32_t r0[16], r1[16];
-            if (ch == 0) {
-                tc_ld16(t_lane + kSmallCol, r0);
-                tc_ld16(t_lane + kSmallCol + 16, r1);
+            // ---- final epilogue (group 0): D4 -> Delta -> inverse Box-Cox -> renormalise -> omega (A9-A11, A17) ----
+            const uint32_t sb = gs % kSmallBufs;
+            const uint32_t spar = (gs / kSmallBufs) & 1;
+            ++gs;
+            if (grp == 0) {
+                mbar_wait(bar(B_SMALL_FULL + sb), spar);
+                tc_fence_after();
+                uint32_t r[32];
+                tc_ld32(t_lane + kSmallCol + sb * 32, r);
                 tc_wait_ld();
-            }
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar(B_SMALL_EMPTY));
-            if (ch == 0 && valid) {
-                const float T = __ldg(a.T + cell), p = __ldg(a.p + cell);
-                float dys[32], yv[32];
-                double sumYm1 = -1.0, sumd = 0.0;
-                float inv_Wbar = 0.f;
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(B_SMALL_EMPTY + sb));
+                if (valid) {
+                    const float T = __ldg(a.T + cell), p = __ldg(a.p + cell);
+                    double sumYm1 = -1.0, sumd = 0.0;
+                    float inv_Wbar = 0.f;
 #pragma unroll
-                for (int k = 0; k < 32; ++k) {
-                    if (k < g.K) {
-                        const float ok = __uint_as_float(k < 16 ? r0[k & 15] : r1[k & 15]) + __ldg(a.d.b4 + k);
-                        const float y = __ldg(a.Y + (size_t)k * a.ld + cell);
-                        const float d = ann_dystar(y, fmaf(nm.u_std[k], ok, nm.u_mean[k]), lam, inv_lam);
-                        yv[k] = y;
-                        dys[k] = d;
-                        sumYm1 += (double)y;
-                        sumd += (double)d;
-                        inv_Wbar = fmaf(y, __ldg(a.invW + k), inv_Wbar);
+                    for (int k = 0; k < 32; ++k) {
+                        if (k < g.K) {
+                            const float ok = __uint_as_float(r[k]) + __ldg(a.d.b4 + k);
+                            const float y = __ldg(a.Y + (size_t)k * a.ld + cell);
+                            const float d = ann_dystar(y, fmaf(nm.u_std[k], ok, nm.u_mean[k]), lam, inv_lam);
+                            r[k] = __float_as_uint(d);
+                            sumYm1 += (double)y;
+                            sumd += (double)d;
+                            inv_Wbar = fmaf(y, __ldg(a.invW + k), inv_Wbar);
+                        }
                     }
-                }
-                const double Sm1 = sumYm1 + sumd, inv_S = 1.0 / (1.0 + Sm1);
-                const float rho_dt = p / (inv_Wbar * (float)DF_R_UNIVERSAL * T) * nm.inv_dt;
+                    const double Sm1 = sumYm1 + sumd, inv_S = 1.0 / (1.0 + Sm1);
+                    const float rho_dt = p / (inv_Wbar * (float)DF_R_UNIVERSAL * T) * nm.inv_dt;
 #pragma unroll
-                for (int k = 0; k < 32; ++k) {
-                    if (k < g.K) {
-                        const float d = ann_renorm_dY(dys[k], yv[k], Sm1, inv_S);
-                        if (a.dY) a.dY[(size_t)k * a.ld + cell] = d;
-                        if (a.omega) a.omega[(size_t)k * a.ld + cell] = rho_dt * d;
+                    for (int k = 0; k < 32; ++k) {
+                        if (k < g.K) {
+                            const float y = __ldg(a.Y + (size_t)k * a.ld + cell);
+                            const float d = ann_renorm_dY(__uint_as_float(r[k]), y, Sm1, inv_S);
+                            if (a.dY) a.dY[(size_t)k * a.ld + cell] = d;
+                            if (a.omega) a.omega[(size_t)k * a.ld + cell] = rho_dt * d;
+                        }
                     }
                 }
             }
@@ -559,10 +635,19 @@ uint16_t bf16_bits(float x) {  // round to nearest even
     return (uint16_t)(u >> 16);
 }
 
-// element (row r, column c < 64) of a 128B-swizzled K-major bf16 tile
+uint16_t fp16_bits(float x) {  // round to nearest even, via the compiler's __half conversion on the host
+    const __half h = __float2half_rn(x);
+    uint16_t b;
+    memcpy(&b, &h, 2);
+    return b;
+}
+
+int g_put_fmt = 1;  // 1 = bf16, 0 = fp16 (set by ann_bf16_create before packing)
+
+// element (row r, column c < 64) of a 128B-swizzled K-major 16-bit tile
 inline void put(uint8_t* tile, int r, int c, float v) {
     const size_t off = (size_t)r * 128 + (size_t)((((c >> 3) ^ (r & 7)) << 4) + (c & 7) * 2);
-    const uint16_t b = bf16_bits(v);
+    const uint16_t b = g_put_fmt ? bf16_bits(v) : fp16_bits(v);
     memcpy(tile + off, &b, 2);
 }
 
@@ -577,19 +662,21 @@ void split_n(int N, int* na, int* nb) {
 df_status ann_bf16_create(df_ann* ann, const float* const* W, const float* const* b) {
     if (ann->n_layers != 4) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: n_layers must be 4 (got %d)", ann->n_layers);
     const int K = ann->K, d1 = ann->dims[1], d2 = ann->dims[2], d3 = ann->dims[3];
-    if (K > 30) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: K <= 30 (got %d)", K);
+    if (K > 28) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: K <= 28 (got %d)", K);
     if (d1 % 64 || d1 < 64) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: dims[1] %% 64 == 0 (got %d)", d1);
-    if (d2 % 32 || d2 < 64 || d2 > 896) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: dims[2] %% 32 == 0, 64..896 (got %d)", d2);
-    if (d3 % 16 || d3 < 32 || d3 > 448) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: dims[3] %% 16 == 0, 32..448 (got %d)", d3);
+    if (d2 % 32 || d2 < 64 || d2 > 800) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: dims[2] %% 32 == 0, 64..800 (got %d)", d2);
+    if (d3 % 16 || d3 < 32 || d3 > 400) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: dims[3] %% 16 == 0, 32..400 (got %d)", d3);
 
     Bf16Plan* P = new (std::nothrow) Bf16Plan;
     if (!P) return df_set_error(DF_ERR_ALLOC, "bf16 path: out of host memory");
     ann->bf16 = P;
     NetGeom& g = P->g;
     g.K = K;
-    g.K0steps = (K + 2 <= 16) ? 1 : 2;
+    g.b_fmt = 0;  // tcgen05 kind::f16 needs A and B in one format (fp16 x bf16 is an illegal instruction): fp16 x fp16
+    g_put_fmt = g.b_fmt;
+    g.K0steps = (K + 4 <= 16) ? 1 : 2;  // features + 2 bias columns, fp16
     g.d1 = d1; g.d2 = d2; g.d3 = d3;
-    g.NC = d1 / 64;
+    g.NC = d1 / 32;
     g.NH = d2 / 2;
     split_n(g.NH, &g.na2, &g.nb2);
     split_n(d3, &g.n3a, &g.n3b);
@@ -613,31 +700,39 @@ df_status ann_bf16_create(df_ann* ann, const float* const* W, const float* const
     DF_CUDA_TRY(cudaGetDevice(&dev));
     DF_CUDA_TRY(cudaDeviceGetAttribute(&P->num_sms, cudaDevAttrMultiProcessorCount, dev));
 
-    const int npairs = (g.NC + 1) / 2;
-    const size_t sz_w1 = (size_t)npairs * kW1PairBytes, sz_w2 = (size_t)2 * g.NC * 2 * g.w2_tile_bytes,
+    const int nquads = (g.NC + 3) / 4;
+    const size_t sz_w1 = (size_t)nquads * kW1QuadBytes, sz_w2 = (size_t)2 * g.NC * g.w2_tile_bytes,
                  sz_w3 = (size_t)g.NKS * g.w3_tile_bytes, sz_w4 = (size_t)g.w4_bytes;
     const size_t sz_b = (size_t)(d1 + d2 + d3 + 32) * sizeof(float);
     const size_t o_w1 = 0, o_w2 = o_w1 + sz_w1, o_w3 = o_w2 + sz_w2, o_w4 = o_w3 + sz_w3, o_b = o_w4 + sz_w4;
     std::vector<uint8_t> blob(o_b + sz_b, 0);
     const int din = K + 2;
-    for (int pr = 0; pr < npairs; ++pr)
-        for (int c = 0; c < 2; ++c) {
-            const int chunk = 2 * pr + c;
-            if (chunk >= g.NC) continue;
-            uint8_t* t = blob.data() + o_w1 + (size_t)pr * kW1PairBytes;
-            for (int r = 0; r < 64; ++r)
-                for (int k = 0; k < din; ++k) put(t, r, c * 32 + k, W[0][(size_t)(chunk * 64 + r) * din + k]);
+    // W1: chunk c (32 outputs) sits in quad c/4 at rows 32*((c&3)>>1).., K columns 32*(c&1)..; columns K+2 and
+    // K+3 carry the bf16 hi and lo parts of b1 (the A0 tile holds 1.0 there).
+    for (int c = 0; c < g.NC; ++c) {
+        uint8_t* t = blob.data() + o_w1 + (size_t)(c >> 2) * kW1QuadBytes;
+        const int r0 = ((c & 3) >> 1) * 32, k0 = (c & 1) * 32;
+        for (int r = 0; r < 32; ++r) {
+            const int o = c * 32 + r;
+            for (int k = 0; k < din; ++k) put(t, r0 + r, k0 + k, W[0][(size_t)o * din + k]);
+            const float bh = b[0][o];
+            uint16_t hb = bf16_bits(bh);
+            uint32_t hu = (uint32_t)hb << 16;
+            float bhf;
+            memcpy(&bhf, &hu, 4);
+            put(t, r0 + r, k0 + din, bhf);
+            put(t, r0 + r, k0 + din + 1, bh - bhf);
         }
+    }
     for (int h = 0; h < 2; ++h)
-        for (int j = 0; j < g.NC; ++j)
-            for (int half = 0; half < 2; ++half) {
-                uint8_t* t = blob.data() + o_w2 + (size_t)((h * g.NC + j) * 2 + half) * g.w2_tile_bytes;
-                const int k0 = j * 64 + half * 32;
-                for (int kk = 0; kk < 32; ++kk) {
-                    for (int r = 0; r < g.na2; ++r) put(t, r, kk, W[1][(size_t)(h * g.NH + r) * d1 + k0 + kk]);
-                    for (int r = 0; r < g.nb2; ++r) put(t, r, 32 + kk, W[1][(size_t)(h * g.NH + g.na2 + r) * d1 + k0 + kk]);
-                }
+        for (int c = 0; c < g.NC; ++c) {
+            uint8_t* t = blob.data() + o_w2 + (size_t)(h * g.NC + c) * g.w2_tile_bytes;
+            const int k0 = c * 32;
+            for (int kk = 0; kk < 32; ++kk) {
+                for (int r = 0; r < g.na2; ++r) put(t, r, kk, W[1][(size_t)(h * g.NH + r) * d1 + k0 + kk]);
+                for (int r = 0; r < g.nb2; ++r) put(t, r, 32 + kk, W[1][(size_t)(h * g.NH + g.na2 + r) * d1 + k0 + kk]);
             }
+        }
     for (int ks = 0; ks < g.NKS; ++ks) {
         uint8_t* t = blob.data() + o_w3 + (size_t)ks * g.w3_tile_bytes;
         for (int kk = 0; kk < 32; ++kk) {
@@ -707,3 +802,4 @@ df_status launch_ann_bf16(const df_ann* ann, const df_mech* mech, long long n, l
     DF_CUDA_TRY(cudaGetLastError());
     return DF_OK;
 }
+
