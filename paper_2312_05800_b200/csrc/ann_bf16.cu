@@ -41,7 +41,9 @@ constexpr int kTileM = 128;
 #endif
 constexpr int kGroups = KGROUPS;                  // epilogue groups of 4 warps (one warp per TMEM lane quarter)
 constexpr int kThreads = 128 + kGroups * 128;
-constexpr int kWStages = 5;
+constexpr int kWStages = 4;
+constexpr int kA1Tiles = 3;                 // [128 x 64] activation tiles of the A1 ring = 2 * kA1Tiles 32-column slots
+constexpr int kA1Slots = 2 * kA1Tiles;
 constexpr int kChunkBytes = kTileM * 128;  // one [128 x 64] bf16 K-major swizzled operand tile
 constexpr int kW1QuadBytes = 64 * 128;     // four 32-row layer-1 chunks: [2 x 32 rows] x [2 x 32 K] bf16
 constexpr int kSmallCol = 400;             // TMEM columns [400, 496): three 32-column D1 buffers (D4 reuses the first)
@@ -112,7 +114,8 @@ __device__ __forceinline__ void tma_bulk_g2s(uint32_t dst, const void* src, uint
                  "l"(src), "r"(bytes), "r"(bar)
                  : "memory");
 }
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }  // all state spaces (global scratch)
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -207,7 +210,7 @@ __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&r)[32]) {
 enum {
     B_W_FULL = 0, B_W_EMPTY = B_W_FULL + kWStages, B_W1_FULL = B_W_EMPTY + kWStages, B_W1_EMPTY = B_W1_FULL + 2,
     B_A0_FULL = B_W1_EMPTY + 2, B_SMALL_FULL, B_SMALL_EMPTY = B_SMALL_FULL + kSmallBufs,
-    B_A1_FULL = B_SMALL_EMPTY + kSmallBufs, B_A1_EMPTY = B_A1_FULL + 4, B_ACC_FULL = B_A1_EMPTY + 4, B_ACC_EMPTY,
+    B_A1_FULL = B_SMALL_EMPTY + kSmallBufs, B_A1_EMPTY = B_A1_FULL + kA1Slots, B_ACC_FULL = B_A1_EMPTY + kA1Slots, B_ACC_EMPTY,
     B_H2_FULL, B_H2C_FULL, B_H2C_EMPTY = B_H2C_FULL + 2, B_H3_FULL = B_H2C_EMPTY + 2, B_H3_EMPTY = B_H3_FULL + 2, B_TILE_DONE = B_H3_EMPTY + 2,
     B_W4_FULL, B_COUNT
 };
@@ -239,7 +242,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
     if (threadIdx.x == 32) {
         for (int i = 0; i < B_COUNT; ++i) {
             uint32_t cnt = 1;
-            if ((i >= B_SMALL_EMPTY && i < B_SMALL_EMPTY + kSmallBufs) || (i >= B_A1_FULL && i < B_A1_FULL + 4)) cnt = 4;
+            if ((i >= B_SMALL_EMPTY && i < B_SMALL_EMPTY + kSmallBufs) || (i >= B_A1_FULL && i < B_A1_FULL + kA1Slots)) cnt = 4;
             if (i == B_A0_FULL || i == B_ACC_EMPTY || i == B_H3_FULL || i == B_H3_FULL + 1) cnt = 4 * kGroups;
             if (i == B_H2_FULL) cnt = 8 * kGroups;
             mbar_init(bar(i), cnt);
@@ -273,9 +276,9 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                 ++cnt;
             };
             for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
-                const int n2 = 2 * g.NC;
+                const int n2 = 2 * (g.NC + 1);  // per half: the bias tile, then one tile per layer-1 chunk
                 for (int i = 0; i < n2; ++i) load(a.d.w2t + (size_t)i * g.w2_tile_bytes, g.w2_tile_bytes);
-                for (int ks = 0; ks < g.NKS; ++ks) load(a.d.w3t + (size_t)ks * g.w3_tile_bytes, g.w3_tile_bytes);
+                for (int ks = 0; ks <= g.NKS; ++ks) load(a.d.w3t + (size_t)ks * g.w3_tile_bytes, g.w3_tile_bytes);
             }
         }
     } else if (warp == 3) {
@@ -306,40 +309,46 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                 }
             }
         }
+    } else if (warp == 2) {
+        // ================= layer-1 MMA issuer (this warp also owns the TMEM allocation) =================
+        // Layer 1 has its own issuing warp so that neither issuer has more than two mbarrier round trips per
+        // 32-column chunk: it runs ahead of layer 2 as far as the three D1 buffers allow.  Whole warp convergent,
+        // one elected lane issues (ptxas then keeps descriptors and barrier addresses in uniform registers).
+        const uint32_t id32 = umma_idesc(32, g.b_fmt);
+        const uint64_t dA0 = umma_desc(s_r2), dW1 = umma_desc(s_r2 + kChunkBytes);
+        uint32_t w1c = 0, gs = 0, tc = 0;
+        for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tc) {
+            mbar_wait(bar(B_A0_FULL), tc & 1);
+            for (int h = 0; h < 2; ++h)
+                for (int c = 0; c < g.NC; ++c, ++gs) {
+                    const uint32_t slot = w1c & 1, sb = gs % kSmallBufs;
+                    if ((c & 3) == 0) mbar_wait(bar(B_W1_FULL + slot), (w1c >> 1) & 1);
+                    mbar_wait(bar(B_SMALL_EMPTY + sb), ((gs / kSmallBufs) & 1) ^ 1);
+                    tc_fence_after();
+                    const bool quad_done = (c & 3) == 3 || c == g.NC - 1;
+                    if (elect_one()) {
+                        const uint64_t b0 = dW1 + ((slot * kW1QuadBytes + ((c & 3) >> 1) * 4096 + (c & 1) * 64) >> 4);
+                        const uint32_t dd = tmem + kSmallCol + sb * 32;
+                        tc_mma(dd, dA0, b0, id32, 0u);
+                        if (g.K0steps > 1) tc_mma(dd, dA0 + 2, b0 + 2, id32, 1u);
+                        tc_commit(bar(B_SMALL_FULL + sb));
+                        if (quad_done) tc_commit(bar(B_W1_EMPTY + slot));
+                    }
+                    __syncwarp();
+                    if (quad_done) ++w1c;
+                }
+            ++gs;  // the D4 accumulation of this tile (issued by warp 1) takes the next buffer of the ring
+        }
     } else if (warp == 1) {
-        // ================= MMA issuer =================
-        // The whole warp runs this loop convergently (all control flow is warp-uniform) and one elected lane
-        // issues the tcgen05 instructions: ptxas then keeps descriptors and barrier addresses in uniform
-        // registers instead of wrapping every UTCHMMA in a per-thread election loop.
+        // ================= layer-2/3/4 MMA issuer (whole warp convergent, one elected lane issues) =================
         const uint32_t id32 = umma_idesc(32, g.b_fmt);
         const uint32_t id2a = umma_idesc(g.na2, g.b_fmt), id2b = umma_idesc(g.nb2 > 0 ? g.nb2 : 16, g.b_fmt);
         const uint32_t id3a = umma_idesc(g.n3a, g.b_fmt), id3b = umma_idesc(g.n3b > 0 ? g.n3b : 16, g.b_fmt);
-        const uint64_t dA0 = umma_desc(s_r2), dW1 = umma_desc(s_r2 + kChunkBytes), dR1 = umma_desc(s_r1);
-        const uint64_t dW = umma_desc(s_w), dW4 = umma_desc(s_w4);
+        const uint64_t dR2 = umma_desc(s_r2), dR1 = umma_desc(s_r1), dW = umma_desc(s_w), dW4 = umma_desc(s_w4);
         const uint32_t w_slot16 = (uint32_t)g.w_slot_bytes >> 4;
         // gs: uses of the small-accumulator ring (layer-1 chunks and D4); ac: uses of the A1 quarter-slots
-        uint32_t wc = 0, w1c = 0, gs = 0, ac = 0, ae = 0, h2cc = 0, h3c = 0, tc = 0;
+        uint32_t wc = 0, gs = 0, ac = 0, ae = 0, h2cc = 0, h3c = 0, tc = 0;
 
-        // layer-1 chunk c -> D1 buffer gs % 3 (caller has checked that the buffer and the W1 quad are ready)
-        auto issue_L1 = [&](int c) {
-            const uint32_t slot = w1c & 1, sb = gs % kSmallBufs;
-            ++gs;
-            tc_fence_after();
-            if (elect_one()) {
-                const uint64_t b0 = dW1 + ((slot * kW1QuadBytes + ((c & 3) >> 1) * 4096 + (c & 1) * 64) >> 4);
-                const uint32_t dd = tmem + kSmallCol + sb * 32;
-                tc_mma(dd, dA0, b0, id32, 0u);
-                if (g.K0steps > 1) tc_mma(dd, dA0 + 2, b0 + 2, id32, 1u);
-                tc_commit(bar(B_SMALL_FULL + sb));
-                if ((c & 3) == 3 || c == g.NC - 1) tc_commit(bar(B_W1_EMPTY + slot));
-            }
-            __syncwarp();
-            if ((c & 3) == 3 || c == g.NC - 1) ++w1c;
-        };
-        auto L1_ready = [&](int c) {
-            if ((c & 3) == 0 && !mbar_test(bar(B_W1_FULL + (w1c & 1)), (w1c >> 1) & 1)) return false;
-            return mbar_test(bar(B_SMALL_EMPTY + gs % kSmallBufs), ((gs / kSmallBufs) & 1) ^ 1);
-        };
         // one 32-wide K stage of a [128 x N] += A[128 x 32] W^T update, N split into two MMA pieces;
         // `extra` is a second barrier to commit to (the A-operand slot), or 0.
         auto issue_stage = [&](uint64_t ad, int na, int nb, uint32_t ida, uint32_t idb, bool first, uint32_t extra) {
@@ -360,40 +369,33 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
         };
 
         for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tc) {
+            // ---- phase A: layer 2, one half of its outputs at a time, one stage per layer-1 chunk ----
             mbar_wait(bar(B_A0_FULL), tc & 1);
-            // ---- phase A: layers 1+2, one half of layer 2's outputs at a time.  Event loop: layer-1 chunks are
-            //      issued as soon as a D1 buffer is free, layer-2 stages as soon as their A1 slot is full, so the
-            //      epilogue groups always have a chunk to work on while the tensor pipe runs layer 2. ----
             for (int h = 0; h < 2; ++h) {
-                int l1 = 0, l2 = 0;
-                while (l2 < g.NC) {
-                    if (l1 < g.NC && L1_ready(l1)) {
-                        issue_L1(l1++);
-                        continue;
-                    }
-                    const uint32_t slot = ac & 3;
-                    if (l2 < l1 && mbar_test(bar(B_A1_FULL + slot), (ac >> 2) & 1)) {
-                        if (l2 == 0) {
-                            mbar_wait(bar(B_ACC_EMPTY), (ae & 1) ^ 1);
-                            ++ae;
-                        }
-                        issue_stage(dR1 + (((slot >> 1) * kChunkBytes + (slot & 1) * 64) >> 4), g.na2, g.nb2, id2a, id2b,
-                                    l2 == 0, bar(B_A1_EMPTY + slot));
-                        ++ac;
-                        ++l2;
-                    }
+                // bias stage: D2 = A0 Wb2^T, where Wb2 is zero except for the fp16 hi/lo parts of b2 in the two
+                // K rows that meet the ones columns of A0 -- the accumulator starts from the bias
+                mbar_wait(bar(B_ACC_EMPTY), (ae & 1) ^ 1);
+                ++ae;
+                issue_stage(dR2, g.na2, g.nb2, id2a, id2b, true, 0u);
+                for (int c = 0; c < g.NC; ++c, ++ac) {
+                    const uint32_t slot = ac % kA1Slots;
+                    mbar_wait(bar(B_A1_FULL + slot), (ac / kA1Slots) & 1);
+                    issue_stage(dR1 + (((slot >> 1) * kChunkBytes + (slot & 1) * 64) >> 4), g.na2, g.nb2, id2a, id2b, false,
+                                bar(B_A1_EMPTY + slot));
                 }
                 if (elect_one()) tc_commit(bar(B_ACC_FULL));
                 __syncwarp();
             }
+            gs += 2 * g.NC;
             // ---- phase B: layer 3 from the H2 chunks, then layer 4 fed by the D3 drain ----
             mbar_wait(bar(B_ACC_EMPTY), (ae & 1) ^ 1);
             ++ae;
+            issue_stage(dR2, g.n3a, g.n3b, id3a, id3b, true, 0u);  // bias stage of layer 3 (A0 is still intact)
             for (int ks = 0; ks < g.NKS; ++ks) {
                 const uint32_t slot = h2cc & 1;
                 if ((ks & 1) == 0) mbar_wait(bar(B_H2C_FULL + slot), (h2cc >> 1) & 1);
                 const bool last = (ks & 1) == 1 || ks == g.NKS - 1;
-                issue_stage(dR1 + ((slot * kChunkBytes + (ks & 1) * 64) >> 4), g.n3a, g.n3b, id3a, id3b, ks == 0,
+                issue_stage(dR1 + ((slot * kChunkBytes + (ks & 1) * 64) >> 4), g.n3a, g.n3b, id3a, id3b, false,
                             last ? bar(B_H2C_EMPTY + slot) : 0u);
                 if (last) ++h2cc;
             }
@@ -408,7 +410,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                 tc_fence_after();
                 if (elect_one()) {
                     const int ksteps = min(64, g.d3 - jj * 64) / 16;
-                    const uint64_t ha = dA0 + ((slot * kChunkBytes) >> 4), wa = dW4 + ((jj * 4096) >> 4);
+                    const uint64_t ha = dR2 + ((slot * kChunkBytes) >> 4), wa = dW4 + ((jj * 4096) >> 4);
                     for (int kk = 0; kk < ksteps; ++kk)
                         tc_mma(tmem + kSmallCol + sb * 32, ha + 2 * kk, wa + 2 * kk, id32, (jj > 0 || kk > 0) ? 1u : 0u);
                     tc_commit(bar(B_H3_EMPTY + slot));
@@ -436,20 +438,19 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
         auto st_shared16 = [&](uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
             asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
         };
-        // +bias, GELU on 16 accumulators -> 8 packed fp16x2 words
-        auto act16 = [&](const uint32_t* r, const float* bias, uint32_t (&o)[8]) {
-            const float4* b4 = reinterpret_cast<const float4*>(bias);
+        // GELU on 16 accumulators (biases are already in them) -> 8 packed fp16x2 words
+        auto gelu16 = [&](const uint32_t* r, uint32_t (&o)[8]) {
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const float4 b = __ldg(b4 + i);
-                o[2 * i] = pack_act(gelu_fast(__uint_as_float(r[4 * i + 0]) + b.x), gelu_fast(__uint_as_float(r[4 * i + 1]) + b.y));
-                o[2 * i + 1] = pack_act(gelu_fast(__uint_as_float(r[4 * i + 2]) + b.z), gelu_fast(__uint_as_float(r[4 * i + 3]) + b.w));
-            }
+            for (int i = 0; i < 8; ++i)
+                o[i] = pack_act(gelu_fast(__uint_as_float(r[2 * i])), gelu_fast(__uint_as_float(r[2 * i + 1])));
         };
 
-        for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+        uint32_t tcnt = 0;
+        for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tcnt) {
             const long long cell = tile * kTileM + row;
             const bool valid = cell < a.n;
+            // A0 shares its shared memory with the first H3 slot: the previous tile's layer-4 MMAs must be done
+            if (tcnt > 0) mbar_wait(bar(B_TILE_DONE), (tcnt - 1) & 1);
             // ---- prologue: features + two bias columns of ones -> fp16 A0 [128 x 32]; group grp writes
             //      feature columns [8 grp, 8 grp + 8) ----
             for (int fc = grp; fc < 4; fc += kGroups) {
@@ -480,7 +481,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                 }
                 st_shared16(s_r2 + swz(row, fc), o[0], o[1], o[2], o[3]);
             }
-            fence_proxy_async();
+            fence_proxy_async_smem();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(B_A0_FULL));
             // ---- phase A ----
@@ -500,13 +501,13 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
 #pragma unroll
                     for (int i = 0; i < 16; ++i)   // b1 is already in the accumulator (bias columns of W1)
                         o[i] = pack_act(gelu_fast(__uint_as_float(r[2 * i])), gelu_fast(__uint_as_float(r[2 * i + 1])));
-                    const uint32_t slot = ac & 3;
-                    mbar_wait(bar(B_A1_EMPTY + slot), ((ac >> 2) & 1) ^ 1);
+                    const uint32_t slot = ac % kA1Slots;
+                    mbar_wait(bar(B_A1_EMPTY + slot), ((ac / kA1Slots) & 1) ^ 1);
                     const uint32_t base = s_r1 + (slot >> 1) * kChunkBytes;
 #pragma unroll
                     for (int c4 = 0; c4 < 4; ++c4)
                         st_shared16(base + swz(row, (slot & 1) * 4 + c4), o[4 * c4], o[4 * c4 + 1], o[4 * c4 + 2], o[4 * c4 + 3]);
-                    fence_proxy_async();
+                    fence_proxy_async_smem();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar(B_A1_FULL + slot));
                 }
@@ -514,16 +515,32 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                 mbar_wait(bar(B_ACC_FULL), af & 1);
                 ++af;
                 tc_fence_after();
-                for (int c0 = grp * 16; c0 < g.NH; c0 += 16 * kGroups) {
-                    uint32_t r[16], o[8];
-                    tc_ld16(t_lane + c0, r);
-                    tc_wait_ld();
-                    const int gc = h * g.NH + c0;
-                    act16(r, a.d.b2 + gc, o);
-                    uint8_t* dst = scratch + (size_t)(gc >> 6) * kChunkBytes;
-                    const int c16 = (gc & 63) >> 3;
-                    *reinterpret_cast<uint4*>(dst + swz(row, c16)) = make_uint4(o[0], o[1], o[2], o[3]);
-                    *reinterpret_cast<uint4*>(dst + swz(row, c16 + 1)) = make_uint4(o[4], o[5], o[6], o[7]);
+                {
+                    // software-pipelined: the TMEM load of the next 16-column unit is in flight during the math
+                    auto store_unit = [&](const uint32_t* r, int c0) {
+                        uint32_t o[8];
+                        gelu16(r, o);
+                        const int gc = h * g.NH + c0;
+                        uint8_t* dst = scratch + (size_t)(gc >> 6) * kChunkBytes;
+                        const int c16 = (gc & 63) >> 3;
+                        *reinterpret_cast<uint4*>(dst + swz(row, c16)) = make_uint4(o[0], o[1], o[2], o[3]);
+                        *reinterpret_cast<uint4*>(dst + swz(row, c16 + 1)) = make_uint4(o[4], o[5], o[6], o[7]);
+                    };
+                    constexpr int kStep = 16 * kGroups;
+                    uint32_t ra[16], rb[16];
+                    int c0 = grp * 16;
+                    if (c0 < g.NH) tc_ld16(t_lane + c0, ra);
+                    while (c0 < g.NH) {
+                        tc_wait_ld();
+                        if (c0 + kStep < g.NH) tc_ld16(t_lane + c0 + kStep, rb);
+                        store_unit(ra, c0);
+                        c0 += kStep;
+                        if (c0 >= g.NH) break;
+                        tc_wait_ld();
+                        if (c0 + kStep < g.NH) tc_ld16(t_lane + c0 + kStep, ra);
+                        store_unit(rb, c0);
+                        c0 += kStep;
+                    }
                 }
                 tc_fence_before();
                 __threadfence();
@@ -550,7 +567,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                         uint32_t r[16];
                         tc_ld16(t_lane + c0, r);
                         tc_wait_ld();
-                        act16(r, a.d.b3 + c0, o[i]);
+                        gelu16(r, o[i]);
                     }
                 }
                 const uint32_t slot = h3c & 1;
@@ -563,7 +580,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                         st_shared16(base + swz(row, u * 2), o[i][0], o[i][1], o[i][2], o[i][3]);
                         st_shared16(base + swz(row, u * 2 + 1), o[i][4], o[i][5], o[i][6], o[i][7]);
                     }
-                fence_proxy_async();
+                fence_proxy_async_smem();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar(B_H3_FULL + slot));
             }
@@ -690,7 +707,7 @@ df_status ann_bf16_create(df_ann* ann, const float* const* W, const float* const
     g.w4_bytes = g.NJ * 4096;
     g.off_w = 0;
     g.off_r1 = kWStages * g.w_slot_bytes;
-    g.off_r2 = g.off_r1 + 2 * kChunkBytes;
+    g.off_r2 = g.off_r1 + kA1Tiles * kChunkBytes;
     g.off_w4 = g.off_r2 + 2 * kChunkBytes;
     g.off_bar = g.off_w4 + g.w4_bytes;
     g.smem_bytes = g.off_bar + B_COUNT * 8 + 16 + 1024;
@@ -701,12 +718,26 @@ df_status ann_bf16_create(df_ann* ann, const float* const* W, const float* const
     DF_CUDA_TRY(cudaDeviceGetAttribute(&P->num_sms, cudaDevAttrMultiProcessorCount, dev));
 
     const int nquads = (g.NC + 3) / 4;
-    const size_t sz_w1 = (size_t)nquads * kW1QuadBytes, sz_w2 = (size_t)2 * g.NC * g.w2_tile_bytes,
-                 sz_w3 = (size_t)g.NKS * g.w3_tile_bytes, sz_w4 = (size_t)g.w4_bytes;
+    const size_t sz_w1 = (size_t)nquads * kW1QuadBytes, sz_w2 = (size_t)2 * (g.NC + 1) * g.w2_tile_bytes,
+                 sz_w3 = (size_t)(g.NKS + 1) * g.w3_tile_bytes, sz_w4 = (size_t)g.w4_bytes;
     const size_t sz_b = (size_t)(d1 + d2 + d3 + 32) * sizeof(float);
     const size_t o_w1 = 0, o_w2 = o_w1 + sz_w1, o_w3 = o_w2 + sz_w2, o_w4 = o_w3 + sz_w3, o_b = o_w4 + sz_w4;
     std::vector<uint8_t> blob(o_b + sz_b, 0);
     const int din = K + 2;
+    auto put_bias_w1 = [&](uint8_t* t, int r, int col0, float bv) {
+        const uint16_t hb = g.b_fmt ? bf16_bits(bv) : fp16_bits(bv);
+        float hf;
+        if (g.b_fmt) {
+            const uint32_t hu = (uint32_t)hb << 16;
+            memcpy(&hf, &hu, 4);
+        } else {
+            __half hh;
+            memcpy(&hh, &hb, 2);
+            hf = __half2float(hh);
+        }
+        put(t, r, col0 + din, hf);
+        put(t, r, col0 + din + 1, bv - hf);
+    };
     // W1: chunk c (32 outputs) sits in quad c/4 at rows 32*((c&3)>>1).., K columns 32*(c&1)..; columns K+2 and
     // K+3 carry the bf16 hi and lo parts of b1 (the A0 tile holds 1.0 there).
     for (int c = 0; c < g.NC; ++c) {
@@ -715,18 +746,38 @@ df_status ann_bf16_create(df_ann* ann, const float* const* W, const float* const
         for (int r = 0; r < 32; ++r) {
             const int o = c * 32 + r;
             for (int k = 0; k < din; ++k) put(t, r0 + r, k0 + k, W[0][(size_t)o * din + k]);
-            const float bh = b[0][o];
-            uint16_t hb = bf16_bits(bh);
-            uint32_t hu = (uint32_t)hb << 16;
-            float bhf;
-            memcpy(&bhf, &hu, 4);
-            put(t, r0 + r, k0 + din, bhf);
-            put(t, r0 + r, k0 + din + 1, bh - bhf);
+            put_bias_w1(t, r0 + r, k0, b[0][o]);
         }
+    }
+    // bias tiles: zero except K rows din, din + 1 (the ones columns of A0) = hi / lo parts of the bias
+    auto put_bias = [&](uint8_t* t, int r, int col0, float bv) {
+        g_put_fmt = g.b_fmt;
+        const uint16_t hb = g.b_fmt ? bf16_bits(bv) : fp16_bits(bv);
+        float hf;
+        if (g.b_fmt) {
+            const uint32_t hu = (uint32_t)hb << 16;
+            memcpy(&hf, &hu, 4);
+        } else {
+            __half hh;
+            memcpy(&hh, &hb, 2);
+            hf = __half2float(hh);
+        }
+        put(t, r, col0 + din, hf);
+        put(t, r, col0 + din + 1, bv - hf);
+    };
+    for (int h = 0; h < 2; ++h) {
+        uint8_t* t = blob.data() + o_w2 + (size_t)(h * (g.NC + 1)) * g.w2_tile_bytes;
+        for (int r = 0; r < g.na2; ++r) put_bias(t, r, 0, b[1][h * g.NH + r]);
+        for (int r = 0; r < g.nb2; ++r) put_bias(t, r, 32, b[1][h * g.NH + g.na2 + r]);
+    }
+    {
+        uint8_t* t = blob.data() + o_w3;
+        for (int r = 0; r < g.n3a; ++r) put_bias(t, r, 0, b[2][r]);
+        for (int r = 0; r < g.n3b; ++r) put_bias(t, r, 32, b[2][g.n3a + r]);
     }
     for (int h = 0; h < 2; ++h)
         for (int c = 0; c < g.NC; ++c) {
-            uint8_t* t = blob.data() + o_w2 + (size_t)(h * g.NC + c) * g.w2_tile_bytes;
+            uint8_t* t = blob.data() + o_w2 + (size_t)(h * (g.NC + 1) + 1 + c) * g.w2_tile_bytes;
             const int k0 = c * 32;
             for (int kk = 0; kk < 32; ++kk) {
                 for (int r = 0; r < g.na2; ++r) put(t, r, kk, W[1][(size_t)(h * g.NH + r) * d1 + k0 + kk]);
@@ -734,7 +785,7 @@ df_status ann_bf16_create(df_ann* ann, const float* const* W, const float* const
             }
         }
     for (int ks = 0; ks < g.NKS; ++ks) {
-        uint8_t* t = blob.data() + o_w3 + (size_t)ks * g.w3_tile_bytes;
+        uint8_t* t = blob.data() + o_w3 + (size_t)(ks + 1) * g.w3_tile_bytes;
         for (int kk = 0; kk < 32; ++kk) {
             for (int r = 0; r < g.n3a; ++r) put(t, r, kk, W[2][(size_t)r * d2 + ks * 32 + kk]);
             for (int r = 0; r < g.n3b; ++r) put(t, r, 32 + kk, W[2][(size_t)(g.n3a + r) * d2 + ks * 32 + kk]);
