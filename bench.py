@@ -109,7 +109,8 @@ def run_reference(args):
     if rank != 0:
         return
     from oracle import oracle
-    ns = args.ref_cells
+    # bounded sample per step: about 2e6 cell-updates in total (~2 minutes on 16 cores), never above --ref-cells
+    ns = max(4096, min(args.ref_cells, int(2.0e6 / max(1, args.steps + args.warmup))))
     mech, ann, cells = make_inputs(ns, 0)
     om, oa = oracle.Mech(mech), oracle.Ann(ann)
     _, h = om.mixture_cp_h(cells.T, cells.Y)
@@ -139,6 +140,21 @@ def run_reference(args):
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
+
+
+def max_over_ranks(dist, x: float, device="cpu") -> float:
+    """Timing rule for N > 1: the slowest rank defines the step (no-op without a process group)."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([x], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(world: int, cells_per_gpu: int, ms_per_step: float) -> float:
+    """Whole-job cells/s of `world` replicas that each process cells_per_gpu cells per step (weak scaling)."""
+    return world * cells_per_gpu / (ms_per_step * 1e-3)
 
 
 def cpu_baseline(ns: int):
@@ -220,12 +236,9 @@ def run_gpu(args):
         barrier()
         w1 = time.perf_counter()
     ms = t_start.elapsed_time(t_end)
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(dist, ms, "cuda")
     ms_step = ms / args.steps
-    value = world * n / (ms_step * 1e-3)
+    value = aggregate_value(world, n, ms_step)
     k_ms = [float(np.mean([e[i].elapsed_time(e[i + 1]) for e in marks])) for i in range(3)]
 
     # ---- e2e: the same step through df_step_host with pinned HOST buffers ----
@@ -242,10 +255,7 @@ def run_gpu(args):
     for _ in range(e2e_steps):
         ctx.step(n, n, hh, hp, hg, hY, T=oT, cp=ocp, mu=omu, lam=olam, D=oD, omega=oom)   # synchronises inside
     e2e_s = (time.perf_counter() - t0) / e2e_steps
-    if dist is not None:
-        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(dist, e2e_s, "cuda")
     h2d = 4 * n * (3 + K)
     d2h = 4 * n * (4 + 2 * K)
 
@@ -258,7 +268,7 @@ def run_gpu(args):
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "vs_baseline": None, "dtype": "f16 operands (bf16-valued weights) / f32 accumulate; f32 thermo+transport", "data": "synthetic",
         "config": {"workload": f"configs[2]: {n} cells/GPU, K=19, T_from_h -> properties -> bf16 MLP 21-1600-800-400-19",
                    "cells_per_gpu": n, "l2": "inputs (176 MB/step at the full size) exceed the 126 MB L2; no explicit flush",
                    "parallelism": f"replicas x{world} (no collective in the data path)"},

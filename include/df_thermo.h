@@ -83,9 +83,11 @@ DF_API int df_mech_num_species(const df_mech* mech);
  * n_layers linear layers, dims[0] = K+2 inputs (T, p, F(Y_0..K-1)), dims[n_layers] = K outputs,
  * GELU after every layer but the last.  W[l] is [dims[l+1]][dims[l]] row-major (y = x W^T + b).
  * precision 0: fp32 FFMA path (any n_layers >= 1, every dims[l] <= 256).
- * precision 1: bf16 operands / fp32 accumulate on tcgen05 (weights are rounded to bf16 at
- *              create; n_layers == 4, dims[1..3] multiples of 16 with dims[1] % 64 == 0,
- *              dims[2] % 32 == 0 and dims[2] <= 1024, dims[3] <= 512, K <= 30).
+ * precision 1: 16-bit tensor-core path (tcgen05, fp32 accumulate in TMEM).  Weights are expected to be
+ *              bf16-valued (as BASELINE's "bf16 weights"); tcgen05 kind::f16 needs both operands in one format,
+ *              so they are held in fp16 (exact for |w| >= 2^-14) and activations are rounded to fp16 (A21).
+ *              n_layers == 4, dims[1] % 64 == 0, dims[2] % 32 == 0 with 64 <= dims[2] <= 800,
+ *              dims[3] % 16 == 0 with 32 <= dims[3] <= 400, K <= 28.
  * x_mean/x_std [K+2] and u_mean/u_std [K] are the Z-score statistics; the network output
  * o is the z-scored change in Box-Cox space (A9): Delta_k = u_std[k] o_k + u_mean[k].
  * F(y) = (y^lambda - 1)/lambda with lambda = boxcox_lambda > 0 (A10); dt in seconds. */

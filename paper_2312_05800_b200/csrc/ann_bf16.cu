@@ -1,27 +1,26 @@
-// ann_bf16.cu -- K4: the ANN source term with bf16 operands / fp32 accumulation on the 5th-gen
-// tensor cores (tcgen05.mma, accumulators in TMEM, weights streamed by TMA bulk copies), one
-// persistent warp-specialised kernel for the whole chain (1600-800-400 GELU MLP;
-// DESIGN.md "K4").
+// ann_bf16.cu -- K4: the ANN source term on the 5th-gen tensor cores (tcgen05.mma, fp32 accumulators in TMEM,
+// weights streamed by TMA bulk copies): one persistent warp-specialised kernel for the whole chain
+// (1600-800-400 GELU MLP; DESIGN.md section 6 "K4" and reading A21).
 //
 // Per 128-cell tile (UMMA M = 128, one cell per TMEM lane) a CTA runs
-//   prologue   T, p, Y -> Box-Cox + z-score -> bf16 A0 [128 x 32]                    (threads)
+//   prologue   T, p, Y -> Box-Cox + z-score -> fp16 A0 [128 x 32] (+ two columns of ones for the biases) (threads)
 //   phase A    for each half h of layer 2's outputs (N = d2/2 <= 400 TMEM columns):
-//                for each 64-wide chunk j of layer 1:  D1 = A0 W1_j^T  (K = 32)     (tcgen05)
-//                  epilogue warps: +b1, GELU, bf16 -> A1 ring (swizzled smem)       (threads)
-//                  D2 += A1_j W2[h, j]^T                                            (tcgen05)
-//              drain D2: +b2, GELU, bf16 -> this CTA's private H2 scratch (global, L2-resident)
-//   phase B    D3 = H2 W3^T with H2 chunks read back by TMA; drain D3 in 64-wide chunks:
-//              +b3, GELU, bf16 -> H3 ring -> D4 += H3_c W4_c^T; final epilogue: +b4, inverse
-//              Box-Cox, sum-to-one renormalisation, rho, omega -> global (coalesced SoA).
-// Layer 1 is recomputed for each half of layer 2 (K = 32: 2 % of the MMA work) because neither
-// a 128 x 1600 bf16 activation tile (400 KB) nor a 128 x 800 fp32 accumulator (800 TMEM columns)
-// fits on an SM.  All weights are re-tiled at create time into the exact 128B-swizzled K-major
-// shared-memory images the UMMA descriptors expect, in streaming order, so every TMA transfer is
-// one contiguous cp.async.bulk of 8-26 KB.
+//                D2 = A0 Wb2[h]^T                               (bias stage)                      (tcgen05)
+//                for each 32-wide chunk c of layer 1:  D1 = A0 W1_c^T                              (tcgen05)
+//                  an epilogue group: tcgen05.ld, GELU, fp16 -> A1 ring (128B-swizzled smem)       (threads)
+//                  D2 += A1_c W2[h, c]^T                                                           (tcgen05)
+//              drain D2: GELU, fp16 -> this CTA's private H2 scratch (global, L2-resident)
+//   phase B    D3 = A0 Wb3^T + H2 W3^T with the H2 chunks read back by TMA; drain D3 in 64-wide chunks:
+//              GELU, fp16 -> H3 ring -> D4 += H3_c W4_c^T; final epilogue: +b4, inverse Box-Cox, sum-to-one
+//              renormalisation, rho, omega -> global (coalesced SoA).
+// Layer 1 is recomputed for each half of layer 2 (K = 23: 2 % of the MMA work) because neither a 128 x 1600
+// 16-bit activation tile (400 KB) nor a 128 x 800 fp32 accumulator (800 TMEM columns) fits on an SM.  All weights
+// are re-tiled at create time into the exact 128B-swizzled K-major shared-memory images the UMMA descriptors
+// expect, in streaming order, so every TMA transfer is one contiguous cp.async.bulk of 8-26 KB.
 //
-// Warp roles (384 threads): 0 = weight-ring TMA producer, 1 = MMA issuer, 2 = TMEM allocator,
-// 3 = auxiliary TMA producer (W1 pairs, H2 chunks, W4), 4..11 = epilogue (8 warps; warp w owns
-// TMEM lanes 32 (w % 4) .. +31 and one half of the columns of every chunk).
+// Warp roles (128 + 128 kGroups threads): 0 = weight-ring TMA producer, 1 = layer-2/3/4 MMA issuer, 2 = TMEM
+// allocator and layer-1 MMA issuer, 3 = auxiliary TMA producer (W1 quads, H2 chunks, W4), 4.. = kGroups epilogue
+// groups of four warps (warp w owns TMEM lanes 32 (w % 4) .. +31); group g takes every kGroups-th layer-1 chunk.
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
