@@ -274,7 +274,9 @@ def run_gpu(args):
                    "parallelism": f"replicas x{world} (no collective in the data path)"},
         "kernel_ms": {"T_from_h": k_ms[0], "properties": k_ms[1], "ann_bf16": k_ms[2]},
         "roofline": {"bound": "tensor", "kernel": "ann_bf16_kernel", "achieved": achieved, "peak": pk["bf16"],
-                     "unit": "TFLOP/s", "frac": achieved / pk["bf16"], "traffic": None,
+                     "unit": "TFLOP/s", "frac": achieved / pk["bf16"],
+                     # dram__bytes_read.sum + dram__bytes_write.sum of one launch at the full size (profiles/r1_summary.md)
+                     "traffic": 325.4e6 if n == 2097152 else None,
                      "peak_source": f"{pk['src']} bf16 burst (sustained: {pk['bf16_sust']})",
                      "algorithmic": f"{FLOPS_PER_CELL_MLP} flop/cell x {n} cells/launch"},
         "e2e": {"value": world * n / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
