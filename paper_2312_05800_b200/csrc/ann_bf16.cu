@@ -39,7 +39,11 @@ constexpr int kTileM = 128;
 #define KGROUPS 3
 #endif
 constexpr int kGroups = KGROUPS;                  // epilogue groups of 4 warps (one warp per TMEM lane quarter)
-constexpr int kThreads = 128 + kGroups * 128;
+#ifndef DF_EXTRA_WARPS
+#define DF_EXTRA_WARPS 0
+#endif
+constexpr int kIssuer2Warp = 4 + 4 * kGroups;  // second layer-2/3 MMA issuer (after the epilogue warps)
+constexpr int kThreads = 128 + kGroups * 128 + 32 + 32 * DF_EXTRA_WARPS;
 constexpr int kWStages = 4;
 constexpr int kA1Tiles = 3;                 // [128 x 64] activation tiles of the A1 ring = 2 * kA1Tiles 32-column slots
 constexpr int kA1Slots = 2 * kA1Tiles;
@@ -184,6 +188,21 @@ __device__ __forceinline__ float gelu_fast(float v) {
     const float hv = 0.5f * v;
     return fmaf(hv, tanh_approx(u), hv);
 }
+// GELU (tanh form) on two packed fp16 values: 6 half2 instructions + 1 MUFU for two activations.  The inputs are the
+// fp32 accumulators rounded to fp16 (2^-11), the arithmetic adds ~1e-3 relative: well inside the 2e-2 budget (A12).
+__device__ __forceinline__ uint32_t gelu_h2(uint32_t v) {
+    uint32_t r;
+    asm("{\n\t.reg .b32 vv, t, u, th, hv;\n\t"
+        "mul.f16x2 vv, %1, %1;\n\t"
+        "fma.rn.f16x2 t, vv, %2, %3;\n\t"
+        "mul.f16x2 u, t, %1;\n\t"
+        "tanh.approx.f16x2 th, u;\n\t"
+        "mul.f16x2 hv, %1, %4;\n\t"
+        "fma.rn.f16x2 %0, hv, th, hv;\n\t}"
+        : "=r"(r)
+        : "r"(v), "r"(0x28912891u) /* 0.035677 */, "r"(0x3A623A62u) /* 0.79788 */, "r"(0x38003800u) /* 0.5 */);
+    return r;
+}
 // two fp32 -> packed fp16x2 (first argument in the low half = lower K index)
 __device__ __forceinline__ uint32_t pack_act(float lo, float hi) {
     uint32_t r;
@@ -205,13 +224,20 @@ __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&r)[32]) {
         : "memory");
 }
 
+#ifdef DF_DBG_CLK
+__device__ long long g_dbg[16][128];
+#define DBG_REC(row, idx, cond) do { if ((cond) && blockIdx.x == 0 && (idx) < 128) g_dbg[row][idx] = clock64(); } while (0)
+#else
+#define DBG_REC(row, idx, cond) do { } while (0)
+#endif
+
 // barrier indices
 enum {
     B_W_FULL = 0, B_W_EMPTY = B_W_FULL + kWStages, B_W1_FULL = B_W_EMPTY + kWStages, B_W1_EMPTY = B_W1_FULL + 2,
     B_A0_FULL = B_W1_EMPTY + 2, B_SMALL_FULL, B_SMALL_EMPTY = B_SMALL_FULL + kSmallBufs,
     B_A1_FULL = B_SMALL_EMPTY + kSmallBufs, B_A1_EMPTY = B_A1_FULL + kA1Slots, B_ACC_FULL = B_A1_EMPTY + kA1Slots, B_ACC_EMPTY,
     B_H2_FULL, B_H2C_FULL, B_H2C_EMPTY = B_H2C_FULL + 2, B_H3_FULL = B_H2C_EMPTY + 2, B_H3_EMPTY = B_H3_FULL + 2, B_TILE_DONE = B_H3_EMPTY + 2,
-    B_W4_FULL, B_COUNT
+    B_W4_FULL, B_ACC_START, B_COUNT
 };
 
 struct KArgs {
@@ -244,6 +270,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             if ((i >= B_SMALL_EMPTY && i < B_SMALL_EMPTY + kSmallBufs) || (i >= B_A1_FULL && i < B_A1_FULL + kA1Slots)) cnt = 4;
             if (i == B_A0_FULL || i == B_ACC_EMPTY || i == B_H3_FULL || i == B_H3_FULL + 1) cnt = 4 * kGroups;
             if (i == B_H2_FULL) cnt = 8 * kGroups;
+            if (i == B_ACC_FULL || i == B_H2C_EMPTY || i == B_H2C_EMPTY + 1) cnt = 2;  // one commit per issuer
             mbar_init(bar(i), cnt);
         }
         fence_barrier_init();
@@ -323,6 +350,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                     const uint32_t slot = w1c & 1, sb = gs % kSmallBufs;
                     if ((c & 3) == 0) mbar_wait(bar(B_W1_FULL + slot), (w1c >> 1) & 1);
                     mbar_wait(bar(B_SMALL_EMPTY + sb), ((gs / kSmallBufs) & 1) ^ 1);
+                    DBG_REC(0, gs - 150, lane == 0 && gs >= 150);
                     tc_fence_after();
                     const bool quad_done = (c & 3) == 3 || c == g.NC - 1;
                     if (elect_one()) {
@@ -334,26 +362,31 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                         if (quad_done) tc_commit(bar(B_W1_EMPTY + slot));
                     }
                     __syncwarp();
+                    DBG_REC(1, gs - 150, lane == 0 && gs >= 150);
                     if (quad_done) ++w1c;
                 }
             ++gs;  // the D4 accumulation of this tile (issued by warp 1) takes the next buffer of the ring
         }
-    } else if (warp == 1) {
-        // ================= layer-2/3/4 MMA issuer (whole warp convergent, one elected lane issues) =================
+    } else if (warp == 1 || warp == kIssuer2Warp) {
+        // ================= layer-2/3/4 MMA issuers (two warps, each convergent, one elected lane issues) ============
+        // One warp needs ~700 cycles of its own instruction stream per 32-wide K stage (two mbarrier round trips,
+        // four UTCHMMA, two UTCBAR, warp re-convergence) against ~460 cycles of tensor time, so the stages of the
+        // weight ring alternate between two issuing warps: stage st goes to issuer st & 1.  The first stage of every
+        // accumulation (the bias stage, accumulate = 0) is announced on B_ACC_START before the other issuer adds to it;
+        // barriers that follow a whole accumulation / H2 tile (ACC_FULL, H2C_EMPTY) take one commit from each issuer.
+        const int id = (warp == 1) ? 0 : 1;
         const uint32_t id32 = umma_idesc(32, g.b_fmt);
         const uint32_t id2a = umma_idesc(g.na2, g.b_fmt), id2b = umma_idesc(g.nb2 > 0 ? g.nb2 : 16, g.b_fmt);
         const uint32_t id3a = umma_idesc(g.n3a, g.b_fmt), id3b = umma_idesc(g.n3b > 0 ? g.n3b : 16, g.b_fmt);
         const uint64_t dR2 = umma_desc(s_r2), dR1 = umma_desc(s_r1), dW = umma_desc(s_w), dW4 = umma_desc(s_w4);
         const uint32_t w_slot16 = (uint32_t)g.w_slot_bytes >> 4;
-        // gs: uses of the small-accumulator ring (layer-1 chunks and D4); ac: uses of the A1 quarter-slots
-        uint32_t wc = 0, gs = 0, ac = 0, ae = 0, h2cc = 0, h3c = 0, tc = 0;
+        // st: stages of the weight ring; gs: uses of the small-accumulator ring; ac: uses of the A1 slots;
+        // acc: accumulations started (three per tile)
+        uint32_t st = 0, gs = 0, ac = 0, ae = 0, h2cc = 0, h3c = 0, tc = 0, acc = 0;
 
-        // one 32-wide K stage of a [128 x N] += A[128 x 32] W^T update, N split into two MMA pieces;
-        // `extra` is a second barrier to commit to (the A-operand slot), or 0.
         auto issue_stage = [&](uint64_t ad, int na, int nb, uint32_t ida, uint32_t idb, bool first, uint32_t extra) {
-            const uint32_t slot = wc % kWStages;
-            mbar_wait(bar(B_W_FULL + slot), (wc / kWStages) & 1);
-            ++wc;
+            const uint32_t slot = st % kWStages;
+            mbar_wait(bar(B_W_FULL + slot), (st / kWStages) & 1);
             tc_fence_after();
             if (elect_one()) {
                 const uint64_t wb = dW + slot * w_slot16;
@@ -366,64 +399,81 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             }
             __syncwarp();
         };
+        // bias stage of an accumulation: whoever owns stage st issues it and announces it; the other waits
+        auto start_acc = [&](int na, int nb, uint32_t ida, uint32_t idb) {
+            if ((int)(st & 1) == id) {
+                mbar_wait(bar(B_ACC_EMPTY), (ae & 1) ^ 1);
+                issue_stage(dR2, na, nb, ida, idb, true, 0u);
+                if (lane == 0) mbar_arrive(bar(B_ACC_START));
+            } else {
+                mbar_wait(bar(B_ACC_START), acc & 1);
+            }
+            ++ae;
+            ++acc;
+            ++st;
+        };
 
         for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tc) {
-            // ---- phase A: layer 2, one half of its outputs at a time, one stage per layer-1 chunk ----
             mbar_wait(bar(B_A0_FULL), tc & 1);
+            // ---- phase A: layer 2, one half of its outputs at a time, one stage per layer-1 chunk ----
             for (int h = 0; h < 2; ++h) {
-                // bias stage: D2 = A0 Wb2^T, where Wb2 is zero except for the fp16 hi/lo parts of b2 in the two
-                // K rows that meet the ones columns of A0 -- the accumulator starts from the bias
-                mbar_wait(bar(B_ACC_EMPTY), (ae & 1) ^ 1);
-                ++ae;
-                issue_stage(dR2, g.na2, g.nb2, id2a, id2b, true, 0u);
-                for (int c = 0; c < g.NC; ++c, ++ac) {
+                start_acc(g.na2, g.nb2, id2a, id2b);
+                for (int c = 0; c < g.NC; ++c, ++ac, ++st) {
+                    if ((int)(st & 1) != id) continue;
                     const uint32_t slot = ac % kA1Slots;
                     mbar_wait(bar(B_A1_FULL + slot), (ac / kA1Slots) & 1);
+                    DBG_REC(2, ac - 150, lane == 0 && ac >= 150);
                     issue_stage(dR1 + (((slot >> 1) * kChunkBytes + (slot & 1) * 64) >> 4), g.na2, g.nb2, id2a, id2b, false,
                                 bar(B_A1_EMPTY + slot));
+                    DBG_REC(3, ac - 150, lane == 0 && ac >= 150);
                 }
                 if (elect_one()) tc_commit(bar(B_ACC_FULL));
                 __syncwarp();
             }
             gs += 2 * g.NC;
             // ---- phase B: layer 3 from the H2 chunks, then layer 4 fed by the D3 drain ----
-            mbar_wait(bar(B_ACC_EMPTY), (ae & 1) ^ 1);
-            ++ae;
-            issue_stage(dR2, g.n3a, g.n3b, id3a, id3b, true, 0u);  // bias stage of layer 3 (A0 is still intact)
-            for (int ks = 0; ks < g.NKS; ++ks) {
+            start_acc(g.n3a, g.n3b, id3a, id3b);   // A0 is still intact (it is overwritten by the D3 drain)
+            for (int ks = 0; ks < g.NKS; ++ks, ++st) {
                 const uint32_t slot = h2cc & 1;
-                if ((ks & 1) == 0) mbar_wait(bar(B_H2C_FULL + slot), (h2cc >> 1) & 1);
                 const bool last = (ks & 1) == 1 || ks == g.NKS - 1;
-                issue_stage(dR1 + ((slot * kChunkBytes + (ks & 1) * 64) >> 4), g.n3a, g.n3b, id3a, id3b, false,
-                            last ? bar(B_H2C_EMPTY + slot) : 0u);
-                if (last) ++h2cc;
+                if ((int)(st & 1) == id) {
+                    mbar_wait(bar(B_H2C_FULL + slot), (h2cc >> 1) & 1);
+                    issue_stage(dR1 + ((slot * kChunkBytes + (ks & 1) * 64) >> 4), g.n3a, g.n3b, id3a, id3b, false, 0u);
+                }
+                if (last) {   // both issuers commit once per H2 tile (a commit with nothing outstanding arrives at once)
+                    if (elect_one()) tc_commit(bar(B_H2C_EMPTY + slot));
+                    __syncwarp();
+                    ++h2cc;
+                }
             }
             if (elect_one()) tc_commit(bar(B_ACC_FULL));
             __syncwarp();
-            if (tc == 0) mbar_wait(bar(B_W4_FULL), 0);
             const uint32_t sb = gs % kSmallBufs;
-            for (int jj = 0; jj < g.NJ; ++jj, ++h3c) {
-                const uint32_t slot = h3c & 1;
-                mbar_wait(bar(B_H3_FULL + slot), (h3c >> 1) & 1);
-                if (jj == 0) mbar_wait(bar(B_SMALL_EMPTY + sb), ((gs / kSmallBufs) & 1) ^ 1);
-                tc_fence_after();
+            if (id == 0) {
+                if (tc == 0) mbar_wait(bar(B_W4_FULL), 0);
+                for (int jj = 0; jj < g.NJ; ++jj, ++h3c) {
+                    const uint32_t slot = h3c & 1;
+                    mbar_wait(bar(B_H3_FULL + slot), (h3c >> 1) & 1);
+                    if (jj == 0) mbar_wait(bar(B_SMALL_EMPTY + sb), ((gs / kSmallBufs) & 1) ^ 1);
+                    tc_fence_after();
+                    if (elect_one()) {
+                        const int ksteps = min(64, g.d3 - jj * 64) / 16;
+                        const uint64_t ha = dR2 + ((slot * kChunkBytes) >> 4), wa = dW4 + ((jj * 4096) >> 4);
+                        for (int kk = 0; kk < ksteps; ++kk)
+                            tc_mma(tmem + kSmallCol + sb * 32, ha + 2 * kk, wa + 2 * kk, id32, (jj > 0 || kk > 0) ? 1u : 0u);
+                        tc_commit(bar(B_H3_EMPTY + slot));
+                    }
+                    __syncwarp();
+                }
                 if (elect_one()) {
-                    const int ksteps = min(64, g.d3 - jj * 64) / 16;
-                    const uint64_t ha = dR2 + ((slot * kChunkBytes) >> 4), wa = dW4 + ((jj * 4096) >> 4);
-                    for (int kk = 0; kk < ksteps; ++kk)
-                        tc_mma(tmem + kSmallCol + sb * 32, ha + 2 * kk, wa + 2 * kk, id32, (jj > 0 || kk > 0) ? 1u : 0u);
-                    tc_commit(bar(B_H3_EMPTY + slot));
+                    tc_commit(bar(B_SMALL_FULL + sb));
+                    tc_commit(bar(B_TILE_DONE));
                 }
                 __syncwarp();
             }
-            if (elect_one()) {
-                tc_commit(bar(B_SMALL_FULL + sb));
-                tc_commit(bar(B_TILE_DONE));
-            }
-            __syncwarp();
             ++gs;
         }
-    } else if (warp >= 4) {
+    } else if (warp >= 4 && warp < 4 + 4 * kGroups) {
         // ================= epilogue warps: kGroups groups of four (one warp per TMEM lane quarter) =================
         // Group grp takes every kGroups-th layer-1 chunk (so several chunks are in flight), every kGroups-th
         // 16-column unit of the D2/D3 drains, and one 16-byte column chunk of the A0 feature tile.
@@ -440,8 +490,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
         // GELU on 16 accumulators (biases are already in them) -> 8 packed fp16x2 words
         auto gelu16 = [&](const uint32_t* r, uint32_t (&o)[8]) {
 #pragma unroll
-            for (int i = 0; i < 8; ++i)
-                o[i] = pack_act(gelu_fast(__uint_as_float(r[2 * i])), gelu_fast(__uint_as_float(r[2 * i + 1])));
+            for (int i = 0; i < 8; ++i) o[i] = gelu_h2(pack_act(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1])));
         };
 
         uint32_t tcnt = 0;
@@ -489,6 +538,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                     if ((int)(ac % kGroups) != grp) continue;
                     const uint32_t sb = gs % kSmallBufs;
                     mbar_wait(bar(B_SMALL_FULL + sb), (gs / kSmallBufs) & 1);
+                    DBG_REC(4, gs - 150, lane == 0 && q == 0 && gs >= 150);
                     tc_fence_after();
                     uint32_t r[32];
                     tc_ld32(t_lane + kSmallCol + sb * 32, r);
@@ -496,11 +546,13 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar(B_SMALL_EMPTY + sb));
+                    DBG_REC(5, gs - 150, lane == 0 && q == 0 && gs >= 150);
                     uint32_t o[16];
 #pragma unroll
                     for (int i = 0; i < 16; ++i)   // b1 is already in the accumulator (bias columns of W1)
-                        o[i] = pack_act(gelu_fast(__uint_as_float(r[2 * i])), gelu_fast(__uint_as_float(r[2 * i + 1])));
+                        o[i] = gelu_h2(pack_act(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1])));
                     const uint32_t slot = ac % kA1Slots;
+                    DBG_REC(6, ac - 150, lane == 0 && q == 0 && ac >= 150);
                     mbar_wait(bar(B_A1_EMPTY + slot), ((ac / kA1Slots) & 1) ^ 1);
                     const uint32_t base = s_r1 + (slot >> 1) * kChunkBytes;
 #pragma unroll
@@ -509,6 +561,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                     fence_proxy_async_smem();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar(B_A1_FULL + slot));
+                    DBG_REC(7, ac - 150, lane == 0 && q == 0 && ac >= 150);
                 }
                 // drain D2 (this half): +b2, GELU, fp16 -> H2 scratch in the chunk images phase B loads
                 mbar_wait(bar(B_ACC_FULL), af & 1);
@@ -853,3 +906,9 @@ df_status launch_ann_bf16(const df_ann* ann, const df_mech* mech, long long n, l
     return DF_OK;
 }
 
+
+#ifdef DF_DBG_CLK
+extern "C" __attribute__((visibility("default"))) int df_debug_read(long long* out) {
+    return (int)cudaMemcpyFromSymbol(out, g_dbg, sizeof(g_dbg));
+}
+#endif
