@@ -66,7 +66,7 @@ struct NetGeom {
     int w2_tile_bytes, w3_tile_bytes, w_slot_bytes, w4_bytes;
     int smem_bytes;
     // shared-memory offsets (bytes from the 1024-aligned base)
-    int off_w, off_r1, off_r2, off_w4, off_bar;
+    int off_w, off_r1, off_r2, off_w4, off_bar, off_cell;  // off_cell: raw T, p, Y of the tile, [K+2][128] fp32
 };
 
 struct Bf16Dev {
@@ -82,6 +82,7 @@ struct Bf16Dev {
 struct Bf16Plan {
     NetGeom g;
     Bf16Dev d;
+    float b4_host[32] = {0};
     void* blob = nullptr;
     int num_sms = 0;
 };
@@ -203,6 +204,19 @@ __device__ __forceinline__ uint32_t gelu_h2(uint32_t v) {
         : "r"(v), "r"(0x28912891u) /* 0.035677 */, "r"(0x3A623A62u) /* 0.79788 */, "r"(0x38003800u) /* 0.5 */);
     return r;
 }
+// dY*_k of ann_common.cuh with MUFU-grade transcendentals (ex2/lg2/rcp.approx): 5 MUFU + a few FMA per species
+// instead of powf/log1pf/expm1f (~400 instructions).  Its error (<= 2e-4 relative for |lambda Delta| >= 1e-3 Y^lambda)
+// is far inside the 2e-2 budget of this path; the fp32 path (ann_fp32.cu) keeps the accurate form.
+__device__ __forceinline__ float ann_dystar_fast(float y, float delta, float lambda, float inv_lambda) {
+    if (y > 0.f) {
+        const float q = exp2f(lambda * __log2f(y));
+        const float z = lambda * delta * rcp_approx(q);
+        if (!(z > -1.0f)) return -y;
+        return y * (exp2f(__log2f(1.0f + z) * inv_lambda) - 1.0f);
+    }
+    const float base = lambda * delta;
+    return base > 0.f ? exp2f(__log2f(base) * inv_lambda) : 0.f;
+}
 // two fp32 -> packed fp16x2 (first argument in the low half = lower K index)
 __device__ __forceinline__ uint32_t pack_act(float lo, float hi) {
     uint32_t r;
@@ -237,13 +251,13 @@ enum {
     B_A0_FULL = B_W1_EMPTY + 2, B_SMALL_FULL, B_SMALL_EMPTY = B_SMALL_FULL + kSmallBufs,
     B_A1_FULL = B_SMALL_EMPTY + kSmallBufs, B_A1_EMPTY = B_A1_FULL + kA1Slots, B_ACC_FULL = B_A1_EMPTY + kA1Slots, B_ACC_EMPTY,
     B_H2_FULL, B_H2C_FULL, B_H2C_EMPTY = B_H2C_FULL + 2, B_H3_FULL = B_H2C_EMPTY + 2, B_H3_EMPTY = B_H3_FULL + 2, B_TILE_DONE = B_H3_EMPTY + 2,
-    B_W4_FULL, B_ACC_START, B_COUNT
+    B_W4_FULL, B_ACC_START, B_FINAL_DONE, B_COUNT
 };
 
 struct KArgs {
     NetGeom g;
     Bf16Dev d;
-    const float* invW;
+    float invW[32], b4[32];   // 1/W_k and the last layer's bias as constant-bank operands of the final epilogue
     long long n, ld;
     const float *T, *p, *Y;
     float *omega, *dY;
@@ -270,6 +284,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             if ((i >= B_SMALL_EMPTY && i < B_SMALL_EMPTY + kSmallBufs) || (i >= B_A1_FULL && i < B_A1_FULL + kA1Slots)) cnt = 4;
             if (i == B_A0_FULL || i == B_ACC_EMPTY || i == B_H3_FULL || i == B_H3_FULL + 1) cnt = 4 * kGroups;
             if (i == B_H2_FULL) cnt = 8 * kGroups;
+            if (i == B_FINAL_DONE) cnt = 4;
             if (i == B_ACC_FULL || i == B_H2C_EMPTY || i == B_H2C_EMPTY + 1) cnt = 2;  // one commit per issuer
             mbar_init(bar(i), cnt);
         }
@@ -483,6 +498,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
         uint8_t* scratch = a.scratch + (size_t)blockIdx.x * g.NKC * kChunkBytes;
         uint32_t gs = 0, ac = 0, af = 0, h3c = 0;
         const float lam = nm.lambda, inv_lam = nm.inv_lambda;
+        float* cellbuf = reinterpret_cast<float*>(sgen + g.off_cell);  // [K+2][128]: T, p, Y_k of this tile's cells
 
         auto st_shared16 = [&](uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
             asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
@@ -498,10 +514,27 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             const long long cell = tile * kTileM + row;
             const bool valid = cell < a.n;
             // A0 shares its shared memory with the first H3 slot: the previous tile's layer-4 MMAs must be done
-            if (tcnt > 0) mbar_wait(bar(B_TILE_DONE), (tcnt - 1) & 1);
+            DBG_REC(12, tcnt * 16 + 0, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
+            if (tcnt > 0) {
+                mbar_wait(bar(B_TILE_DONE), (tcnt - 1) & 1);
+                mbar_wait(bar(B_FINAL_DONE), (tcnt - 1) & 1);  // the previous final epilogue has read the cell buffer
+            }
+            DBG_REC(12, tcnt * 16 + 1, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
             // ---- prologue: features + two bias columns of ones -> fp16 A0 [128 x 32]; group grp writes
             //      feature columns [8 grp, 8 grp + 8) ----
             for (int fc = grp; fc < 4; fc += kGroups) {
+                // issue the 8 loads of this feature chunk first (clamped addresses), then do the arithmetic
+                float raw[8];
+                const long long cl = valid ? cell : 0;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const int f = fc * 8 + j;
+                    raw[j] = (f == 0) ? __ldg(a.T + cl) : (f == 1) ? __ldg(a.p + cl)
+                           : (f < g.K + 2) ? __ldg(a.Y + (size_t)(f - 2) * a.ld + cl) : 0.f;
+                }
+#pragma unroll
+                for (int j = 0; j < 8; ++j)
+                    if (fc * 8 + j < g.K + 2) cellbuf[(fc * 8 + j) * kTileM + row] = raw[j];
                 uint32_t o[4];
 #pragma unroll
                 for (int i = 0; i < 4; ++i) {
@@ -512,16 +545,14 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                         float x = 0.f;
                         if (f < g.K + 2) {
                             if (valid) {
-                                if (f == 0) x = (__ldg(a.T + cell) - nm.x_mean[0]) * nm.x_inv_std[0];
-                                else if (f == 1) x = (__ldg(a.p + cell) - nm.x_mean[1]) * nm.x_inv_std[1];
+                                if (f < 2) x = (raw[2 * i + e] - nm.x_mean[f]) * nm.x_inv_std[f];
                                 else {
-                                    const float y = __ldg(a.Y + (size_t)(f - 2) * a.ld + cell);
-                                    const float qy = exp2f(lam * __log2f(y));  // y^lambda, 0 -> 0
+                                    const float qy = exp2f(lam * __log2f(raw[2 * i + e]));  // y^lambda, 0 -> 0
                                     x = ((qy - 1.0f) * inv_lam - nm.x_mean[f]) * nm.x_inv_std[f];
                                 }
                             }
                         } else if (f < g.K + 4) {
-                            x = 1.0f;  // multiplies the bf16 hi / lo parts of b1 stored as W1 columns K+2, K+3
+                            x = 1.0f;  // multiplies the hi / lo parts of b1 (and b2, b3) stored as weight columns K+2, K+3
                         }
                         v[e] = x;
                     }
@@ -532,6 +563,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             fence_proxy_async_smem();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(B_A0_FULL));
+            DBG_REC(12, tcnt * 16 + 2, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
             // ---- phase A ----
             for (int h = 0; h < 2; ++h) {
                 for (int c = 0; c < g.NC; ++c, ++gs, ++ac) {
@@ -564,8 +596,10 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                     DBG_REC(7, ac - 150, lane == 0 && q == 0 && ac >= 150);
                 }
                 // drain D2 (this half): +b2, GELU, fp16 -> H2 scratch in the chunk images phase B loads
+                DBG_REC(12, tcnt * 16 + 3 + 3 * h, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
                 mbar_wait(bar(B_ACC_FULL), af & 1);
                 ++af;
+                DBG_REC(12, tcnt * 16 + 4 + 3 * h, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
                 tc_fence_after();
                 {
                     // software-pipelined: the TMEM load of the next 16-column unit is in flight during the math
@@ -602,10 +636,13 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                     mbar_arrive(bar(B_ACC_EMPTY));
                     mbar_arrive(bar(B_H2_FULL));
                 }
+                DBG_REC(12, tcnt * 16 + 5 + 3 * h, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
             }
             // ---- phase B: drain D3 in 64-wide chunks -> H3 ring (feeds layer 4); group grp owns 16-column unit grp ----
+            DBG_REC(12, tcnt * 16 + 9, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
             mbar_wait(bar(B_ACC_FULL), af & 1);
             ++af;
+            DBG_REC(12, tcnt * 16 + 10, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
             tc_fence_after();
             for (int jj = 0; jj < g.NJ; ++jj, ++h3c) {
                 // 16-column units u = grp, grp + kGroups, ... of this 64-wide chunk (at most two per group)
@@ -639,6 +676,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(B_ACC_EMPTY));
+            DBG_REC(12, tcnt * 16 + 11, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
             // ---- final epilogue (group 0): D4 -> Delta -> inverse Box-Cox -> renormalise -> omega (A9-A11, A17) ----
             const uint32_t sb = gs % kSmallBufs;
             const uint32_t spar = (gs / kSmallBufs) & 1;
@@ -652,34 +690,39 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar(B_SMALL_EMPTY + sb));
+                DBG_REC(12, tcnt * 16 + 12, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
                 if (valid) {
-                    const float T = __ldg(a.T + cell), p = __ldg(a.p + cell);
+                    // T, p, Y come from the cell buffer the prologue filled; 1/W, b4 and the z-score tables are kernel
+                    // parameters: no global load in this block (with 227 KB of shared memory there is no L1 to hit)
+                    const float T = cellbuf[row], p = cellbuf[kTileM + row];
                     double sumYm1 = -1.0, sumd = 0.0;
                     float inv_Wbar = 0.f;
 #pragma unroll
                     for (int k = 0; k < 32; ++k) {
                         if (k < g.K) {
-                            const float ok = __uint_as_float(r[k]) + __ldg(a.d.b4 + k);
-                            const float y = __ldg(a.Y + (size_t)k * a.ld + cell);
-                            const float d = ann_dystar(y, fmaf(nm.u_std[k], ok, nm.u_mean[k]), lam, inv_lam);
+                            const float y = cellbuf[(2 + k) * kTileM + row];
+                            const float ok = __uint_as_float(r[k]) + a.b4[k];
+                            const float d = ann_dystar_fast(y, fmaf(nm.u_std[k], ok, nm.u_mean[k]), lam, inv_lam);
                             r[k] = __float_as_uint(d);
                             sumYm1 += (double)y;
                             sumd += (double)d;
-                            inv_Wbar = fmaf(y, __ldg(a.invW + k), inv_Wbar);
+                            inv_Wbar = fmaf(y, a.invW[k], inv_Wbar);
                         }
                     }
-                    const double Sm1 = sumYm1 + sumd, inv_S = 1.0 / (1.0 + Sm1);
+                    // S - 1 in fp64 (it is a difference of O(1) sums); the per-species update in fp32 (2e-2 path)
+                    const float Sm1 = (float)(sumYm1 + sumd), inv_S = 1.0f / (1.0f + Sm1);
                     const float rho_dt = p / (inv_Wbar * (float)DF_R_UNIVERSAL * T) * nm.inv_dt;
 #pragma unroll
                     for (int k = 0; k < 32; ++k) {
                         if (k < g.K) {
-                            const float y = __ldg(a.Y + (size_t)k * a.ld + cell);
-                            const float d = ann_renorm_dY(__uint_as_float(r[k]), y, Sm1, inv_S);
+                            const float d = (__uint_as_float(r[k]) - cellbuf[(2 + k) * kTileM + row] * Sm1) * inv_S;
                             if (a.dY) a.dY[(size_t)k * a.ld + cell] = d;
                             if (a.omega) a.omega[(size_t)k * a.ld + cell] = rho_dt * d;
                         }
                     }
                 }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(B_FINAL_DONE));
             }
         }
     }
@@ -762,7 +805,8 @@ df_status ann_bf16_create(df_ann* ann, const float* const* W, const float* const
     g.off_r2 = g.off_r1 + kA1Tiles * kChunkBytes;
     g.off_w4 = g.off_r2 + 2 * kChunkBytes;
     g.off_bar = g.off_w4 + g.w4_bytes;
-    g.smem_bytes = g.off_bar + B_COUNT * 8 + 16 + 1024;
+    g.off_cell = (g.off_bar + B_COUNT * 8 + 16 + 127) / 128 * 128;
+    g.smem_bytes = g.off_cell + (K + 2) * kTileM * (int)sizeof(float) + 1024;
     if (g.smem_bytes > 227 * 1024) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: layer widths need %d B of shared memory", g.smem_bytes);
 
     int dev = 0;
@@ -853,6 +897,7 @@ df_status ann_bf16_create(df_ann* ann, const float* const* W, const float* const
     memcpy(hb + d1, b[1], sizeof(float) * d2);
     memcpy(hb + d1 + d2, b[2], sizeof(float) * d3);
     memcpy(hb + d1 + d2 + d3, b[3], sizeof(float) * K);
+    memcpy(P->b4_host, b[3], sizeof(float) * K);
 
     if (cudaMalloc(&P->blob, blob.size()) != cudaSuccess) return df_set_error(DF_ERR_ALLOC, "bf16 path: cudaMalloc of %zu bytes failed", blob.size());
     DF_CUDA_TRY(cudaMemcpy(P->blob, blob.data(), blob.size(), cudaMemcpyHostToDevice));
@@ -894,7 +939,8 @@ df_status launch_ann_bf16(const df_ann* ann, const df_mech* mech, long long n, l
     KArgs a;
     a.g = P->g;
     a.d = P->d;
-    a.invW = mech->dev.invW;
+    for (int k = 0; k < 32; ++k) a.invW[k] = k < mech->K ? (float)(1.0 / mech->W_host[k]) : 0.f;
+    memcpy(a.b4, P->b4_host, sizeof(a.b4));
     a.n = n;
     a.ld = ld;
     a.T = T; a.p = p; a.Y = Y;
