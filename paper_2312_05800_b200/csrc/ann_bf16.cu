@@ -609,8 +609,14 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                         const int gc = h * g.NH + c0;
                         uint8_t* dst = scratch + (size_t)(gc >> 6) * kChunkBytes;
                         const int c16 = (gc & 63) >> 3;
-                        *reinterpret_cast<uint4*>(dst + swz(row, c16)) = make_uint4(o[0], o[1], o[2], o[3]);
-                        *reinterpret_cast<uint4*>(dst + swz(row, c16 + 1)) = make_uint4(o[4], o[5], o[6], o[7]);
+                        // the two 16-byte chunks of a 16-column unit share one 32-byte sector of the swizzled row (their
+                        // order inside it depends on the row parity): one 256-bit store instead of two scattered 128-bit ones
+                        const bool sw = row & 1;
+                        uint8_t* d32 = dst + row * 128 + (((c16 ^ (row & 7)) & ~1) << 4);
+                        asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(d32), "r"(sw ? o[4] : o[0]),
+                                     "r"(sw ? o[5] : o[1]), "r"(sw ? o[6] : o[2]), "r"(sw ? o[7] : o[3]), "r"(sw ? o[0] : o[4]),
+                                     "r"(sw ? o[1] : o[5]), "r"(sw ? o[2] : o[6]), "r"(sw ? o[3] : o[7])
+                                     : "memory");
                     };
                     constexpr int kStep = 16 * kGroups;
                     uint32_t ra[16], rb[16];
@@ -628,6 +634,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                         c0 += kStep;
                     }
                 }
+                DBG_REC(12, tcnt * 16 + 13 + h, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
                 tc_fence_before();
                 __threadfence();
                 fence_proxy_async();
