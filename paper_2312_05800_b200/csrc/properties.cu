@@ -17,128 +17,189 @@ namespace {
 constexpr int kThreads = 128;
 
 // ------------------------------------------------------------------------------------------------
-// fixed K
+// fixed K: two cells per thread, packed fp32x2 arithmetic
 // ------------------------------------------------------------------------------------------------
+// sm_100a has no constant-bank operand form for FFMA: every table coefficient costs a share of an LDCU/LDC issue
+// slot.  Two adjacent cells per thread, held as float2 and updated with FFMA2 (fma.rn.f32x2, whose third form
+// broadcasts one scalar uniform register to both halves), halve both the FMA issue slots and the coefficient loads
+// per cell.
+typedef float2 f2;
+__device__ __forceinline__ f2 bc(float s) { return make_float2(s, s); }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ f2 fma2(f2 a, float s, f2 c) { return __ffma2_rn(a, bc(s), c); }
+__device__ __forceinline__ f2 fma2(float s, f2 a, f2 c) { return __ffma2_rn(bc(s), a, c); }
+__device__ __forceinline__ f2 fma2(f2 a, float s, float c) { return __ffma2_rn(a, bc(s), bc(c)); }
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ f2 mul2(f2 a, float s) { return __fmul2_rn(a, bc(s)); }
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ f2 rcp2(f2 a) { return make_float2(rcp_approx(a.x), rcp_approx(a.y)); }
+__device__ __forceinline__ f2 poly4_2(const float* c, f2 u) {
+    return fma2(fma2(fma2(fma2(u, c[4], c[3]), u, bc(c[2])), u, bc(c[1])), u, bc(c[0]));
+}
+
+#ifndef DF_PROPS_MINBLOCKS
+#define DF_PROPS_MINBLOCKS 4
+#endif
 template <int K, bool TRANSPORT>
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kThreads, DF_PROPS_MINBLOCKS)
 props_fixed_kernel(const __grid_constant__ PropTables<K> tab, long long n, long long ld,
                    const float* __restrict__ Tg, const float* __restrict__ pg, const float* __restrict__ Yg,
                    float* __restrict__ cp_o, float* __restrict__ h_o, float* __restrict__ mu_o,
                    float* __restrict__ lam_o, float* __restrict__ D_o) {
-    const long long i = (long long)blockIdx.x * kThreads + threadIdx.x;
+    const long long i = ((long long)blockIdx.x * kThreads + threadIdx.x) * 2;
     if (i >= n) return;
-    const float T = __ldg(Tg + i);
-    float Y[K];
+    const bool two = (i + 1 < n);   // ld % 4 == 0 and 16-byte aligned bases make the float2 accesses legal
+    auto ld2 = [&](const float* p) -> f2 {
+        if (two) return __ldg(reinterpret_cast<const float2*>(p + i));
+        const float v = __ldg(p + i);
+        return make_float2(v, v);
+    };
+    auto st2 = [&](float* p, f2 v) {
+        if (two) *reinterpret_cast<float2*>(p + i) = v;
+        else p[i] = v.x;
+    };
+    const f2 T = ld2(Tg);
+    f2 Y[K];
 #pragma unroll
-    for (int k = 0; k < K; ++k) Y[k] = __ldg(Yg + (size_t)k * ld + i);
+    for (int k = 0; k < K; ++k) Y[k] = ld2(Yg + (size_t)k * ld);
 
     // ---- thermo: mixture polynomial in tau, both ranges, select at the end ---------------------
-    const float tau = (T - tab.sc.T_mid) * tab.sc.inv_S;
-    const bool lo = T < tab.sc.T_mid;  // A2: hi for T >= T_mid
+    const f2 tau = mul2(add2(T, bc(-tab.sc.T_mid)), tab.sc.inv_S);
+    const bool lo0 = T.x < tab.sc.T_mid, lo1 = T.y < tab.sc.T_mid;  // A2: hi for T >= T_mid
     if (cp_o || h_o) {
-        float Cl[5] = {0.f, 0.f, 0.f, 0.f, 0.f}, Ch[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
-        double H0l = 0.0, H0h = 0.0;
+        f2 Cl[5], Ch[5];
+#pragma unroll
+        for (int m = 0; m < 5; ++m) Cl[m] = Ch[m] = bc(0.f);
+        double H0l0 = 0.0, H0h0 = 0.0, H0l1 = 0.0, H0h1 = 0.0;
 #pragma unroll
         for (int k = 0; k < K; ++k) {
 #pragma unroll
             for (int m = 0; m < 5; ++m) {
-                Cl[m] = fmaf(Y[k], tab.th[k][0][m], Cl[m]);
-                Ch[m] = fmaf(Y[k], tab.th[k][1][m], Ch[m]);
+                Cl[m] = fma2(Y[k], tab.th[k][0][m], Cl[m]);
+                Ch[m] = fma2(Y[k], tab.th[k][1][m], Ch[m]);
             }
-            const double yd = (double)Y[k];
-            H0l = fma(yd, tab.h0[k][0], H0l);
-            H0h = fma(yd, tab.h0[k][1], H0h);
+            H0l0 = fma((double)Y[k].x, tab.h0[k][0], H0l0);
+            H0h0 = fma((double)Y[k].x, tab.h0[k][1], H0h0);
+            H0l1 = fma((double)Y[k].y, tab.h0[k][0], H0l1);
+            H0h1 = fma((double)Y[k].y, tab.h0[k][1], H0h1);
         }
-        float q[5];
+        f2 q[5];
 #pragma unroll
-        for (int m = 0; m < 5; ++m) q[m] = lo ? Cl[m] : Ch[m];
-        const float sens = tau * fmaf(fmaf(fmaf(fmaf(q[4], tau, q[3]), tau, q[2]), tau, q[1]), tau, q[0]);
-        if (h_o) h_o[i] = (float)((lo ? H0l : H0h) + (double)sens);
+        for (int m = 0; m < 5; ++m) q[m] = make_float2(lo0 ? Cl[m].x : Ch[m].x, lo1 ? Cl[m].y : Ch[m].y);
+        const f2 sens = mul2(tau, fma2(fma2(fma2(fma2(q[4], tau, q[3]), tau, q[2]), tau, q[1]), tau, q[0]));
+        if (h_o)
+            st2(h_o, make_float2((float)((lo0 ? H0l0 : H0h0) + (double)sens.x), (float)((lo1 ? H0l1 : H0h1) + (double)sens.y)));
         if (cp_o)
-            cp_o[i] = fmaf(fmaf(fmaf(fmaf(5.f * q[4], tau, 4.f * q[3]), tau, 3.f * q[2]), tau, 2.f * q[1]), tau, q[0]) *
-                      tab.sc.inv_S;
+            st2(cp_o, mul2(fma2(fma2(fma2(fma2(mul2(q[4], 5.f), tau, mul2(q[3], 4.f)), tau, mul2(q[2], 3.f)), tau,
+                                     mul2(q[1], 2.f)), tau, q[0]),
+                           tab.sc.inv_S));
     }
     if (!TRANSPORT) return;
 
     // ---- mole fractions -----------------------------------------------------------------------
-    float X[K];
-    float sumx = 0.f;
+    f2 X[K];
+    f2 sumx = bc(0.f);
 #pragma unroll
     for (int k = 0; k < K; ++k) {
-        X[k] = Y[k] * tab.invW[k];
-        sumx += X[k];
+        X[k] = mul2(Y[k], tab.invW[k]);
+        sumx = add2(sumx, X[k]);
     }
-    const float inv_sumx = 1.0f / sumx;
+    const f2 inv_sumx = make_float2(1.0f / sumx.x, 1.0f / sumx.y);
 #pragma unroll
-    for (int k = 0; k < K; ++k) X[k] *= inv_sumx;
+    for (int k = 0; k < K; ++k) X[k] = mul2(X[k], inv_sumx);
 
-    const float u = (logf(T) - tab.sc.Lc) * tab.sc.inv_Ls;
-    const float sqrtT = sqrtf(T);
+    const f2 u = mul2(add2(make_float2(logf(T.x), logf(T.y)), bc(-tab.sc.Lc)), tab.sc.inv_Ls);
+    const f2 sqrtT = make_float2(sqrtf(T.x), sqrtf(T.y));
 
     // ---- Wilke viscosity ----------------------------------------------------------------------
     if (mu_o) {
-        float g[K], b2[K], c[K];
+#ifdef DF_WILKE_3VEC
+        f2 g[K], b2[K], c[K];
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-            g[k] = poly4(tab.visc[k], u);
-            const float rg = rcp_approx(g[k]);
-            const float xr = X[k] * rg;
-            b2[k] = 2.f * xr;
-            c[k] = xr * rg;
+            g[k] = poly4_2(tab.visc[k], u);
+            const f2 rg = rcp2(g[k]);
+            const f2 xr = mul2(X[k], rg);
+            b2[k] = add2(xr, xr);
+            c[k] = mul2(xr, rg);
         }
-        float acc = 0.f;
+        f2 acc = bc(0.f);
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-            float den = 0.f;
+            f2 den = bc(0.f);
 #pragma unroll
-            for (int j = 0; j < K; ++j) den = fmaf(tab.B[k][j], fmaf(g[k], fmaf(g[k], c[j], b2[j]), X[j]), den);
-            acc = fmaf(X[k] * tab.sqrtW[k] * g[k] * g[k], rcp_approx(den), acc);
+            for (int j = 0; j < K; ++j) den = fma2(tab.B[k][j], fma2(g[k], fma2(g[k], c[j], b2[j]), X[j]), den);
+            acc = fma2(mul2(mul2(X[k], tab.sqrtW[k]), mul2(g[k], g[k])), rcp2(den), acc);
         }
-        mu_o[i] = sqrtT * acc;
+#else
+        // Phi_kj = B_kj (1 + g_k/g_j)^2 with only two per-species vectors live (X_j and r_j = 1/g_j): 4 packed
+        // instructions per (k,j) instead of the 3 of the three-vector form, but 76 registers less, which buys the
+        // occupancy this latency-sensitive kernel needs
+        f2 r[K];
+#pragma unroll
+        for (int k = 0; k < K; ++k) r[k] = rcp2(poly4_2(tab.visc[k], u));
+        f2 acc = bc(0.f);
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const f2 gk = rcp2(r[k]);
+            f2 den = bc(0.f);
+#pragma unroll
+            for (int j = 0; j < K; ++j) {
+                const f2 t = fma2(gk, r[j], bc(1.0f));
+                den = fma2(mul2(X[j], mul2(t, t)), tab.B[k][j], den);
+            }
+            acc = fma2(mul2(mul2(X[k], tab.sqrtW[k]), mul2(gk, gk)), rcp2(den), acc);
+        }
+#endif
+        st2(mu_o, mul2(sqrtT, acc));
     }
 
     // ---- combination-rule conductivity (A6) ---------------------------------------------------
     if (lam_o) {
-        float s1 = 0.f, s2 = 0.f;
+        f2 s1 = bc(0.f), s2 = bc(0.f);
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-            const float lk = poly4(tab.cond[k], u);
-            s1 = fmaf(X[k], lk, s1);
-            s2 = fmaf(X[k], rcp_approx(lk), s2);
+            const f2 lk = poly4_2(tab.cond[k], u);
+            s1 = fma2(X[k], lk, s1);
+            s2 = fma2(X[k], rcp2(lk), s2);
         }
-        lam_o[i] = 0.5f * sqrtT * (s1 + rcp_approx(s2));
+        st2(lam_o, mul2(mul2(sqrtT, 0.5f), add2(s1, rcp2(s2))));
     }
 
     // ---- mixture-averaged diffusivities (A7) ---------------------------------------------
     if (D_o) {
-        const float p = __ldg(pg + i);
-        const float scale = T * sqrtT / p;
-        float S[K];
+        const f2 p = ld2(pg);
+        const f2 scale = make_float2(T.x * sqrtT.x / p.x, T.y * sqrtT.y / p.y);
+        f2 S[K];
 #pragma unroll
-        for (int k = 0; k < K; ++k) S[k] = 0.f;
+        for (int k = 0; k < K; ++k) S[k] = bc(0.f);
         {
             int idx = 0;
 #pragma unroll
             for (int j = 0; j < K; ++j)
 #pragma unroll
                 for (int k = j + 1; k < K; ++k, ++idx) {
-                    const float r = rcp_approx(poly4(tab.dpair[idx], u));
-                    S[k] = fmaf(X[j], r, S[k]);
-                    S[j] = fmaf(X[k], r, S[j]);
+                    const f2 r = rcp2(poly4_2(tab.dpair[idx], u));
+                    S[k] = fma2(X[j], r, S[k]);
+                    S[j] = fma2(X[k], r, S[j]);
                 }
         }
-        // N_k = sum_{j != k} Y_j as prefix + suffix (never 1 - Y_k: cancels when Y_k -> 1)
-        float suf[K + 1];
-        suf[K] = 0.f;
+        // N_k = sum_{j != k} Y_j as prefix + suffix (never 1 - Y_k: cancels when Y_k -> 1).  Y is re-read here (L2 hit)
+        // instead of being kept live through the Wilke block: 38 registers less at the kernel's pressure peak.
 #pragma unroll
-        for (int k = K - 1; k >= 0; --k) suf[k] = suf[k + 1] + Y[k];
-        float pre = 0.f;
+        for (int k = 0; k < K; ++k) Y[k] = ld2(Yg + (size_t)k * ld);
+        f2 suf[K + 1];
+        suf[K] = bc(0.f);
+#pragma unroll
+        for (int k = K - 1; k >= 0; --k) suf[k] = add2(suf[k + 1], Y[k]);
+        f2 pre = bc(0.f);
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-            const float Nk = pre + suf[k + 1];
-            pre += Y[k];
-            const float Dk = (S[k] > 0.f) ? Nk / S[k] : poly4(tab.ddiag[k], u);
-            D_o[(size_t)k * ld + i] = Dk * scale;
+            const f2 Nk = add2(pre, suf[k + 1]);
+            pre = add2(pre, Y[k]);
+            const f2 dk = poly4_2(tab.ddiag[k], u);
+            const f2 Dk = make_float2(S[k].x > 0.f ? Nk.x / S[k].x : dk.x, S[k].y > 0.f ? Nk.y / S[k].y : dk.y);
+            st2(D_o + (size_t)k * ld, mul2(Dk, scale));
         }
     }
 }
@@ -255,7 +316,7 @@ props_generic_kernel(MechDev md, long long n, long long ld, const float* __restr
 template <int K>
 df_status launch_fixed(const PropTables<K>* tab, long long n, long long ld, const float* T, const float* p,
                        const float* Y, float* cp, float* h, float* mu, float* lam, float* D, cudaStream_t s) {
-    const unsigned blocks = (unsigned)((n + kThreads - 1) / kThreads);
+    const unsigned blocks = (unsigned)((n + 2 * kThreads - 1) / (2 * kThreads));
     if (mu || lam || D)
         props_fixed_kernel<K, true><<<blocks, kThreads, 0, s>>>(*tab, n, ld, T, p, Y, cp, h, mu, lam, D);
     else
