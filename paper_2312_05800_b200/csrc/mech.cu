@@ -175,6 +175,51 @@ extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const
         df_mech_destroy(mech);
         return st;
     }
+    {   // padded / tiled tables of the any-K kernel
+        const int Kp = (K + 7) / 8 * 8, nt = Kp / 8;
+        d.Kp = Kp;
+        std::vector<float> small((size_t)Kp * 24, 0.f), thp((size_t)Kp * 12, 0.f), BT((size_t)Kp * Kp, 1.f);
+        std::vector<double> h0p((size_t)Kp * 2, 0.0);
+        std::vector<float> dt((size_t)nt * (nt + 1) / 2 * 64 * 8, 0.f);
+        for (int k = 0; k < Kp; ++k) {
+            float* sp = &small[(size_t)k * 24];
+            if (k < K) {
+                sp[0] = t.invW[k];
+                sp[1] = t.sqrtW[k];
+                for (int m = 0; m < 5; ++m) {
+                    sp[2 + m] = t.visc[k * 5 + m];
+                    sp[7 + m] = t.cond[k * 5 + m];
+                    sp[12 + m] = t.ddiag[k * 5 + m];
+                }
+                for (int i = 0; i < 12; ++i) thp[(size_t)k * 12 + i] = t.th32[(size_t)k * 12 + i];
+                h0p[k * 2] = t.th64[(size_t)(k * 2) * 6];
+                h0p[k * 2 + 1] = t.th64[(size_t)(k * 2 + 1) * 6];
+            } else {
+                sp[2] = 1.f;   // g = 1
+                sp[7] = 1.f;   // lambda_k = 1 (X_k = 0 anyway)
+                sp[12] = 1.f;
+            }
+        }
+        for (int j = 0; j < K; ++j)
+            for (int k = 0; k < K; ++k) BT[(size_t)j * Kp + k] = t.wilkeB[(size_t)k * K + j];
+        size_t tix = 0;
+        for (int kt = 0; kt < nt; ++kt)
+            for (int jt = kt; jt < nt; ++jt, ++tix)
+                for (int a = 0; a < 8; ++a)
+                    for (int b = 0; b < 8; ++b) {
+                        float* c = &dt[((tix * 8 + a) * 8 + b) * 8];
+                        const int k = kt * 8 + a, j = jt * 8 + b;
+                        if (k < K && j < K)
+                            for (int m = 0; m < 5; ++m) c[m] = t.dfull[((size_t)k * K + j) * 5 + m];
+                        else
+                            c[0] = 1.f;
+                    }
+        if ((st = to_device(&d.small_p, small)) || (st = to_device(&d.thp, thp)) || (st = to_device(&d.h0p, h0p)) ||
+            (st = to_device(&d.BT, BT)) || (st = to_device(&d.dtile, dt))) {
+            df_mech_destroy(mech);
+            return st;
+        }
+    }
     if (K == 9) mech->t9 = make_fixed<9>(t);
     if (K == 19) mech->t19 = make_fixed<19>(t);
     *out = mech;
@@ -193,6 +238,11 @@ extern "C" df_status df_mech_destroy(df_mech* mech) {
     cudaFree(d.ddiag);
     cudaFree(d.dfull);
     cudaFree(d.wilkeB);
+    cudaFree(d.small_p);
+    cudaFree(d.thp);
+    cudaFree(d.h0p);
+    cudaFree(d.BT);
+    cudaFree(d.dtile);
     delete mech->t9;
     delete mech->t19;
     delete mech;
