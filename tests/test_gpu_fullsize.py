@@ -1,0 +1,115 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times: the kernels run on the whole
+field, the oracle on a strided sample of cells (plus the whole ragged tail), and size-independent properties
+(sum-to-one, positivity, convergence counter) are checked on every cell."""
+import numpy as np
+import pytest
+
+from tests import helpers
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2312_05800_b200 import binding
+    return binding
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def sample_idx(n, m=4096):
+    return np.unique(np.concatenate([np.arange(0, n, max(1, n // m)), np.arange(max(0, n - 300), n)]))
+
+
+def test_cfg3_full_pipeline(B):
+    """configs[2]: 2,097,152 cells, K = 19, T_from_h -> properties -> 16-bit tensor MLP, as bench.py runs it."""
+    from oracle import oracle
+    from paper_2312_05800_b200 import synth
+    n, K = 2097152, 19
+    mech, ann, cells = synth.make_config(3)
+    om, oa = oracle.Mech(mech), oracle.Ann(ann)
+    gm, ga = B.Mech(mech), B.Ann(ann)
+    T0, p, Y = dev(cells.T), dev(cells.p), dev(cells.Y)
+    h = torch.empty(n, device="cuda")
+    B.df_thermo_properties(gm, T0, p, Y, h=h)              # the enthalpy field a solver would hold
+    T = dev(cells.T_guess)
+    cnt = torch.zeros(1, dtype=torch.int32, device="cuda")
+    mu, lam = torch.empty(n, device="cuda"), torch.empty(n, device="cuda")
+    D, omega, dY = (torch.empty(K, n, device="cuda") for _ in range(3))
+    B.df_thermo_T_from_h(gm, h, Y, T, n_unconverged=cnt)
+    B.df_thermo_properties(gm, T, p, Y, mu=mu, lam=lam, D=D)
+    B.df_chem_ann_source(ga, gm, T, p, Y, omega=omega, dY=dY, workspace=B.alloc_workspace(ga, n))
+    torch.cuda.synchronize()
+    assert int(cnt.item()) == 0
+    # properties that hold at any size, every cell
+    s = (Y.double() + dY.double()).sum(dim=0)
+    assert float((s - 1.0).abs().max()) <= 2e-6
+    assert bool((D > 0).all()) and bool((mu > 0).all()) and bool((lam > 0).all())
+    # sampled cells against the oracle (A20: properties / ANN judged at the fp32 T the Newton call wrote)
+    idx = sample_idx(n)
+    hs, Ys, Ts = h.cpu().numpy()[idx], np.ascontiguousarray(cells.Y[:, idx]), T.cpu().numpy()[idx]
+    T_ref = om.T_from_h(hs, Ys, cells.T_guess[idx])
+    assert np.abs(Ts - T_ref).max() <= 1e-3
+    ref = om.properties(Ts, cells.p[idx], Ys)
+    for name, got in (("mu", mu), ("lam", lam)):
+        assert helpers.rel_err(got.cpu().numpy()[idx], ref[name]).max() <= 1e-5, name
+    assert helpers.rel_err(D.cpu().numpy()[:, idx], ref["D"][:, :len(idx)]).max() <= 1e-5
+    om_r, dY_r = oa.source(om, Ts, cells.p[idx], Ys)
+    for name, got, r in (("dY", dY, dY_r), ("omega", omega, om_r)):
+        mixed, norm = helpers.mixed_err(got.cpu().numpy()[:, idx], r[:, :len(idx)])
+        assert norm <= 2e-2 and mixed <= 1e-1, f"{name}: mixed {mixed:.3e} normwise {norm:.3e}"
+
+
+def test_cfg4_properties_K53(B):
+    """configs[3]: 2,097,152 cells, K = 53, property pass only."""
+    from oracle import oracle
+    from paper_2312_05800_b200 import synth
+    mech, _, cells = synth.make_config(4)
+    n, K = cells.n, 53
+    gm = B.Mech(mech)
+    T, p, Y = dev(cells.T), dev(cells.p), dev(cells.Y)
+    out = {k: torch.empty(n, device="cuda") for k in ("cp", "h", "mu", "lam")}
+    D = torch.empty(K, n, device="cuda")
+    B.df_thermo_properties(gm, T, p, Y, D=D, **out)
+    torch.cuda.synchronize()
+    assert bool((D > 0).all()) and bool(torch.isfinite(D).all())
+    idx = sample_idx(n, 2048)
+    ref = oracle.Mech(mech).properties(cells.T[idx], cells.p[idx], np.ascontiguousarray(cells.Y[:, idx]))
+    for k in ("cp", "mu", "lam"):
+        assert helpers.rel_err(out[k].cpu().numpy()[idx], ref[k]).max() <= 1e-5, k
+    eh = np.abs(out["h"].cpu().numpy()[idx] - ref["h"]) / np.maximum(np.abs(ref["h"]), ref["cp"] * cells.T[idx])
+    assert eh.max() <= 1e-5
+    assert helpers.rel_err(D.cpu().numpy()[:, idx], ref["D"][:, :len(idx)]).max() <= 1e-5
+
+
+@pytest.mark.parametrize("guess", ["warm", "cold"])
+def test_cfg5_T_from_h_robustness(B, guess):
+    """configs[4]: 16,777,216 cells, K = 19, T in 250..3500 K, near-pure and 1e-20-trace cells."""
+    from oracle import oracle
+    from paper_2312_05800_b200 import synth
+    mech, _, cells = synth.make_config(5)
+    n = cells.n
+    gm = B.Mech(mech)
+    Y = dev(cells.Y)
+    h = torch.empty(n, device="cuda")
+    B.df_thermo_properties(gm, dev(cells.T), None, Y, h=h)
+    g = cells.T_guess if guess == "warm" else np.full(n, 1000.0, np.float32)
+    T, cp = dev(g), torch.empty(n, device="cuda")
+    cnt = torch.zeros(1, dtype=torch.int32, device="cuda")
+    B.df_thermo_T_from_h(gm, h, Y, T, cp=cp, n_unconverged=cnt)
+    torch.cuda.synchronize()
+    assert int(cnt.item()) == 0
+    # the state was drawn at cells.T: the root must come back to it (fp32 h rounding moves it by < 1e-2 K)
+    assert float((T - dev(cells.T)).abs().max()) <= 2e-2
+    idx = sample_idx(n)
+    om = oracle.Mech(mech)
+    Ys = np.ascontiguousarray(cells.Y[:, idx])
+    T_ref = om.T_from_h(h.cpu().numpy()[idx], Ys, g[idx])
+    assert np.abs(T.cpu().numpy()[idx] - T_ref).max() <= 1e-3
+    cp_ref, _ = om.mixture_cp_h(T.cpu().numpy()[idx], Ys)
+    assert helpers.rel_err(cp.cpu().numpy()[idx], cp_ref).max() <= 1e-5
