@@ -284,7 +284,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             if ((i >= B_SMALL_EMPTY && i < B_SMALL_EMPTY + kSmallBufs) || (i >= B_A1_FULL && i < B_A1_FULL + kA1Slots)) cnt = 4;
             if (i == B_A0_FULL || i == B_ACC_EMPTY || i == B_H3_FULL || i == B_H3_FULL + 1) cnt = 4 * kGroups;
             if (i == B_H2_FULL) cnt = 8 * kGroups;
-            if (i == B_FINAL_DONE) cnt = 4;
+            if (i == B_FINAL_DONE) cnt = 4 * kGroups;
             if (i == B_ACC_FULL || i == B_H2C_EMPTY || i == B_H2C_EMPTY + 1) cnt = 2;  // one commit per issuer
             mbar_init(bar(i), cnt);
         }
@@ -684,44 +684,50 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(B_ACC_EMPTY));
             DBG_REC(12, tcnt * 16 + 11, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
-            // ---- final epilogue (group 0): D4 -> Delta -> inverse Box-Cox -> renormalise -> omega (A9-A11, A17) ----
+            // ---- final epilogue: D4 -> Delta -> inverse Box-Cox -> renormalise -> omega (A9-A11, A17).  All groups take
+            //      part: group g owns the species k = g (mod kGroups) of its rows, the per-row sum of dY* is exchanged
+            //      through shared memory (one named barrier over the epilogue warps) ----
             const uint32_t sb = gs % kSmallBufs;
             const uint32_t spar = (gs / kSmallBufs) & 1;
             ++gs;
-            if (grp == 0) {
+            {
                 mbar_wait(bar(B_SMALL_FULL + sb), spar);
                 tc_fence_after();
                 uint32_t r[32];
                 tc_ld32(t_lane + kSmallCol + sb * 32, r);
                 tc_wait_ld();
                 tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar(B_SMALL_EMPTY + sb));
-                DBG_REC(12, tcnt * 16 + 12, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
-                if (valid) {
-                    // T, p, Y come from the cell buffer the prologue filled; 1/W, b4 and the z-score tables are kernel
-                    // parameters: no global load in this block (with 227 KB of shared memory there is no L1 to hit)
-                    const float T = cellbuf[row], p = cellbuf[kTileM + row];
-                    double sumYm1 = -1.0, sumd = 0.0;
-                    float inv_Wbar = 0.f;
+                float* red = cellbuf + (g.K + 2) * kTileM;   // [kGroups][128] partial sums of dY*
+                const float T = cellbuf[row], p = cellbuf[kTileM + row];
+                float sumY = 0.f, part = 0.f, inv_Wbar = 0.f;
 #pragma unroll
-                    for (int k = 0; k < 32; ++k) {
-                        if (k < g.K) {
-                            const float y = cellbuf[(2 + k) * kTileM + row];
+                for (int k = 0; k < 32; ++k) {
+                    if (k < g.K) {
+                        const float y = cellbuf[(2 + k) * kTileM + row];
+                        sumY += y;
+                        inv_Wbar = fmaf(y, a.invW[k], inv_Wbar);
+                        if (k % kGroups == grp) {
                             const float ok = __uint_as_float(r[k]) + a.b4[k];
                             const float d = ann_dystar_fast(y, fmaf(nm.u_std[k], ok, nm.u_mean[k]), lam, inv_lam);
                             r[k] = __float_as_uint(d);
-                            sumYm1 += (double)y;
-                            sumd += (double)d;
-                            inv_Wbar = fmaf(y, a.invW[k], inv_Wbar);
+                            part += d;
                         }
                     }
-                    // S - 1 in fp64 (it is a difference of O(1) sums); the per-species update in fp32 (2e-2 path)
-                    const float Sm1 = (float)(sumYm1 + sumd), inv_S = 1.0f / (1.0f + Sm1);
-                    const float rho_dt = p / (inv_Wbar * (float)DF_R_UNIVERSAL * T) * nm.inv_dt;
+                }
+                red[grp * kTileM + row] = part;
+                // every epilogue warp has read D4 and written its partial sum
+                asm volatile("bar.sync 1, %0;" ::"n"(kGroups * 128) : "memory");
+                if (grp == 0 && lane == 0) mbar_arrive(bar(B_SMALL_EMPTY + sb));
+                float sumd = 0.f;
+#pragma unroll
+                for (int gg = 0; gg < kGroups; ++gg) sumd += red[gg * kTileM + row];
+                // S - 1 = (sum Y - 1) + sum dY*: both terms are small and well conditioned in fp32 on this 2e-2 path
+                const float Sm1 = (sumY - 1.0f) + sumd, inv_S = 1.0f / (1.0f + Sm1);
+                const float rho_dt = p / (inv_Wbar * (float)DF_R_UNIVERSAL * T) * nm.inv_dt;
+                if (valid) {
 #pragma unroll
                     for (int k = 0; k < 32; ++k) {
-                        if (k < g.K) {
+                        if (k < g.K && k % kGroups == grp) {
                             const float d = (__uint_as_float(r[k]) - cellbuf[(2 + k) * kTileM + row] * Sm1) * inv_S;
                             if (a.dY) a.dY[(size_t)k * a.ld + cell] = d;
                             if (a.omega) a.omega[(size_t)k * a.ld + cell] = rho_dt * d;
@@ -813,7 +819,7 @@ df_status ann_bf16_create(df_ann* ann, const float* const* W, const float* const
     g.off_w4 = g.off_r2 + 2 * kChunkBytes;
     g.off_bar = g.off_w4 + g.w4_bytes;
     g.off_cell = (g.off_bar + B_COUNT * 8 + 16 + 127) / 128 * 128;
-    g.smem_bytes = g.off_cell + (K + 2) * kTileM * (int)sizeof(float) + 1024;
+    g.smem_bytes = g.off_cell + (K + 2 + kGroups) * kTileM * (int)sizeof(float) + 1024;  // cells + partial sums
     if (g.smem_bytes > 227 * 1024) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: layer widths need %d B of shared memory", g.smem_bytes);
 
     int dev = 0;
