@@ -41,8 +41,8 @@ __device__ __forceinline__ void diff_tile(const float* __restrict__ coef, f2 u, 
     for (int a = 0; a < 8; ++a)
 #pragma unroll
         for (int b = DIAG ? a + 1 : 0; b < 8; ++b) {
-            const float4 c0 = __ldg(reinterpret_cast<const float4*>(coef + (a * 8 + b) * 8));
-            const float c4 = __ldg(coef + (a * 8 + b) * 8 + 4);
+            const float4 c0 = *reinterpret_cast<const float4*>(coef + (a * 8 + b) * 8);   // warp-uniform: broadcast LDS
+            const float c4 = coef[(a * 8 + b) * 8 + 4];
             const f2 r = rcp2(poly4_2(c0.x, c0.y, c0.z, c0.w, c4, u));
             Sk[a] = fma2(Xj[b], r, Sk[a]);
             Sj[b] = fma2(Xk[a], r, Sj[b]);
@@ -57,9 +57,16 @@ props_tiled_kernel(MechDev md, long long n, long long ld, const float* __restric
     const int K = md.K, Kp = md.Kp, nt = Kp >> 3, t = threadIdx.x;
     f2* sX = sm2;                 // [Kp][kTT] mole fractions
     f2* sR = sX + Kp * kTT;       // 1/g (Wilke), then the S_k accumulators (diffusion)
-    const long long i = ((long long)blockIdx.x * kTT + t) * 2;
-    if (i >= n) return;
-    const bool two = (i + 1 < n);
+    float* sBT = reinterpret_cast<float*>(sR + Kp * kTT);   // [Kp][Kp] Wilke table (transposed), staged once per block
+    float* sCo = sBT + Kp * Kp;                             // [2][512] double-buffered diffusion coefficient tiles
+    // every thread stays alive (the tile staging below uses block-wide barriers); threads past the end of the field
+    // work on cell 0 and do not store
+    const long long i_raw = ((long long)blockIdx.x * kTT + t) * 2;
+    const bool valid = i_raw < n;
+    const long long i = valid ? i_raw : 0;
+    const bool two = valid && (i + 1 < n);
+    for (int e = t; e < Kp * Kp / 4; e += kTT)
+        reinterpret_cast<float4*>(sBT)[e] = __ldg(reinterpret_cast<const float4*>(md.BT) + e);
     auto ld2 = [&](const float* p) -> f2 {
         if (two) return __ldg(reinterpret_cast<const float2*>(p + i));
         const float v = __ldg(p + i);
@@ -67,7 +74,7 @@ props_tiled_kernel(MechDev md, long long n, long long ld, const float* __restric
     };
     auto st2 = [&](float* p, f2 v) {
         if (two) *reinterpret_cast<float2*>(p + i) = v;
-        else p[i] = v.x;
+        else if (valid) p[i] = v.x;
     };
     const f2 T = ld2(Tg);
     const f2 tau = mul2(add2(T, bc(-md.sc.T_mid)), md.sc.inv_S);
@@ -109,7 +116,8 @@ props_tiled_kernel(MechDev md, long long n, long long ld, const float* __restric
                                      mul2(q[1], 2.f)), tau, q[0]),
                            md.sc.inv_S));
     }
-    if (!mu_o && !lam_o && !D_o) return;
+    if (!mu_o && !lam_o && !D_o) return;   // block-uniform
+    __syncthreads();                       // sBT is staged
 
     // ---- phase 2: X_k, r_k = 1/g_k, conductivity ---------------------------------------------------------------
     const f2 inv_sumx = make_float2(1.0f / sumx.x, 1.0f / sumx.y);
@@ -144,8 +152,8 @@ props_tiled_kernel(MechDev md, long long n, long long ld, const float* __restric
 #pragma unroll 2
             for (int j = 0; j < Kp; ++j) {
                 const f2 xj = sX[j * kTT + t], rj = sR[j * kTT + t];
-                const float4* bt = reinterpret_cast<const float4*>(md.BT + (size_t)j * Kp + k0);
-                const float4 b0 = __ldg(bt), b1 = __ldg(bt + 1);
+                const float4* bt = reinterpret_cast<const float4*>(sBT + j * Kp + k0);
+                const float4 b0 = bt[0], b1 = bt[1];
                 const float B[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
 #pragma unroll
                 for (int a = 0; a < 8; ++a) {
@@ -179,7 +187,14 @@ props_tiled_kernel(MechDev md, long long n, long long ld, const float* __restric
             }
         }
         f2 pre = bc(0.f);
-        const float* coef = md.dtile;
+        // coefficient tiles (2 KB each, in loop order) are staged through shared memory, double-buffered: the whole
+        // block copies tile tix + 1 while it computes tile tix
+        const float4* gco = reinterpret_cast<const float4*>(md.dtile);
+        const int ntiles = nt * (nt + 1) / 2;
+        reinterpret_cast<float4*>(sCo)[t] = __ldg(gco + t);
+        reinterpret_cast<float4*>(sCo)[t + kTT] = __ldg(gco + t + kTT);
+        __syncthreads();
+        int tix = 0;
         for (int kt = 0; kt < nt; ++kt) {
             const int k0 = kt * 8;
             f2 Xk[8], Sk[8];
@@ -188,8 +203,15 @@ props_tiled_kernel(MechDev md, long long n, long long ld, const float* __restric
                 Xk[a] = sX[(k0 + a) * kTT + t];
                 Sk[a] = bc(0.f);
             }
-            for (int jt = kt; jt < nt; ++jt, coef += 512) {
+            for (int jt = kt; jt < nt; ++jt, ++tix) {
                 const int j0 = jt * 8;
+                const float* coef = sCo + (tix & 1) * 512;
+                float4 n0, n1;
+                const bool more = tix + 1 < ntiles;
+                if (more) {
+                    n0 = __ldg(gco + (size_t)(tix + 1) * 128 + t);
+                    n1 = __ldg(gco + (size_t)(tix + 1) * 128 + t + kTT);
+                }
                 f2 Xj[8], Sj[8];
 #pragma unroll
                 for (int b = 0; b < 8; ++b) {
@@ -200,6 +222,12 @@ props_tiled_kernel(MechDev md, long long n, long long ld, const float* __restric
                 else diff_tile<false>(coef, u, Xk, Xj, Sk, Sj);
 #pragma unroll
                 for (int b = 0; b < 8; ++b) sR[(j0 + b) * kTT + t] = add2(sR[(j0 + b) * kTT + t], Sj[b]);
+                if (more) {
+                    float4* dst = reinterpret_cast<float4*>(sCo + ((tix + 1) & 1) * 512);
+                    dst[t] = n0;
+                    dst[t + kTT] = n1;
+                }
+                __syncthreads();
             }
 #pragma unroll
             for (int a = 0; a < 8; ++a) {
@@ -224,7 +252,7 @@ props_tiled_kernel(MechDev md, long long n, long long ld, const float* __restric
 df_status launch_properties_tiled(const df_mech* mech, long long n, long long ld, const float* T, const float* p,
                                   const float* Y, float* cp, float* h, float* mu, float* lam, float* D, cudaStream_t s) {
     const MechDev& md = mech->dev;
-    const size_t smem = (size_t)2 * md.Kp * kTT * sizeof(float2);
+    const size_t smem = (size_t)2 * md.Kp * kTT * sizeof(float2) + ((size_t)md.Kp * md.Kp + 1024) * sizeof(float);
     static bool attr_set = false;
     if (!attr_set) {
         DF_CUDA_TRY(cudaFuncSetAttribute(props_tiled_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
