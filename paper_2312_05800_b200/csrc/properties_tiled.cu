@@ -86,7 +86,8 @@ props_tiled_kernel(MechDev md, long long n, long long ld, const float* __restric
     for (int m = 0; m < 5; ++m) Cl[m] = Ch[m] = bc(0.f);
     double H0l0 = 0.0, H0h0 = 0.0, H0l1 = 0.0, H0h1 = 0.0;
     f2 sumx = bc(0.f);
-    for (int k = 0; k < K; ++k) {
+#pragma unroll 8
+    for (int k = 0; k < K; ++k) {   // unrolled: eight rounds of (L2-latency) loads in flight per thread
         const f2 y = ld2(Yg + (size_t)k * ld);
         const float4* th = reinterpret_cast<const float4*>(md.thp + k * 12);
         const float4 a = __ldg(th), b = __ldg(th + 1), c = __ldg(th + 2);  // lo c0..c5 | hi c0..c5
@@ -125,6 +126,7 @@ props_tiled_kernel(MechDev md, long long n, long long ld, const float* __restric
     const f2 sqrtT = make_float2(sqrtf(T.x), sqrtf(T.y));
     {
         f2 s1 = bc(0.f), s2 = bc(0.f);
+#pragma unroll 8
         for (int k = 0; k < Kp; ++k) {
             const f2 X = mul2(sX[k * kTT + t], inv_sumx);
             sX[k * kTT + t] = X;
@@ -178,6 +180,7 @@ props_tiled_kernel(MechDev md, long long n, long long ld, const float* __restric
             f2 suf = bc(0.f);
             // suffix sums sum_{j > k} Y_j are parked in the output array (read back, then overwritten, below):
             // a third per-thread vector in shared memory would cost a third of the occupancy
+#pragma unroll 8
             for (int k = Kp - 1; k >= 0; --k) {
                 sR[k * kTT + t] = bc(0.f);
                 if (k < K) {
