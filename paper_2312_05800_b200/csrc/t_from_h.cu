@@ -137,11 +137,139 @@ t_from_h_kernel(int K, MechScalars sc, const float* __restrict__ th32, const dou
     if (n_unconv && bad) atomicAdd(n_unconv, bad);
 }
 
+
+// ---- fixed K: two cells per thread, every load issued before the first use ---------------------------------------
+// The generic kernel above alternates a load phase (4 float4 loads in flight per thread) with a long per-cell
+// Newton / fp64 phase and re-reads Y for the fp64 step; it sustains ~2 TB/s.  For the species counts of the configs
+// the whole column of Y (K float2 per thread) fits in registers: all K loads are in flight at once (3x the bytes in
+// flight per SM) and the fp64 step needs no second pass.
+#ifndef DF_TFH_MINBLOCKS
+#define DF_TFH_MINBLOCKS 5
+#endif
+template <int K>
+__global__ void __launch_bounds__(kThreads, DF_TFH_MINBLOCKS)
+t_from_h_fixed_kernel(MechScalars sc, const float* __restrict__ th32, const double* __restrict__ th64, long long n,
+                      long long ld, const float* __restrict__ h, const float* __restrict__ Y, float* __restrict__ T,
+                      float* __restrict__ cp_out, int* __restrict__ n_unconv) {
+    __shared__ __align__(16) double s64[K * 12];
+    __shared__ __align__(16) float s32[K * 12];
+    const long long i0 = ((long long)blockIdx.x * kThreads + threadIdx.x) * 2;
+    const bool any = i0 < n, two = i0 + 1 < n;
+    const long long ic = any ? i0 : 0;
+    // the field loads go out first; the table staging below overlaps with their latency
+    float2 y[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const float* yp = Y + (size_t)k * ld + ic;
+        if (two) y[k] = __ldg(reinterpret_cast<const float2*>(yp));
+        else { const float v = __ldg(yp); y[k] = make_float2(v, v); }
+    }
+    float2 hin, tg;
+    if (two) { hin = __ldg(reinterpret_cast<const float2*>(h + ic)); tg = *reinterpret_cast<const float2*>(T + ic); }
+    else { hin = make_float2(__ldg(h + ic), 0.f); hin.y = hin.x; tg = make_float2(T[ic], T[ic]); }
+    for (int i = threadIdx.x; i < K * 12; i += kThreads) {
+        s64[i] = th64[i];
+        s32[i] = th32[i];
+    }
+    __syncthreads();
+    if (!any) return;
+
+    // mixture polynomial coefficients, both ranges, both cells packed (FFMA2, coefficient broadcast)
+    float2 P[12];
+#pragma unroll
+    for (int m = 0; m < 12; ++m) P[m] = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const float4* cf = reinterpret_cast<const float4*>(s32 + k * 12);
+        const float4 a = cf[0], b = cf[1], d = cf[2];
+        const float co[12] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w, d.x, d.y, d.z, d.w};
+#pragma unroll
+        for (int m = 0; m < 12; ++m) P[m] = __ffma2_rn(y[k], make_float2(co[m], co[m]), P[m]);
+    }
+    float tauv[2], Tout[2], cpv[2];
+    const float hv[2] = {hin.x, hin.y}, tgv[2] = {tg.x, tg.y};
+    int bad = 0;
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+        float C[12];
+#pragma unroll
+        for (int m = 0; m < 12; ++m) C[m] = c ? P[m].y : P[m].x;
+        float tau = (tgv[c] > 0.f && tgv[c] < 3.0e38f) ? (tgv[c] - sc.T_mid) * sc.inv_S : 0.f;  // A4
+        tau = fminf(fmaxf(tau, sc.tau_min), sc.tau_max);
+        for (int it = 0; it < kMaxIter; ++it) {
+            const bool lo = tau < 0.f;
+            const float q0 = lo ? C[0] : C[6], q1 = lo ? C[1] : C[7], q2 = lo ? C[2] : C[8], q3 = lo ? C[3] : C[9],
+                        q4 = lo ? C[4] : C[10], q5 = lo ? C[5] : C[11];
+            const float hh = fmaf(fmaf(fmaf(fmaf(fmaf(q5, tau, q4), tau, q3), tau, q2), tau, q1), tau, q0);
+            const float dh = fmaf(fmaf(fmaf(fmaf(5.f * q5, tau, 4.f * q4), tau, 3.f * q3), tau, 2.f * q2), tau, q1);
+            const float delta = (hv[c] - hh) / dh;
+            tau = fminf(fmaxf(tau + delta, sc.tau_min), sc.tau_max);
+            if (fabsf(delta) < 1e-5f) break;  // 10 mK: above the fp32 noise floor of h; the fp64 step does the rest
+        }
+        tauv[c] = tau;
+    }
+    // one fp64 Newton step on the species-level polynomials (Y still in registers), the two cells interleaved
+    const int r0 = tauv[0] < 0.f ? 0 : 6, r1 = tauv[1] < 0.f ? 0 : 6;
+    const double t0 = (double)tauv[0], t1 = (double)tauv[1];
+    double h0 = 0.0, h1 = 0.0;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const double* q0 = s64 + k * 12 + r0;
+        const double* q1 = s64 + k * 12 + r1;
+        const double p0 = fma(fma(fma(fma(fma(q0[5], t0, q0[4]), t0, q0[3]), t0, q0[2]), t0, q0[1]), t0, q0[0]);
+        const double p1 = fma(fma(fma(fma(fma(q1[5], t1, q1[4]), t1, q1[3]), t1, q1[2]), t1, q1[1]), t1, q1[0]);
+        h0 = fma((double)y[k].x, p0, h0);
+        h1 = fma((double)y[k].y, p1, h1);
+    }
+    const double hv64[2] = {h0, h1};
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+        const float tau = tauv[c];
+        const bool hi = !(tau < 0.f);
+        const float q1 = c ? (hi ? P[7].y : P[1].y) : (hi ? P[7].x : P[1].x), q2 = c ? (hi ? P[8].y : P[2].y) : (hi ? P[8].x : P[2].x),
+                    q3 = c ? (hi ? P[9].y : P[3].y) : (hi ? P[9].x : P[3].x), q4 = c ? (hi ? P[10].y : P[4].y) : (hi ? P[10].x : P[4].x),
+                    q5 = c ? (hi ? P[11].y : P[5].y) : (hi ? P[11].x : P[5].x);
+        const float dh = fmaf(fmaf(fmaf(fmaf(5.f * q5, tau, 4.f * q4), tau, 3.f * q3), tau, 2.f * q2), tau, q1);
+        const double delta = ((double)hv[c] - hv64[c]) / (double)dh;
+        double t2 = (double)tau + delta;
+        t2 = fmin(fmax(t2, (double)sc.tau_min), (double)sc.tau_max);
+        Tout[c] = (float)fma(t2, (double)sc.S, (double)sc.T_mid);
+        const float tf = (float)t2;
+        const bool lo = tf < 0.f;  // cp at the solution: range by the polished tau (A2)
+        const float p1 = c ? (lo ? P[1].y : P[7].y) : (lo ? P[1].x : P[7].x), p2 = c ? (lo ? P[2].y : P[8].y) : (lo ? P[2].x : P[8].x),
+                    p3 = c ? (lo ? P[3].y : P[9].y) : (lo ? P[3].x : P[9].x), p4 = c ? (lo ? P[4].y : P[10].y) : (lo ? P[4].x : P[10].x),
+                    p5 = c ? (lo ? P[5].y : P[11].y) : (lo ? P[5].x : P[11].x);
+        cpv[c] = fmaf(fmaf(fmaf(fmaf(5.f * p5, tf, 4.f * p4), tf, 3.f * p3), tf, 2.f * p2), tf, p1) * sc.inv_S;
+        if ((c == 0 || two) && !(fabs(delta) * (double)sc.S <= 1e-2)) ++bad;
+    }
+    if (two) {
+        *reinterpret_cast<float2*>(T + i0) = make_float2(Tout[0], Tout[1]);
+        if (cp_out) *reinterpret_cast<float2*>(cp_out + i0) = make_float2(cpv[0], cpv[1]);
+    } else {
+        T[i0] = Tout[0];
+        if (cp_out) cp_out[i0] = cpv[0];
+    }
+    if (n_unconv && bad) atomicAdd(n_unconv, bad);
+}
+
+template <int K>
+df_status launch_fixed(const df_mech* mech, long long n, long long ld, const float* h, const float* Y, float* T, float* cp,
+                       int* n_unconv, cudaStream_t s) {
+    const long long blocks = (n + 2 * kThreads - 1) / (2 * kThreads);
+    if (blocks > 0x7fffffffLL) return df_set_error(DF_ERR_UNSUPPORTED, "df_thermo_T_from_h: n_cells too large");
+    t_from_h_fixed_kernel<K><<<(unsigned)blocks, kThreads, 0, s>>>(mech->dev.sc, mech->dev.th32, mech->dev.th64, n, ld, h, Y,
+                                                                   T, cp, n_unconv);
+    DF_CUDA_TRY(cudaGetLastError());
+    return DF_OK;
+}
+
 }  // namespace
 
 df_status launch_T_from_h(const df_mech* mech, long long n, long long ld, const float* h, const float* Y, float* T,
                           float* cp, int* n_unconv, cudaStream_t s) {
     const int K = mech->K;
+    if (K == 19) return launch_fixed<19>(mech, n, ld, h, Y, T, cp, n_unconv, s);
+    if (K == 9) return launch_fixed<9>(mech, n, ld, h, Y, T, cp, n_unconv, s);
     const size_t smem = (size_t)K * 12 * (sizeof(double) + sizeof(float));
     const long long per_block = (long long)kThreads * 4;
     const long long blocks = (n + per_block - 1) / per_block;
