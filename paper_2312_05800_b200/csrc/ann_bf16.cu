@@ -208,14 +208,14 @@ __device__ __forceinline__ uint32_t gelu_h2(uint32_t v) {
 // instead of powf/log1pf/expm1f (~400 instructions).  Its error (<= 2e-4 relative for |lambda Delta| >= 1e-3 Y^lambda)
 // is far inside the 2e-2 budget of this path; the fp32 path (ann_fp32.cu) keeps the accurate form.
 __device__ __forceinline__ float ann_dystar_fast(float y, float delta, float lambda, float inv_lambda) {
-    if (y > 0.f) {
-        const float q = exp2f(lambda * __log2f(y));
-        const float z = lambda * delta * rcp_approx(q);
-        if (!(z > -1.0f)) return -y;
-        return y * (exp2f(__log2f(1.0f + z) * inv_lambda) - 1.0f);
-    }
+    // branch-free: y > 0: Y (2^(log2(1 + z)/lambda) - 1), z = lambda Delta / Y^lambda, Y* = 0 when z <= -1;
+    //              y = 0: max(lambda Delta, 0)^(1/lambda)
+    const float q = exp2f(lambda * __log2f(y));
+    const float z = lambda * delta * rcp_approx(q);
+    const float pos = y * (exp2f(__log2f(1.0f + z) * inv_lambda) - 1.0f);
     const float base = lambda * delta;
-    return base > 0.f ? exp2f(__log2f(base) * inv_lambda) : 0.f;
+    const float zero = base > 0.f ? exp2f(__log2f(base) * inv_lambda) : 0.f;
+    return y > 0.f ? ((z > -1.0f) ? pos : -y) : zero;
 }
 // two fp32 -> packed fp16x2 (first argument in the low half = lower K index)
 __device__ __forceinline__ uint32_t pack_act(float lo, float hi) {
@@ -634,7 +634,6 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                         c0 += kStep;
                     }
                 }
-                DBG_REC(12, tcnt * 16 + 13 + h, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
                 tc_fence_before();
                 __threadfence();
                 fence_proxy_async();
@@ -692,6 +691,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             ++gs;
             {
                 mbar_wait(bar(B_SMALL_FULL + sb), spar);
+                DBG_REC(12, tcnt * 16 + 12, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
                 tc_fence_after();
                 uint32_t r[32];
                 tc_ld32(t_lane + kSmallCol + sb * 32, r);
@@ -706,18 +706,31 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                         const float y = cellbuf[(2 + k) * kTileM + row];
                         sumY += y;
                         inv_Wbar = fmaf(y, a.invW[k], inv_Wbar);
-                        if (k % kGroups == grp) {
-                            const float ok = __uint_as_float(r[k]) + a.b4[k];
-                            const float d = ann_dystar_fast(y, fmaf(nm.u_std[k], ok, nm.u_mean[k]), lam, inv_lam);
-                            r[k] = __float_as_uint(d);
-                            part += d;
-                        }
                     }
                 }
+                // this group's species k = grp + kGroups * kk: branch-free (selects) so that the MUFU chains of the
+                // species interleave; dys[kk] stays in registers for the renormalisation below
+                float dys[(32 + kGroups - 1) / kGroups];
+#pragma unroll
+                for (int kk = 0; kk < (32 + kGroups - 1) / kGroups; ++kk) {
+                    const int k = grp + kGroups * kk;
+                    float o = 0.f;
+#pragma unroll
+                    for (int gg = 0; gg < kGroups; ++gg)
+                        if (kGroups * kk + gg < 32 && gg == grp) o = __uint_as_float(r[kGroups * kk + gg]);
+                    const bool on = k < g.K;
+                    const int kc = on ? k : 0;
+                    const float y = cellbuf[(2 + kc) * kTileM + row];
+                    const float d = ann_dystar_fast(y, fmaf(nm.u_std[kc], o + a.b4[kc], nm.u_mean[kc]), lam, inv_lam);
+                    dys[kk] = on ? d : 0.f;
+                    part += dys[kk];
+                }
                 red[grp * kTileM + row] = part;
+                DBG_REC(12, tcnt * 16 + 13, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
                 // every epilogue warp has read D4 and written its partial sum
                 asm volatile("bar.sync 1, %0;" ::"n"(kGroups * 128) : "memory");
                 if (grp == 0 && lane == 0) mbar_arrive(bar(B_SMALL_EMPTY + sb));
+                DBG_REC(12, tcnt * 16 + 14, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
                 float sumd = 0.f;
 #pragma unroll
                 for (int gg = 0; gg < kGroups; ++gg) sumd += red[gg * kTileM + row];
@@ -726,9 +739,10 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                 const float rho_dt = p / (inv_Wbar * (float)DF_R_UNIVERSAL * T) * nm.inv_dt;
                 if (valid) {
 #pragma unroll
-                    for (int k = 0; k < 32; ++k) {
-                        if (k < g.K && k % kGroups == grp) {
-                            const float d = (__uint_as_float(r[k]) - cellbuf[(2 + k) * kTileM + row] * Sm1) * inv_S;
+                    for (int kk = 0; kk < (32 + kGroups - 1) / kGroups; ++kk) {
+                        const int k = grp + kGroups * kk;
+                        if (k < g.K) {
+                            const float d = (dys[kk] - cellbuf[(2 + k) * kTileM + row] * Sm1) * inv_S;
                             if (a.dY) a.dY[(size_t)k * a.ld + cell] = d;
                             if (a.omega) a.omega[(size_t)k * a.ld + cell] = rho_dt * d;
                         }
