@@ -238,6 +238,12 @@ __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&r)[32]) {
         : "memory");
 }
 
+#ifdef DF_DBG_PROGRESS
+__device__ volatile int* g_prog = nullptr;   // mapped host memory: [role][8] progress counters of block 0
+#define PROG(role, slot, val) do { if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && g_prog) g_prog[(role) * 8 + (slot)] = (val); } while (0)
+#else
+#define PROG(role, slot, val) do { } while (0)
+#endif
 #ifdef DF_DBG_CLK
 __device__ long long g_dbg[16][128];
 #define DBG_REC(row, idx, cond) do { if ((cond) && blockIdx.x == 0 && (idx) < 128) g_dbg[row][idx] = clock64(); } while (0)
@@ -248,7 +254,7 @@ __device__ long long g_dbg[16][128];
 // barrier indices
 enum {
     B_W_FULL = 0, B_W_EMPTY = B_W_FULL + kWStages, B_W1_FULL = B_W_EMPTY + kWStages, B_W1_EMPTY = B_W1_FULL + 2,
-    B_A0_FULL = B_W1_EMPTY + 2, B_SMALL_FULL, B_SMALL_EMPTY = B_SMALL_FULL + kSmallBufs,
+    B_A0_FULL = B_W1_EMPTY + 2, B_SMALL_FULL, B_SMALL_EMPTY = B_SMALL_FULL + kGroups,
     B_A1_FULL = B_SMALL_EMPTY + kSmallBufs, B_A1_EMPTY = B_A1_FULL + kA1Slots, B_ACC_FULL = B_A1_EMPTY + kA1Slots, B_ACC_EMPTY,
     B_H2_FULL, B_H2C_FULL, B_H2C_EMPTY = B_H2C_FULL + 2, B_H3_FULL = B_H2C_EMPTY + 2, B_H3_EMPTY = B_H3_FULL + 2, B_TILE_DONE = B_H3_EMPTY + 2,
     B_W4_FULL, B_ACC_START, B_FINAL_DONE, B_COUNT
@@ -357,14 +363,16 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
         // one elected lane issues (ptxas then keeps descriptors and barrier addresses in uniform registers).
         const uint32_t id32 = umma_idesc(32, g.b_fmt);
         const uint64_t dA0 = umma_desc(s_r2), dW1 = umma_desc(s_r2 + kChunkBytes);
-        uint32_t w1c = 0, gs = 0, tc = 0;
+        uint32_t w1c = 0, gs = 0, ac = 0, tc = 0;
         for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tc) {
             mbar_wait(bar(B_A0_FULL), tc & 1);
             for (int h = 0; h < 2; ++h)
-                for (int c = 0; c < g.NC; ++c, ++gs) {
+                for (int c = 0; c < g.NC; ++c, ++gs, ++ac) {
                     const uint32_t slot = w1c & 1, sb = gs % kSmallBufs;
                     if ((c & 3) == 0) mbar_wait(bar(B_W1_FULL + slot), (w1c >> 1) & 1);
+                    PROG(0, 0, (int)gs);
                     mbar_wait(bar(B_SMALL_EMPTY + sb), ((gs / kSmallBufs) & 1) ^ 1);
+                    PROG(0, 1, (int)gs);
                     DBG_REC(0, gs - 150, lane == 0 && gs >= 150);
                     tc_fence_after();
                     const bool quad_done = (c & 3) == 3 || c == g.NC - 1;
@@ -373,7 +381,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                         const uint32_t dd = tmem + kSmallCol + sb * 32;
                         tc_mma(dd, dA0, b0, id32, 0u);
                         if (g.K0steps > 1) tc_mma(dd, dA0 + 2, b0 + 2, id32, 1u);
-                        tc_commit(bar(B_SMALL_FULL + sb));
+                        tc_commit(bar(B_SMALL_FULL + ac % kGroups));
                         if (quad_done) tc_commit(bar(B_W1_EMPTY + slot));
                     }
                     __syncwarp();
@@ -436,7 +444,9 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                 for (int c = 0; c < g.NC; ++c, ++ac, ++st) {
                     if ((int)(st & 1) != id) continue;
                     const uint32_t slot = ac % kA1Slots;
+                    PROG(1 + id, 0, (int)ac);
                     mbar_wait(bar(B_A1_FULL + slot), (ac / kA1Slots) & 1);
+                    PROG(1 + id, 1, (int)ac);
                     DBG_REC(2, ac - 150, lane == 0 && ac >= 150);
                     issue_stage(dR1 + (((slot >> 1) * kChunkBytes + (slot & 1) * 64) >> 4), g.na2, g.nb2, id2a, id2b, false,
                                 bar(B_A1_EMPTY + slot));
@@ -481,8 +491,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                     __syncwarp();
                 }
                 if (elect_one()) {
-                    tc_commit(bar(B_SMALL_FULL + sb));
-                    tc_commit(bar(B_TILE_DONE));
+                    tc_commit(bar(B_TILE_DONE));   // D4 is complete: the final epilogue may read it, R2 is free
                 }
                 __syncwarp();
             }
@@ -569,7 +578,9 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                 for (int c = 0; c < g.NC; ++c, ++gs, ++ac) {
                     if ((int)(ac % kGroups) != grp) continue;
                     const uint32_t sb = gs % kSmallBufs;
-                    mbar_wait(bar(B_SMALL_FULL + sb), (gs / kSmallBufs) & 1);
+                    if (q == 0) PROG(3 + grp, 0, (int)gs);
+                    mbar_wait(bar(B_SMALL_FULL + grp), (ac / kGroups) & 1);
+                    if (q == 0) PROG(3 + grp, 1, (int)gs);
                     DBG_REC(4, gs - 150, lane == 0 && q == 0 && gs >= 150);
                     tc_fence_after();
                     uint32_t r[32];
@@ -585,7 +596,9 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                         o[i] = gelu_h2(pack_act(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1])));
                     const uint32_t slot = ac % kA1Slots;
                     DBG_REC(6, ac - 150, lane == 0 && q == 0 && ac >= 150);
+                    if (q == 0) PROG(3 + grp, 2, (int)ac);
                     mbar_wait(bar(B_A1_EMPTY + slot), ((ac / kA1Slots) & 1) ^ 1);
+                    if (q == 0) PROG(3 + grp, 3, (int)ac);
                     const uint32_t base = s_r1 + (slot >> 1) * kChunkBytes;
 #pragma unroll
                     for (int c4 = 0; c4 < 4; ++c4)
@@ -597,8 +610,10 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                 }
                 // drain D2 (this half): +b2, GELU, fp16 -> H2 scratch in the chunk images phase B loads
                 DBG_REC(12, tcnt * 16 + 3 + 3 * h, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
+                if (q == 0) PROG(3 + grp, 4, (int)af);
                 mbar_wait(bar(B_ACC_FULL), af & 1);
                 ++af;
+                if (q == 0) PROG(3 + grp, 5, (int)af);
                 DBG_REC(12, tcnt * 16 + 4 + 3 * h, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
                 tc_fence_after();
                 {
@@ -687,10 +702,9 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             //      part: group g owns the species k = g (mod kGroups) of its rows, the per-row sum of dY* is exchanged
             //      through shared memory (one named barrier over the epilogue warps) ----
             const uint32_t sb = gs % kSmallBufs;
-            const uint32_t spar = (gs / kSmallBufs) & 1;
             ++gs;
             {
-                mbar_wait(bar(B_SMALL_FULL + sb), spar);
+                mbar_wait(bar(B_TILE_DONE), tcnt & 1);
                 DBG_REC(12, tcnt * 16 + 12, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
                 tc_fence_after();
                 uint32_t r[32];
@@ -983,5 +997,13 @@ df_status launch_ann_bf16(const df_ann* ann, const df_mech* mech, long long n, l
 #ifdef DF_DBG_CLK
 extern "C" __attribute__((visibility("default"))) int df_debug_read(long long* out) {
     return (int)cudaMemcpyFromSymbol(out, g_dbg, sizeof(g_dbg));
+}
+#endif
+
+#ifdef DF_DBG_PROGRESS
+extern "C" __attribute__((visibility("default"))) int df_debug_set_progress(int* host_mapped) {
+    int* dptr = nullptr;
+    if (cudaHostGetDevicePointer((void**)&dptr, host_mapped, 0) != cudaSuccess) return -1;
+    return (int)cudaMemcpyToSymbol(g_prog, &dptr, sizeof(dptr));
 }
 #endif
