@@ -39,11 +39,9 @@ constexpr int kTileM = 128;
 #define KGROUPS 3
 #endif
 constexpr int kGroups = KGROUPS;                  // epilogue groups of 4 warps (one warp per TMEM lane quarter)
-#ifndef DF_EXTRA_WARPS
-#define DF_EXTRA_WARPS 0
-#endif
 constexpr int kIssuer2Warp = 4 + 4 * kGroups;  // second layer-2/3 MMA issuer (after the epilogue warps)
-constexpr int kThreads = 128 + kGroups * 128 + 32 + 32 * DF_EXTRA_WARPS;
+constexpr int kIoWarp = kIssuer2Warp + 1;      // four cell-I/O warps: next tile's features -> A0, this tile's D4 -> omega
+constexpr int kThreads = 32 * (kIoWarp + 4);
 constexpr int kWStages = 4;
 constexpr int kA1Tiles = 3;                 // [128 x 64] activation tiles of the A1 ring = 2 * kA1Tiles 32-column slots
 constexpr int kA1Slots = 2 * kA1Tiles;
@@ -66,7 +64,7 @@ struct NetGeom {
     int w2_tile_bytes, w3_tile_bytes, w_slot_bytes, w4_bytes;
     int smem_bytes;
     // shared-memory offsets (bytes from the 1024-aligned base)
-    int off_w, off_r1, off_r2, off_w4, off_bar, off_cell;  // off_cell: raw T, p, Y of the tile, [K+2][128] fp32
+    int off_w, off_r1, off_r2, off_w4, off_bar;
 };
 
 struct Bf16Dev {
@@ -257,7 +255,7 @@ enum {
     B_A0_FULL = B_W1_EMPTY + 2, B_SMALL_FULL, B_SMALL_EMPTY = B_SMALL_FULL + kGroups,
     B_A1_FULL = B_SMALL_EMPTY + kSmallBufs, B_A1_EMPTY = B_A1_FULL + kA1Slots, B_ACC_FULL = B_A1_EMPTY + kA1Slots, B_ACC_EMPTY,
     B_H2_FULL, B_H2C_FULL, B_H2C_EMPTY = B_H2C_FULL + 2, B_H3_FULL = B_H2C_EMPTY + 2, B_H3_EMPTY = B_H3_FULL + 2, B_TILE_DONE = B_H3_EMPTY + 2,
-    B_W4_FULL, B_ACC_START, B_FINAL_DONE, B_COUNT
+    B_W4_FULL, B_ACC_START, B_A0_EMPTY, B_COUNT
 };
 
 struct KArgs {
@@ -288,9 +286,9 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
         for (int i = 0; i < B_COUNT; ++i) {
             uint32_t cnt = 1;
             if ((i >= B_SMALL_EMPTY && i < B_SMALL_EMPTY + kSmallBufs) || (i >= B_A1_FULL && i < B_A1_FULL + kA1Slots)) cnt = 4;
-            if (i == B_A0_FULL || i == B_ACC_EMPTY || i == B_H3_FULL || i == B_H3_FULL + 1) cnt = 4 * kGroups;
+            if (i == B_ACC_EMPTY || i == B_H3_FULL || i == B_H3_FULL + 1) cnt = 4 * kGroups;
+            if (i == B_A0_FULL) cnt = 4;
             if (i == B_H2_FULL) cnt = 8 * kGroups;
-            if (i == B_FINAL_DONE) cnt = 4 * kGroups;
             if (i == B_ACC_FULL || i == B_H2C_EMPTY || i == B_H2C_EMPTY + 1) cnt = 2;  // one commit per issuer
             mbar_init(bar(i), cnt);
         }
@@ -337,7 +335,6 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             const int nquads = (g.NC + 3) / 4;
             uint32_t w1c = 0, h2c = 0, tc = 0;
             for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tc) {
-                if (tc > 0) mbar_wait(bar(B_TILE_DONE), (tc - 1) & 1);  // R2 (the H3 tiles) is free again
                 for (int h = 0; h < 2; ++h)
                     for (int qd = 0; qd < nquads; ++qd, ++w1c) {
                         const uint32_t slot = w1c & 1, par = (w1c >> 1) & 1;
@@ -423,10 +420,10 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             __syncwarp();
         };
         // bias stage of an accumulation: whoever owns stage st issues it and announces it; the other waits
-        auto start_acc = [&](int na, int nb, uint32_t ida, uint32_t idb) {
+        auto start_acc = [&](int na, int nb, uint32_t ida, uint32_t idb, uint32_t extra) {
             if ((int)(st & 1) == id) {
                 mbar_wait(bar(B_ACC_EMPTY), (ae & 1) ^ 1);
-                issue_stage(dR2, na, nb, ida, idb, true, 0u);
+                issue_stage(dR2, na, nb, ida, idb, true, extra);
                 if (lane == 0) mbar_arrive(bar(B_ACC_START));
             } else {
                 mbar_wait(bar(B_ACC_START), acc & 1);
@@ -440,7 +437,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             mbar_wait(bar(B_A0_FULL), tc & 1);
             // ---- phase A: layer 2, one half of its outputs at a time, one stage per layer-1 chunk ----
             for (int h = 0; h < 2; ++h) {
-                start_acc(g.na2, g.nb2, id2a, id2b);
+                start_acc(g.na2, g.nb2, id2a, id2b, 0u);
                 for (int c = 0; c < g.NC; ++c, ++ac, ++st) {
                     if ((int)(st & 1) != id) continue;
                     const uint32_t slot = ac % kA1Slots;
@@ -457,7 +454,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             }
             gs += 2 * g.NC;
             // ---- phase B: layer 3 from the H2 chunks, then layer 4 fed by the D3 drain ----
-            start_acc(g.n3a, g.n3b, id3a, id3b);   // A0 is still intact (it is overwritten by the D3 drain)
+            start_acc(g.n3a, g.n3b, id3a, id3b, bar(B_A0_EMPTY));   // last use of A0: the I/O warps may write the next tile's
             for (int ks = 0; ks < g.NKS; ++ks, ++st) {
                 const uint32_t slot = h2cc & 1;
                 const bool last = (ks & 1) == 1 || ks == g.NKS - 1;
@@ -483,7 +480,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                     tc_fence_after();
                     if (elect_one()) {
                         const int ksteps = min(64, g.d3 - jj * 64) / 16;
-                        const uint64_t ha = dR2 + ((slot * kChunkBytes) >> 4), wa = dW4 + ((jj * 4096) >> 4);
+                        const uint64_t ha = dR1 + ((slot * kChunkBytes) >> 4), wa = dW4 + ((jj * 4096) >> 4);
                         for (int kk = 0; kk < ksteps; ++kk)
                             tc_mma(tmem + kSmallCol + sb * 32, ha + 2 * kk, wa + 2 * kk, id32, (jj > 0 || kk > 0) ? 1u : 0u);
                         tc_commit(bar(B_H3_EMPTY + slot));
@@ -506,8 +503,6 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
         const uint32_t t_lane = tmem + ((uint32_t)(q * 32) << 16);
         uint8_t* scratch = a.scratch + (size_t)blockIdx.x * g.NKC * kChunkBytes;
         uint32_t gs = 0, ac = 0, af = 0, h3c = 0;
-        const float lam = nm.lambda, inv_lam = nm.inv_lambda;
-        float* cellbuf = reinterpret_cast<float*>(sgen + g.off_cell);  // [K+2][128]: T, p, Y_k of this tile's cells
 
         auto st_shared16 = [&](uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
             asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
@@ -520,59 +515,10 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
 
         uint32_t tcnt = 0;
         for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tcnt) {
-            const long long cell = tile * kTileM + row;
-            const bool valid = cell < a.n;
-            // A0 shares its shared memory with the first H3 slot: the previous tile's layer-4 MMAs must be done
             DBG_REC(12, tcnt * 16 + 0, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
-            if (tcnt > 0) {
-                mbar_wait(bar(B_TILE_DONE), (tcnt - 1) & 1);
-                mbar_wait(bar(B_FINAL_DONE), (tcnt - 1) & 1);  // the previous final epilogue has read the cell buffer
-            }
+            // the H3 ring lives in R1: the previous tile's layer-4 MMAs must be done before A1 chunks go there again
+            if (tcnt > 0) mbar_wait(bar(B_TILE_DONE), (tcnt - 1) & 1);
             DBG_REC(12, tcnt * 16 + 1, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
-            // ---- prologue: features + two bias columns of ones -> fp16 A0 [128 x 32]; group grp writes
-            //      feature columns [8 grp, 8 grp + 8) ----
-            for (int fc = grp; fc < 4; fc += kGroups) {
-                // issue the 8 loads of this feature chunk first (clamped addresses), then do the arithmetic
-                float raw[8];
-                const long long cl = valid ? cell : 0;
-#pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const int f = fc * 8 + j;
-                    raw[j] = (f == 0) ? __ldg(a.T + cl) : (f == 1) ? __ldg(a.p + cl)
-                           : (f < g.K + 2) ? __ldg(a.Y + (size_t)(f - 2) * a.ld + cl) : 0.f;
-                }
-#pragma unroll
-                for (int j = 0; j < 8; ++j)
-                    if (fc * 8 + j < g.K + 2) cellbuf[(fc * 8 + j) * kTileM + row] = raw[j];
-                uint32_t o[4];
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    float v[2];
-#pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        const int f = fc * 8 + 2 * i + e;
-                        float x = 0.f;
-                        if (f < g.K + 2) {
-                            if (valid) {
-                                if (f < 2) x = (raw[2 * i + e] - nm.x_mean[f]) * nm.x_inv_std[f];
-                                else {
-                                    const float qy = exp2f(lam * __log2f(raw[2 * i + e]));  // y^lambda, 0 -> 0
-                                    x = ((qy - 1.0f) * inv_lam - nm.x_mean[f]) * nm.x_inv_std[f];
-                                }
-                            }
-                        } else if (f < g.K + 4) {
-                            x = 1.0f;  // multiplies the hi / lo parts of b1 (and b2, b3) stored as weight columns K+2, K+3
-                        }
-                        v[e] = x;
-                    }
-                    o[i] = pack_act(v[0], v[1]);
-                }
-                st_shared16(s_r2 + swz(row, fc), o[0], o[1], o[2], o[3]);
-            }
-            fence_proxy_async_smem();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar(B_A0_FULL));
-            DBG_REC(12, tcnt * 16 + 2, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
             // ---- phase A ----
             for (int h = 0; h < 2; ++h) {
                 for (int c = 0; c < g.NC; ++c, ++gs, ++ac) {
@@ -649,6 +595,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                         c0 += kStep;
                     }
                 }
+                DBG_REC(12, tcnt * 16 + 15, lane == 0 && q == 0 && grp == 0 && tcnt < 8 && h == 1);
                 tc_fence_before();
                 __threadfence();
                 fence_proxy_async();
@@ -682,7 +629,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                 }
                 const uint32_t slot = h3c & 1;
                 mbar_wait(bar(B_H3_EMPTY + slot), ((h3c >> 1) & 1) ^ 1);
-                const uint32_t base = s_r2 + slot * kChunkBytes;
+                const uint32_t base = s_r1 + slot * kChunkBytes;   // R1 is idle once layer 3 has completed
 #pragma unroll
                 for (int i = 0; i < 2; ++i)
                     if (have[i]) {
@@ -698,72 +645,118 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(B_ACC_EMPTY));
             DBG_REC(12, tcnt * 16 + 11, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
-            // ---- final epilogue: D4 -> Delta -> inverse Box-Cox -> renormalise -> omega (A9-A11, A17).  All groups take
-            //      part: group g owns the species k = g (mod kGroups) of its rows, the per-row sum of dY* is exchanged
-            //      through shared memory (one named barrier over the epilogue warps) ----
+            ++gs;   // the D4 accumulation of this tile takes the next buffer of the small ring (read by the I/O warps)
+        }
+    } else if (warp >= kIoWarp && warp < kIoWarp + 4) {
+        // ================= cell-I/O warps: one thread per row of the tile =================
+        // They run one tile ahead on the input side (T, p, Y -> Box-Cox features -> A0) and one tile behind on the
+        // output side (D4 -> Delta -> inverse Box-Cox -> renormalise -> omega, A9-A11, A17), so that neither the
+        // global-memory latency of the cell data nor the MUFU chains of the final epilogue sit between two tiles' MMAs.
+        const int q = warp & 3, row = q * 32 + lane;
+        const uint32_t t_lane = tmem + ((uint32_t)(q * 32) << 16);
+        const float lam = nm.lambda, inv_lam = nm.inv_lambda;
+
+        // features of one cell + two bias columns of ones -> 16 packed fp16x2 words (one A0 row)
+        auto features = [&](long long tile, uint32_t (&o)[16]) {
+            const long long cell = tile * kTileM + row;
+            const bool valid = cell < a.n;
+            const long long cl = valid ? cell : 0;
+            float raw[32];
+#pragma unroll
+            for (int f = 0; f < 32; ++f)
+                raw[f] = (f == 0) ? __ldg(a.T + cl) : (f == 1) ? __ldg(a.p + cl)
+                       : (f < g.K + 2) ? __ldg(a.Y + (size_t)(f - 2) * a.ld + cl) : 0.f;
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                float v[2];
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int f = 2 * i + e;
+                    float x = 0.f;
+                    if (f < g.K + 2) {
+                        if (valid) {
+                            if (f < 2) x = (raw[f] - nm.x_mean[f]) * nm.x_inv_std[f];
+                            else {
+                                const float qy = exp2f(lam * __log2f(raw[f]));  // y^lambda, 0 -> 0
+                                x = ((qy - 1.0f) * inv_lam - nm.x_mean[f]) * nm.x_inv_std[f];
+                            }
+                        }
+                    } else if (f < g.K + 4) {
+                        x = 1.0f;  // multiplies the hi / lo parts of b1 (and b2, b3) stored as weight columns K+2, K+3
+                    }
+                    v[e] = x;
+                }
+                o[i] = pack_act(v[0], v[1]);
+            }
+        };
+        auto write_a0 = [&](const uint32_t (&o)[16]) {
+#pragma unroll
+            for (int fc = 0; fc < 4; ++fc)
+                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(s_r2 + swz(row, fc)), "r"(o[4 * fc]),
+                             "r"(o[4 * fc + 1]), "r"(o[4 * fc + 2]), "r"(o[4 * fc + 3])
+                             : "memory");
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_A0_FULL));
+        };
+
+        uint32_t tcnt = 0, gs = 0;
+        {
+            uint32_t o[16];
+            if ((long long)blockIdx.x < num_tiles) {
+                features(blockIdx.x, o);
+                write_a0(o);
+            }
+        }
+        for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tcnt) {
+            const long long next = tile + gridDim.x;
+            if (next < num_tiles) {
+                uint32_t o[16];
+                features(next, o);
+                mbar_wait(bar(B_A0_EMPTY), tcnt & 1);   // layer 3's bias stage was the last reader of this tile's A0
+                write_a0(o);
+            }
+            gs += 2 * g.NC;
             const uint32_t sb = gs % kSmallBufs;
             ++gs;
-            {
-                mbar_wait(bar(B_TILE_DONE), tcnt & 1);
-                DBG_REC(12, tcnt * 16 + 12, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
-                tc_fence_after();
-                uint32_t r[32];
-                tc_ld32(t_lane + kSmallCol + sb * 32, r);
-                tc_wait_ld();
-                tc_fence_before();
-                float* red = cellbuf + (g.K + 2) * kTileM;   // [kGroups][128] partial sums of dY*
-                const float T = cellbuf[row], p = cellbuf[kTileM + row];
-                float sumY = 0.f, part = 0.f, inv_Wbar = 0.f;
+            const long long cell = tile * kTileM + row;
+            const bool valid = cell < a.n;
+            const long long cl = valid ? cell : 0;
+            const float T = __ldg(a.T + cl), p = __ldg(a.p + cl);
+            mbar_wait(bar(B_TILE_DONE), tcnt & 1);
+            tc_fence_after();
+            uint32_t r[32];
+            tc_ld32(t_lane + kSmallCol + sb * 32, r);
+            tc_wait_ld();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_SMALL_EMPTY + sb));
+            // first pass: dY*_k (kept in r[k]), sum Y, sum dY*, 1 / Wbar; branch-free so the MUFU chains interleave
+            float sumY = 0.f, sumd = 0.f, inv_Wbar = 0.f;
+#pragma unroll
+            for (int k = 0; k < 32; ++k) {
+                const bool on = k < g.K;
+                const int kc = on ? k : 0;
+                const float y = on ? __ldg(a.Y + (size_t)kc * a.ld + cl) : 0.f;
+                sumY += y;
+                inv_Wbar = fmaf(y, a.invW[kc], inv_Wbar);
+                const float d = ann_dystar_fast(y, fmaf(nm.u_std[kc], __uint_as_float(r[k]) + a.b4[kc], nm.u_mean[kc]), lam, inv_lam);
+                r[k] = __float_as_uint(on ? d : 0.f);
+                sumd += __uint_as_float(r[k]);
+            }
+            // S - 1 = (sum Y - 1) + sum dY*: both terms are small and well conditioned in fp32 on this 2e-2 path
+            const float Sm1 = (sumY - 1.0f) + sumd, inv_S = 1.0f / (1.0f + Sm1);
+            const float rho_dt = p / (inv_Wbar * (float)DF_R_UNIVERSAL * T) * nm.inv_dt;
+            if (valid) {
 #pragma unroll
                 for (int k = 0; k < 32; ++k) {
                     if (k < g.K) {
-                        const float y = cellbuf[(2 + k) * kTileM + row];
-                        sumY += y;
-                        inv_Wbar = fmaf(y, a.invW[k], inv_Wbar);
+                        const float y = __ldg(a.Y + (size_t)k * a.ld + cell);   // L2 hit; off the critical path here
+                        const float d = (__uint_as_float(r[k]) - y * Sm1) * inv_S;
+                        if (a.dY) a.dY[(size_t)k * a.ld + cell] = d;
+                        if (a.omega) a.omega[(size_t)k * a.ld + cell] = rho_dt * d;
                     }
                 }
-                // this group's species k = grp + kGroups * kk: branch-free (selects) so that the MUFU chains of the
-                // species interleave; dys[kk] stays in registers for the renormalisation below
-                float dys[(32 + kGroups - 1) / kGroups];
-#pragma unroll
-                for (int kk = 0; kk < (32 + kGroups - 1) / kGroups; ++kk) {
-                    const int k = grp + kGroups * kk;
-                    float o = 0.f;
-#pragma unroll
-                    for (int gg = 0; gg < kGroups; ++gg)
-                        if (kGroups * kk + gg < 32 && gg == grp) o = __uint_as_float(r[kGroups * kk + gg]);
-                    const bool on = k < g.K;
-                    const int kc = on ? k : 0;
-                    const float y = cellbuf[(2 + kc) * kTileM + row];
-                    const float d = ann_dystar_fast(y, fmaf(nm.u_std[kc], o + a.b4[kc], nm.u_mean[kc]), lam, inv_lam);
-                    dys[kk] = on ? d : 0.f;
-                    part += dys[kk];
-                }
-                red[grp * kTileM + row] = part;
-                DBG_REC(12, tcnt * 16 + 13, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
-                // every epilogue warp has read D4 and written its partial sum
-                asm volatile("bar.sync 1, %0;" ::"n"(kGroups * 128) : "memory");
-                if (grp == 0 && lane == 0) mbar_arrive(bar(B_SMALL_EMPTY + sb));
-                DBG_REC(12, tcnt * 16 + 14, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
-                float sumd = 0.f;
-#pragma unroll
-                for (int gg = 0; gg < kGroups; ++gg) sumd += red[gg * kTileM + row];
-                // S - 1 = (sum Y - 1) + sum dY*: both terms are small and well conditioned in fp32 on this 2e-2 path
-                const float Sm1 = (sumY - 1.0f) + sumd, inv_S = 1.0f / (1.0f + Sm1);
-                const float rho_dt = p / (inv_Wbar * (float)DF_R_UNIVERSAL * T) * nm.inv_dt;
-                if (valid) {
-#pragma unroll
-                    for (int kk = 0; kk < (32 + kGroups - 1) / kGroups; ++kk) {
-                        const int k = grp + kGroups * kk;
-                        if (k < g.K) {
-                            const float d = (dys[kk] - cellbuf[(2 + k) * kTileM + row] * Sm1) * inv_S;
-                            if (a.dY) a.dY[(size_t)k * a.ld + cell] = d;
-                            if (a.omega) a.omega[(size_t)k * a.ld + cell] = rho_dt * d;
-                        }
-                    }
-                }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar(B_FINAL_DONE));
             }
         }
     }
@@ -846,8 +839,7 @@ df_status ann_bf16_create(df_ann* ann, const float* const* W, const float* const
     g.off_r2 = g.off_r1 + kA1Tiles * kChunkBytes;
     g.off_w4 = g.off_r2 + 2 * kChunkBytes;
     g.off_bar = g.off_w4 + g.w4_bytes;
-    g.off_cell = (g.off_bar + B_COUNT * 8 + 16 + 127) / 128 * 128;
-    g.smem_bytes = g.off_cell + (K + 2 + kGroups) * kTileM * (int)sizeof(float) + 1024;  // cells + partial sums
+    g.smem_bytes = g.off_bar + B_COUNT * 8 + 16 + 1024;
     if (g.smem_bytes > 227 * 1024) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: layer widths need %d B of shared memory", g.smem_bytes);
 
     int dev = 0;
