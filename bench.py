@@ -44,20 +44,29 @@ def peaks():
 
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled during the timed region (profiling recipe)."""
-    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    NAMES = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+    # asked for as well when this driver's nvidia-smi knows them (probed once): they explain a clock below max
+    EXTRA = ("hw_power_brake_slowdown", "sync_boost", "applications_clocks_setting")
 
     def __init__(self, index: int):
         self.rows, self.proc, self.index = [], None, index
+        self.names = self.NAMES
+
+    def _query(self, names):
+        return "clocks.sm,clocks.max.sm," + ",".join("clocks_event_reasons." + n for n in names)
 
     def __enter__(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "50"],
+            probe = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self._query(self.NAMES + self.EXTRA)}",
+                                    "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=20)
+            if probe.returncode == 0 and probe.stdout.count(",") >= 1 + len(self.NAMES + self.EXTRA):
+                self.names = self.NAMES + self.EXTRA
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self._query(self.names)}",
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thr = threading.Thread(target=self._read, daemon=True)
             self.thr.start()
-        except OSError:
+        except (OSError, subprocess.SubprocessError):
             self.proc = None
         return self
 
@@ -77,7 +86,6 @@ class ClockSampler:
     def summary(self, t0=0.0, t1=float("inf")):
         """Median SM clock and active throttle reasons over the samples read in [t0, t1] (perf_counter)."""
         sm, mx, reasons = [], 0.0, set()
-        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
         for ts, r in self.rows:
             if not (t0 <= ts <= t1 + 0.15):
                 continue
@@ -86,7 +94,7 @@ class ClockSampler:
                 mx = max(mx, float(r[1]))
             except (ValueError, IndexError):
                 continue
-            for nm, v in zip(names, r[2:6]):
+            for nm, v in zip(self.names, r[2:2 + len(self.names)]):
                 if v.lower().startswith("active"):
                     reasons.add(nm)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons),
@@ -268,9 +276,11 @@ def run_gpu(args):
     clocks = clk.summary(w0, w1)
     # B200_PROFILING.md: burst peak for a kernel timed alone, sustained peak for one timed inside a long step; the
     # step loop counts as "long" when the power cap was seen active during the timed region
-    capped = "sw_power_cap" in clocks["reasons"]
+    low = bool(clocks["sm_mhz"] and clocks["sm_max_mhz"] and clocks["sm_mhz"] < 0.95 * clocks["sm_max_mhz"])
+    capped = bool({"sw_power_cap", "hw_power_brake_slowdown"} & set(clocks["reasons"])) or low
     peak = pk["bf16_sust"] if capped else pk["bf16"]
-    peak_src = f"{pk['src']} bf16 {'sustained (sw_power_cap active in the timed region)' if capped else 'burst'}"
+    why = "power-limited clocks in the timed region: " + (", ".join(clocks["reasons"]) or "SM clock below 95 % of max")
+    peak_src = f"{pk['src']} bf16 {'sustained (' + why + ')' if capped else 'burst'}"
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
@@ -300,7 +310,7 @@ def run_gpu(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--cells", type=int, default=2097152, help="cells per GPU (default: configs[2])")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
