@@ -615,20 +615,20 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             for (int jj = 0; jj < g.NJ; ++jj, ++h3c) {
                 // the four 16-column units of this 64-wide chunk go round-robin over the groups, continuing from the
                 // previous chunk (unit jj * 4 + u -> group (jj * 4 + u) % kGroups): one or two per group, balanced
-                // over the drain; both TMEM loads are in flight before the first GELU
                 const int u0 = (grp + kGroups * 4 - (jj * 4) % kGroups) % kGroups;
-                uint32_t o[2][8], r[2][16];
+                uint32_t o[2][8];
                 bool have[2];
 #pragma unroll
                 for (int i = 0; i < 2; ++i) {
                     const int u = u0 + i * kGroups, c0 = jj * 64 + u * 16;
                     have[i] = u < 4 && c0 < g.d3;
-                    if (have[i]) tc_ld16(t_lane + c0, r[i]);
+                    if (have[i]) {
+                        uint32_t r[16];
+                        tc_ld16(t_lane + c0, r);
+                        tc_wait_ld();
+                        gelu16(r, o[i]);
+                    }
                 }
-                tc_wait_ld();
-#pragma unroll
-                for (int i = 0; i < 2; ++i)
-                    if (have[i]) gelu16(r[i], o[i]);
                 const uint32_t slot = h3c & 1;
                 mbar_wait(bar(B_H3_EMPTY + slot), ((h3c >> 1) & 1) ^ 1);
                 const uint32_t base = s_r1 + slot * kChunkBytes;   // R1 is idle once layer 3 has completed
