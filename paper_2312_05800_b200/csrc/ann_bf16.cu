@@ -116,7 +116,7 @@ __device__ __forceinline__ void tma_bulk_g2s(uint32_t dst, const void* src, uint
                  "l"(src), "r"(bytes), "r"(bar)
                  : "memory");
 }
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }  // all state spaces (global scratch)
+__device__ __forceinline__ void fence_proxy_async_global() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -597,8 +597,10 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                 }
                 DBG_REC(12, tcnt * 16 + 15, lane == 0 && q == 0 && grp == 0 && tcnt < 8 && h == 1);
                 tc_fence_before();
-                __threadfence();
-                fence_proxy_async();
+                // generic-proxy stores to the scratch -> async-proxy (TMA) reads by warp 3 of this CTA: the proxy fence for
+                // the global space, then the release/acquire pair of the mbarrier.  (A preceding __threadfence and the
+                // all-spaces form of the fence add a MEMBAR.SC.GPU + ERRBAR: 2 % of the kernel.)
+                fence_proxy_async_global();
                 __syncwarp();
                 if (lane == 0) {
                     mbar_arrive(bar(B_ACC_EMPTY));
