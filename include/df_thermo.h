@@ -133,8 +133,11 @@ DF_API df_status df_chem_ann_source(const df_ann* ann, const df_mech* mech, long
 /* ---- host-buffer step (bench.py's e2e leg) ----------------------------------------------
  * One pass of the whole path over HOST arrays: copies h, p, T_guess, Y host->device, runs
  * T_from_h -> properties -> ann_source (ann may be NULL: skipped) on the context's stream,
- * copies the requested outputs device->host and synchronises.  Host arrays should be pinned
- * for the copies to be asynchronous; pitch of Y, D and omega is ld on both sides.
+ * copies the requested outputs device->host and synchronises.  The cells are processed in up
+ * to 8 slices on three streams (copy-in, kernels, copy-out), so that with pinned host arrays
+ * the PCIe transfers in both directions overlap the kernels; with pageable arrays the copies
+ * are staged by the driver and the call is still correct.  Pitch of Y, D and omega is ld on
+ * both sides.
  * The context owns device staging for up to max_cells cells. */
 DF_API df_status df_host_ctx_create(df_host_ctx** out, const df_mech* mech, const df_ann* ann, long long max_cells);
 DF_API df_status df_host_ctx_destroy(df_host_ctx* ctx);

@@ -163,11 +163,18 @@ extern "C" df_status df_chem_ann_source(const df_ann* ann, const df_mech* mech, 
 }
 
 // ---- host-buffer step ----------------------------------------------------------------------------
+// df_step_host pipelines the step over up to kHostChunks slices of the cells: copy-in of slice c+1 and copy-out of
+// slice c-1 overlap the kernels of slice c (PCIe is full duplex, cells are independent).
+constexpr int kHostChunks = 8;
+constexpr long long kHostChunkMin = 65536;   // cells; below this a slice no longer fills the GPU
+
 struct df_host_ctx {
     const df_mech* mech;
     const df_ann* ann;
     long long cap;  // cells (pitch of the staging arrays)
-    cudaStream_t stream;
+    cudaStream_t stream;             // compute
+    cudaStream_t s_in, s_out;        // host->device and device->host copies (one copy engine each)
+    cudaEvent_t ev_in[kHostChunks], ev_done[kHostChunks], ev_prev;
     float *h, *p, *T, *Y, *cp, *mu, *lam, *D, *omega;
     void* ws;
     size_t ws_bytes;
@@ -185,7 +192,13 @@ extern "C" df_status df_host_ctx_create(df_host_ctx** out, const df_mech* mech, 
     c->cap = (max_cells + 255) / 256 * 256;
     const size_t f = (size_t)c->cap * sizeof(float), K = (size_t)mech->K;
     c->ws_bytes = ann ? df_ann_workspace_bytes(ann, max_cells) : 0;
-    bool ok = cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking) == cudaSuccess;
+    bool ok = cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaEventCreateWithFlags(&c->ev_prev, cudaEventDisableTiming) == cudaSuccess;
+    for (int i = 0; ok && i < kHostChunks; ++i)
+        ok = cudaEventCreateWithFlags(&c->ev_in[i], cudaEventDisableTiming) == cudaSuccess &&
+             cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming) == cudaSuccess;
     ok = ok && cudaMalloc((void**)&c->h, f) == cudaSuccess && cudaMalloc((void**)&c->p, f) == cudaSuccess &&
          cudaMalloc((void**)&c->T, f) == cudaSuccess && cudaMalloc((void**)&c->Y, f * K) == cudaSuccess &&
          cudaMalloc((void**)&c->cp, f) == cudaSuccess && cudaMalloc((void**)&c->mu, f) == cudaSuccess &&
@@ -205,7 +218,14 @@ extern "C" df_status df_host_ctx_destroy(df_host_ctx* c) {
     if (!c) return DF_OK;
     cudaFree(c->h); cudaFree(c->p); cudaFree(c->T); cudaFree(c->Y); cudaFree(c->cp); cudaFree(c->mu);
     cudaFree(c->lam); cudaFree(c->D); cudaFree(c->omega); cudaFree(c->ws);
+    for (int i = 0; i < kHostChunks; ++i) {
+        if (c->ev_in[i]) cudaEventDestroy(c->ev_in[i]);
+        if (c->ev_done[i]) cudaEventDestroy(c->ev_done[i]);
+    }
+    if (c->ev_prev) cudaEventDestroy(c->ev_prev);
     if (c->stream) cudaStreamDestroy(c->stream);
+    if (c->s_in) cudaStreamDestroy(c->s_in);
+    if (c->s_out) cudaStreamDestroy(c->s_out);
     delete c;
     return DF_OK;
 }
@@ -218,33 +238,48 @@ extern "C" df_status df_step_host(df_host_ctx* c, long long n, long long ld, con
     if (n == 0) return DF_OK;
     if (!h || !p || !T_guess || !Y) return df_set_error(DF_ERR_INVALID_ARG, "df_step_host: NULL input");
     if (omega && !c->ann) return df_set_error(DF_ERR_INVALID_ARG, "df_step_host: omega requested but ctx has no ann");
-    const size_t f = (size_t)n * sizeof(float);
     const int K = c->mech->K;
-    cudaStream_t s = c->stream;
-    DF_CUDA_TRY(cudaMemcpyAsync(c->h, h, f, cudaMemcpyHostToDevice, s));
-    DF_CUDA_TRY(cudaMemcpyAsync(c->p, p, f, cudaMemcpyHostToDevice, s));
-    DF_CUDA_TRY(cudaMemcpyAsync(c->T, T_guess, f, cudaMemcpyHostToDevice, s));
-    DF_CUDA_TRY(cudaMemcpy2DAsync(c->Y, (size_t)c->cap * sizeof(float), Y, (size_t)ld * sizeof(float), f, K,
-                                  cudaMemcpyHostToDevice, s));
-    df_status st = df_thermo_T_from_h(c->mech, n, c->cap, c->h, c->Y, c->T, nullptr, nullptr, s);
-    if (st != DF_OK) return st;
-    st = df_thermo_properties(c->mech, n, c->cap, c->T, c->p, c->Y, cp ? c->cp : nullptr, nullptr, mu ? c->mu : nullptr,
-                              lambda ? c->lam : nullptr, D ? c->D : nullptr, s);
-    if (st != DF_OK) return st;
-    if (omega) {
-        st = df_chem_ann_source(c->ann, c->mech, n, c->cap, c->T, c->p, c->Y, c->omega, nullptr, c->ws, c->ws_bytes, s);
+    const size_t dpitch = (size_t)c->cap * sizeof(float), hpitch = (size_t)ld * sizeof(float);
+    // slices of m cells (a multiple of 1024: tile and vector-load alignment of every kernel)
+    long long m = (n + kHostChunks - 1) / kHostChunks;
+    if (m < kHostChunkMin) m = kHostChunkMin;
+    m = (m + 1023) / 1024 * 1024;
+    const int nch = (int)((n + m - 1) / m);
+    // the staging buffers are reused: this call's copies-in must not overtake the previous call's kernels/copies-out
+    // (df_step_host synchronises before it returns, so this only matters after an error return)
+    DF_CUDA_TRY(cudaEventRecord(c->ev_prev, c->s_out));
+    DF_CUDA_TRY(cudaStreamWaitEvent(c->s_in, c->ev_prev, 0));
+    for (int ch = 0; ch < nch; ++ch) {
+        const long long o = (long long)ch * m, nc = (n - o < m) ? n - o : m;
+        const size_t f = (size_t)nc * sizeof(float);
+        DF_CUDA_TRY(cudaMemcpyAsync(c->h + o, h + o, f, cudaMemcpyHostToDevice, c->s_in));
+        DF_CUDA_TRY(cudaMemcpyAsync(c->p + o, p + o, f, cudaMemcpyHostToDevice, c->s_in));
+        DF_CUDA_TRY(cudaMemcpyAsync(c->T + o, T_guess + o, f, cudaMemcpyHostToDevice, c->s_in));
+        DF_CUDA_TRY(cudaMemcpy2DAsync(c->Y + o, dpitch, Y + o, hpitch, f, K, cudaMemcpyHostToDevice, c->s_in));
+        DF_CUDA_TRY(cudaEventRecord(c->ev_in[ch], c->s_in));
+
+        DF_CUDA_TRY(cudaStreamWaitEvent(c->stream, c->ev_in[ch], 0));
+        df_status st = df_thermo_T_from_h(c->mech, nc, c->cap, c->h + o, c->Y + o, c->T + o, nullptr, nullptr, c->stream);
         if (st != DF_OK) return st;
+        st = df_thermo_properties(c->mech, nc, c->cap, c->T + o, c->p + o, c->Y + o, cp ? c->cp + o : nullptr, nullptr,
+                                  mu ? c->mu + o : nullptr, lambda ? c->lam + o : nullptr, D ? c->D + o : nullptr, c->stream);
+        if (st != DF_OK) return st;
+        if (omega) {
+            st = df_chem_ann_source(c->ann, c->mech, nc, c->cap, c->T + o, c->p + o, c->Y + o, c->omega + o, nullptr, c->ws,
+                                    c->ws_bytes, c->stream);
+            if (st != DF_OK) return st;
+        }
+        DF_CUDA_TRY(cudaEventRecord(c->ev_done[ch], c->stream));
+
+        DF_CUDA_TRY(cudaStreamWaitEvent(c->s_out, c->ev_done[ch], 0));
+        if (T) DF_CUDA_TRY(cudaMemcpyAsync(T + o, c->T + o, f, cudaMemcpyDeviceToHost, c->s_out));
+        if (cp) DF_CUDA_TRY(cudaMemcpyAsync(cp + o, c->cp + o, f, cudaMemcpyDeviceToHost, c->s_out));
+        if (mu) DF_CUDA_TRY(cudaMemcpyAsync(mu + o, c->mu + o, f, cudaMemcpyDeviceToHost, c->s_out));
+        if (lambda) DF_CUDA_TRY(cudaMemcpyAsync(lambda + o, c->lam + o, f, cudaMemcpyDeviceToHost, c->s_out));
+        if (D) DF_CUDA_TRY(cudaMemcpy2DAsync(D + o, hpitch, c->D + o, dpitch, f, K, cudaMemcpyDeviceToHost, c->s_out));
+        if (omega) DF_CUDA_TRY(cudaMemcpy2DAsync(omega + o, hpitch, c->omega + o, dpitch, f, K, cudaMemcpyDeviceToHost, c->s_out));
     }
-    if (T) DF_CUDA_TRY(cudaMemcpyAsync(T, c->T, f, cudaMemcpyDeviceToHost, s));
-    if (cp) DF_CUDA_TRY(cudaMemcpyAsync(cp, c->cp, f, cudaMemcpyDeviceToHost, s));
-    if (mu) DF_CUDA_TRY(cudaMemcpyAsync(mu, c->mu, f, cudaMemcpyDeviceToHost, s));
-    if (lambda) DF_CUDA_TRY(cudaMemcpyAsync(lambda, c->lam, f, cudaMemcpyDeviceToHost, s));
-    if (D)
-        DF_CUDA_TRY(cudaMemcpy2DAsync(D, (size_t)ld * sizeof(float), c->D, (size_t)c->cap * sizeof(float), f, K,
-                                      cudaMemcpyDeviceToHost, s));
-    if (omega)
-        DF_CUDA_TRY(cudaMemcpy2DAsync(omega, (size_t)ld * sizeof(float), c->omega, (size_t)c->cap * sizeof(float), f, K,
-                                      cudaMemcpyDeviceToHost, s));
-    DF_CUDA_TRY(cudaStreamSynchronize(s));
+    DF_CUDA_TRY(cudaStreamSynchronize(c->s_out));
+    DF_CUDA_TRY(cudaStreamSynchronize(c->stream));
     return DF_OK;
 }

@@ -222,3 +222,69 @@ def test_ann_source_bf16_multi_tile_per_cta(B):
     mech, ann, cells, _ = make_case(2, n, (n + 3) // 4 * 4)
     sample = np.unique(np.concatenate([np.arange(0, n, 97), np.arange(n - 130, n)]))
     check_source(B, mech, ann, cells, n, 2e-2, sample=sample, tol_mixed=BF16_MIXED)
+
+
+# --------------------------------------------------------------------------------------------
+# df_step_host: the whole path over HOST arrays, pipelined in slices (include/df_thermo.h)
+# --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,n,ld", [(1, 4097, 4100), (1, 150001, 150004), (3, 140003, 140004)])
+def test_step_host_matches_device_path_and_oracle(B, cfg, n, ld):
+    """Several slices (n > 2 x 65536), a ragged last slice and ld > n: the host step must give what the three
+    device calls give on the same inputs (same kernels: T, cp, mu, lambda, D bit for bit; omega bit for bit on the
+    fp32 path, within the run-to-run bound of DESIGN.md on the 16-bit path), and T must match the oracle."""
+    mech, ann, cells, om = make_case(cfg, n, ld)
+    K = mech.K
+    h32 = h_from_T(om, cells)
+    gm, ga = B.Mech(mech), B.Ann(ann)
+    # device path
+    dY, dp = dev(cells.Y), dev(cells.p)
+    T = dev(cells.T_guess.copy())
+    B.df_thermo_T_from_h(gm, dev(h32), dY, T)
+    cp, mu, lam = (torch.empty(n, device="cuda") for _ in range(3))
+    D, omg = torch.zeros(K, ld, device="cuda"), torch.zeros(K, ld, device="cuda")
+    B.df_thermo_properties(gm, T, dp, dY, cp=cp, mu=mu, lam=lam, D=D)
+    B.df_chem_ann_source(ga, gm, T, dp, dY, omega=omg, workspace=B.alloc_workspace(ga, n))
+    torch.cuda.synchronize()
+    # host path
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    oT, ocp, omu, olam = (torch.zeros(n).pin_memory() for _ in range(4))
+    oD, oom = torch.zeros(K, ld).pin_memory(), torch.zeros(K, ld).pin_memory()
+    ctx = B.HostCtx(gm, ga, n)
+    for _ in range(2):   # the second call reuses the staging buffers
+        ctx.step(n, ld, pin(h32), pin(cells.p), pin(cells.T_guess), pin(cells.Y), T=oT, cp=ocp, mu=omu, lam=olam, D=oD,
+                 omega=oom)
+    ctx.close()
+    assert np.array_equal(oT.numpy(), T.cpu().numpy())
+    assert np.array_equal(ocp.numpy(), cp.cpu().numpy())
+    assert np.array_equal(omu.numpy(), mu.cpu().numpy())
+    assert np.array_equal(olam.numpy(), lam.cpu().numpy())
+    assert np.array_equal(oD.numpy()[:, :n], D.cpu().numpy()[:, :n])
+    a, b = oom.numpy()[:, :n].astype(np.float64), omg.cpu().numpy()[:, :n].astype(np.float64)
+    if ann.precision == 0:
+        assert np.array_equal(a, b)
+    else:
+        nw = np.linalg.norm(a - b, axis=1) / np.maximum(np.linalg.norm(b, axis=1), 1e-300)
+        assert nw.max() <= 1e-3, nw.max()
+    assert np.all(oom.numpy()[:, n:] == 0) and np.all(oD.numpy()[:, n:] == 0)   # pitch padding untouched
+    T_ref = om.T_from_h(h32, cells.Y[:, :n], cells.T_guess)
+    assert np.abs(oT.numpy() - T_ref).max() <= 1e-3
+
+
+def test_ann_tensor_path_reuses_scratch_across_launches(B):
+    """The 16-bit path hands H2 from its drain to its TMA loads through a per-CTA scratch: a launch on other data in
+    between must not leak into the next one (differences stay at the accumulation-order level)."""
+    from paper_2312_05800_b200 import synth
+    mech, ann, cells, _ = make_case(3, 148 * 128 * 6 + 76)   # ragged last tile, ld % 4 == 0
+    other = synth.cells_stratified(mech.K, cells.n, 12345)
+    gm, ga = B.Mech(mech), B.Ann(ann)
+    ws = B.alloc_workspace(ga, cells.n)
+    a = [dev(x) for x in (cells.T, cells.p, cells.Y)]
+    b = [dev(x) for x in (other.T, other.p, other.Y)]
+    ref, out, tmp = (torch.empty(mech.K, cells.n, device="cuda") for _ in range(3))
+    B.df_chem_ann_source(ga, gm, *a, omega=ref, workspace=ws)
+    for _ in range(4):
+        B.df_chem_ann_source(ga, gm, *b, omega=tmp, workspace=ws)
+        B.df_chem_ann_source(ga, gm, *a, omega=out, workspace=ws)
+        torch.cuda.synchronize()
+        nw = ((out - ref).double().norm(dim=1) / ref.double().norm(dim=1)).max().item()
+        assert nw <= 1e-3, nw
