@@ -39,8 +39,8 @@ constexpr int kTileM = 128;
 #define KGROUPS 3
 #endif
 constexpr int kGroups = KGROUPS;                  // epilogue groups of 4 warps (one warp per TMEM lane quarter)
-constexpr int kIssuer2Warp = 4 + 4 * kGroups;  // second layer-2/3 MMA issuer (after the epilogue warps)
-constexpr int kIoWarp = kIssuer2Warp + 1;      // four cell-I/O warps: next tile's features -> A0, this tile's D4 -> omega
+constexpr int kIssuer2Warp = 3;                // second layer-2/3 MMA issuer
+constexpr int kIoWarp = 4 + 4 * kGroups;       // four cell-I/O warps: next tile's features -> A0, this tile's D4 -> omega
 constexpr int kThreads = 32 * (kIoWarp + 4);
 constexpr int kWStages = 4;
 constexpr int kA1Tiles = 3;                 // [128 x 64] activation tiles of the A1 ring = 2 * kA1Tiles 32-column slots
@@ -171,6 +171,12 @@ __device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
         : "r"(bar), "r"(parity)
         : "memory");
     return done != 0;
+}
+
+// Non-suspending wait for the two producer lanes that share warp 0: a suspended try_wait of one lane would hold back
+// the other lane's loop.
+__device__ __forceinline__ void mbar_poll(uint32_t bar, uint32_t parity) {
+    while (!mbar_test(bar, parity)) { }
 }
 
 __device__ __forceinline__ float tanh_approx(float x) {
@@ -306,12 +312,14 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
     const uint32_t tmem = *tmem_slot;
 
     if (warp == 0) {
-        // ================= weight-ring TMA producer =================
+        // ================= TMA producers: two lanes of one warp, each with its own loop (the two sides of one divergent
+        // branch make independent progress; 20 warps instead of 21 lifts the register cap from 80 to 96) =================
+        // lane 0: weight ring
         if (lane == 0) {
             uint32_t cnt = 0;
             auto load = [&](const uint8_t* src, uint32_t bytes) {
                 const uint32_t slot = cnt % kWStages, par = (cnt / kWStages) & 1;
-                mbar_wait(bar(B_W_EMPTY + slot), par ^ 1);
+                mbar_poll(bar(B_W_EMPTY + slot), par ^ 1);
 #ifdef DF_DBG_NO_TMA
                 mbar_arrive(bar(B_W_FULL + slot));
 #else
@@ -325,10 +333,8 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                 for (int i = 0; i < n2; ++i) load(a.d.w2t + (size_t)i * g.w2_tile_bytes, g.w2_tile_bytes);
                 for (int ks = 0; ks <= g.NKS; ++ks) load(a.d.w3t + (size_t)ks * g.w3_tile_bytes, g.w3_tile_bytes);
             }
-        }
-    } else if (warp == 3) {
-        // ================= auxiliary TMA producer: W4 (once), W1 quads, H2 chunks =================
-        if (lane == 0) {
+        } else if (lane == 1) {
+            // lane 1: W4 (once), W1 quads, H2 chunks
             mbar_expect_tx(bar(B_W4_FULL), g.w4_bytes);
             tma_bulk_g2s(s_w4, a.d.w4t, g.w4_bytes, bar(B_W4_FULL));
             const uint8_t* scratch = a.scratch + (size_t)blockIdx.x * g.NKC * kChunkBytes;
@@ -338,15 +344,15 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                 for (int h = 0; h < 2; ++h)
                     for (int qd = 0; qd < nquads; ++qd, ++w1c) {
                         const uint32_t slot = w1c & 1, par = (w1c >> 1) & 1;
-                        mbar_wait(bar(B_W1_EMPTY + slot), par ^ 1);
+                        mbar_poll(bar(B_W1_EMPTY + slot), par ^ 1);
                         mbar_expect_tx(bar(B_W1_FULL + slot), kW1QuadBytes);
                         tma_bulk_g2s(s_r2 + kChunkBytes + slot * kW1QuadBytes, a.d.w1t + (size_t)qd * kW1QuadBytes,
                                      kW1QuadBytes, bar(B_W1_FULL + slot));
                     }
-                mbar_wait(bar(B_H2_FULL), tc & 1);  // both halves of H2 are in the scratch
+                mbar_poll(bar(B_H2_FULL), tc & 1);  // both halves of H2 are in the scratch
                 for (int kc = 0; kc < g.NKC; ++kc, ++h2c) {
                     const uint32_t slot = h2c & 1, par = (h2c >> 1) & 1;
-                    mbar_wait(bar(B_H2C_EMPTY + slot), par ^ 1);
+                    mbar_poll(bar(B_H2C_EMPTY + slot), par ^ 1);
                     mbar_expect_tx(bar(B_H2C_FULL + slot), kChunkBytes);
                     tma_bulk_g2s(s_r1 + slot * kChunkBytes, scratch + (size_t)kc * kChunkBytes, kChunkBytes,
                                  bar(B_H2C_FULL + slot));
