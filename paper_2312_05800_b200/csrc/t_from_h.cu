@@ -7,6 +7,7 @@
 // fp32 iterations bring T to within a few mK; one fp64 Newton step on the species-level
 // polynomials (fp64 tables, the selected range only) removes the fp32 cancellation error.
 #include "common.cuh"
+#include <cstdlib>
 
 namespace {
 
@@ -252,13 +253,110 @@ t_from_h_fixed_kernel(MechScalars sc, const float* __restrict__ th32, const doub
     if (n_unconv && bad) atomicAdd(n_unconv, bad);
 }
 
+
+// ---- fixed K, all-fp64 solve: one range per cell, no fp32 pass --------------------------------------------------
+// h(T, Y) is increasing in T and both ranges agree at T_mid, so the side of the root is known before any iteration:
+// hi iff h_in >= h(T_mid, Y) = sum_k Y_k c_{k,0} (an fp32 sum is enough: a cell within ~1 mK of T_mid may take either
+// polynomial, they match there to second derivative).  Only the selected range's six mixture coefficients are then
+// accumulated, in fp64 straight from the fp64 tables (6K DFMA per cell), and Newton runs in fp64 on that one
+// polynomial (5 DFMA per iteration; the slope and its reciprocal in fp32 -- a quasi-Newton step with a 1e-7 relative
+// slope error still contracts the error by 1e-7 per iteration).  Against the fp32-pass + fp64-polish kernel above:
+// no 12K packed FMAs, no fp32 Newton with range selects, same number of fp64 operations.
+template <int K>
+__global__ void __launch_bounds__(kThreads, DF_TFH_MINBLOCKS)
+t_from_h_f64_kernel(MechScalars sc, const float* __restrict__ th32, const double* __restrict__ th64, long long n,
+                    long long ld, const float* __restrict__ h, const float* __restrict__ Y, float* __restrict__ T,
+                    float* __restrict__ cp_out, int* __restrict__ n_unconv) {
+    __shared__ __align__(16) double s64[K * 12];
+    __shared__ __align__(16) float s0[(K + 3) & ~3];
+    const long long i0 = ((long long)blockIdx.x * kThreads + threadIdx.x) * 2;
+    const bool any = i0 < n, two = i0 + 1 < n;
+    const long long ic = any ? i0 : 0;
+    float2 y[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const float* yp = Y + (size_t)k * ld + ic;
+        if (two) y[k] = __ldg(reinterpret_cast<const float2*>(yp));
+        else { const float v = __ldg(yp); y[k] = make_float2(v, v); }
+    }
+    float2 hin, tg;
+    if (two) { hin = __ldg(reinterpret_cast<const float2*>(h + ic)); tg = *reinterpret_cast<const float2*>(T + ic); }
+    else { hin = make_float2(__ldg(h + ic), 0.f); hin.y = hin.x; tg = make_float2(T[ic], T[ic]); }
+    for (int i = threadIdx.x; i < K * 12; i += kThreads) s64[i] = th64[i];
+    if (threadIdx.x < K) s0[threadIdx.x] = th32[threadIdx.x * 12 + 6];
+    __syncthreads();
+    if (!any) return;
+
+    float2 hm = make_float2(0.f, 0.f);  // h(T_mid, Y), both cells
+#pragma unroll
+    for (int k = 0; k < K; ++k) hm = __ffma2_rn(y[k], make_float2(s0[k], s0[k]), hm);
+    const bool hi0 = !(hin.x < hm.x), hi1 = !(hin.y < hm.y);  // A2: hi for T >= T_mid
+    const double* qa = s64 + (hi0 ? 6 : 0);
+    const double* qb = s64 + (hi1 ? 6 : 0);
+    double A[6], Bc[6];
+#pragma unroll
+    for (int m = 0; m < 6; ++m) A[m] = Bc[m] = 0.0;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const double ya = (double)y[k].x, yb = (double)y[k].y;
+#pragma unroll
+        for (int m = 0; m < 6; ++m) {
+            A[m] = fma(ya, qa[k * 12 + m], A[m]);
+            Bc[m] = fma(yb, qb[k * 12 + m], Bc[m]);
+        }
+    }
+    // slope coefficients in fp32
+    const float a1 = (float)A[1], a2 = 2.f * (float)A[2], a3 = 3.f * (float)A[3], a4 = 4.f * (float)A[4], a5 = 5.f * (float)A[5];
+    const float b1 = (float)Bc[1], b2 = 2.f * (float)Bc[2], b3 = 3.f * (float)Bc[3], b4 = 4.f * (float)Bc[4], b5 = 5.f * (float)Bc[5];
+    // A4: invalid guess -> T_mid; the start is moved onto the root's side of T_mid, the iterates stay there
+    float ga = (tg.x > 0.f && tg.x < 3.0e38f) ? (tg.x - sc.T_mid) * sc.inv_S : 0.f;
+    float gb = (tg.y > 0.f && tg.y < 3.0e38f) ? (tg.y - sc.T_mid) * sc.inv_S : 0.f;
+    const double la = hi0 ? 0.0 : (double)sc.tau_min, ua = hi0 ? (double)sc.tau_max : 0.0;
+    const double lb = hi1 ? 0.0 : (double)sc.tau_min, ub = hi1 ? (double)sc.tau_max : 0.0;
+    double ta = fmin(fmax((double)ga, la), ua), tb = fmin(fmax((double)gb, lb), ub);
+    const double ha = (double)hin.x, hb = (double)hin.y;
+    double da = 0.0, db = 0.0;
+    for (int it = 0; it < kMaxIter; ++it) {
+        const double va = fma(fma(fma(fma(fma(A[5], ta, A[4]), ta, A[3]), ta, A[2]), ta, A[1]), ta, A[0]);
+        const double vb = fma(fma(fma(fma(fma(Bc[5], tb, Bc[4]), tb, Bc[3]), tb, Bc[2]), tb, Bc[1]), tb, Bc[0]);
+        const float fa = (float)ta, fb = (float)tb;
+        const float sa = fmaf(fmaf(fmaf(fmaf(a5, fa, a4), fa, a3), fa, a2), fa, a1);
+        const float sb = fmaf(fmaf(fmaf(fmaf(b5, fb, b4), fb, b3), fb, b2), fb, b1);
+        da = (ha - va) * (double)__frcp_rn(sa);
+        db = (hb - vb) * (double)__frcp_rn(sb);
+        ta = fmin(fmax(ta + da, la), ua);
+        tb = fmin(fmax(tb + db, lb), ub);
+        if (!(fmax(fabs(da), fabs(db)) >= 1e-6)) break;  // 1 mK step: the error left is ~1e-9 K (also leaves on NaN)
+    }
+    const float fa = (float)ta, fb = (float)tb;
+    const float cpa = fmaf(fmaf(fmaf(fmaf(a5, fa, a4), fa, a3), fa, a2), fa, a1) * sc.inv_S;
+    const float cpb = fmaf(fmaf(fmaf(fmaf(b5, fb, b4), fb, b3), fb, b2), fb, b1) * sc.inv_S;
+    const float Ta = (float)fma(ta, (double)sc.S, (double)sc.T_mid), Tb = (float)fma(tb, (double)sc.S, (double)sc.T_mid);
+    int bad = 0;
+    if (!(fabs(da) * (double)sc.S <= 1e-2)) ++bad;
+    if (two && !(fabs(db) * (double)sc.S <= 1e-2)) ++bad;
+    if (two) {
+        *reinterpret_cast<float2*>(T + i0) = make_float2(Ta, Tb);
+        if (cp_out) *reinterpret_cast<float2*>(cp_out + i0) = make_float2(cpa, cpb);
+    } else {
+        T[i0] = Ta;
+        if (cp_out) cp_out[i0] = cpa;
+    }
+    if (n_unconv && bad) atomicAdd(n_unconv, bad);
+}
+
 template <int K>
 df_status launch_fixed(const df_mech* mech, long long n, long long ld, const float* h, const float* Y, float* T, float* cp,
                        int* n_unconv, cudaStream_t s) {
     const long long blocks = (n + 2 * kThreads - 1) / (2 * kThreads);
     if (blocks > 0x7fffffffLL) return df_set_error(DF_ERR_UNSUPPORTED, "df_thermo_T_from_h: n_cells too large");
-    t_from_h_fixed_kernel<K><<<(unsigned)blocks, kThreads, 0, s>>>(mech->dev.sc, mech->dev.th32, mech->dev.th64, n, ld, h, Y,
-                                                                   T, cp, n_unconv);
+    static const bool v1 = getenv("DF_TFH_V1") != nullptr;
+    if (v1)
+        t_from_h_fixed_kernel<K><<<(unsigned)blocks, kThreads, 0, s>>>(mech->dev.sc, mech->dev.th32, mech->dev.th64, n, ld, h, Y,
+                                                                       T, cp, n_unconv);
+    else
+        t_from_h_f64_kernel<K><<<(unsigned)blocks, kThreads, 0, s>>>(mech->dev.sc, mech->dev.th32, mech->dev.th64, n, ld, h, Y,
+                                                                     T, cp, n_unconv);
     DF_CUDA_TRY(cudaGetLastError());
     return DF_OK;
 }
