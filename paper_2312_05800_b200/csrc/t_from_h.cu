@@ -283,8 +283,10 @@ t_from_h_sorted_kernel(MechScalars sc, const float* __restrict__ th32, const dou
     // A4: invalid guess -> T_mid; the start is moved onto the root's side of T_mid, the iterates stay there
     const float ga = (tg.x > 0.f && tg.x < 3.0e38f) ? (tg.x - sc.T_mid) * sc.inv_S : 0.f;
     const float gb = (tg.y > 0.f && tg.y < 3.0e38f) ? (tg.y - sc.T_mid) * sc.inv_S : 0.f;
-    const double la = s_hi0 ? 0.0 : (double)sc.tau_min, ua = s_hi0 ? (double)sc.tau_max : 0.0;
-    const double lb = s_hi1 ? 0.0 : (double)sc.tau_min, ub = s_hi1 ? (double)sc.tau_max : 0.0;
+    // (the side was picked in fp32: a root within a few mK of T_mid may lie just across it, hence the 1 K margin)
+    constexpr double kMargin = 1e-3;
+    const double la = s_hi0 ? -kMargin : (double)sc.tau_min, ua = s_hi0 ? (double)sc.tau_max : kMargin;
+    const double lb = s_hi1 ? -kMargin : (double)sc.tau_min, ub = s_hi1 ? (double)sc.tau_max : kMargin;
     double ta = fmin(fmax((double)ga, la), ua), tb = fmin(fmax((double)gb, lb), ub);
     const double ha = (double)hin.x, hb = (double)hin.y;
     double da = 0.0, db = 0.0;

@@ -65,6 +65,40 @@ def test_T_from_h(B, cfg, n, ld, guess):
     assert helpers.rel_err(cp.cpu().numpy(), cp_ref).max() <= 1e-5
 
 
+@pytest.mark.parametrize("n,ld", [(1, 4), (127, 128), (129, 132), (257, 260), (1000, 1000)])
+@pytest.mark.parametrize("side", ["lo", "hi", "mid", "mixed"])
+def test_T_from_h_range_sorted_blocks(B, n, ld, side):
+    """The fixed-K kernel sorts each 256-cell block by NASA range before the coefficient pass: blocks that are all
+    lo, all hi, sit on T_mid (either polynomial is right there, A2) or mix both, at sizes around the warp / block
+    boundaries, must all come back to the oracle's root; the pad between n and ld must stay untouched."""
+    mech, _, cells, om = make_case(3, n, ld)
+    rng = np.random.default_rng(n * 7 + len(side))
+    if side == "lo":
+        cells.T[:] = rng.uniform(300.0, 999.0, n)
+    elif side == "hi":
+        cells.T[:] = rng.uniform(1001.0, 3400.0, n)
+    elif side == "mid":
+        cells.T[:] = 1000.0 + rng.choice([0.0, 1e-3, -1e-3, 0.5, -0.5], n)
+    h32 = h_from_T(om, cells)
+    g = np.full(n, 1000.0, np.float32) if side == "mid" else rng.uniform(300.0, 3400.0, n).astype(np.float32)
+    T_ref = om.T_from_h(h32, cells.Y[:, :n], g)
+    gm = B.Mech(mech)
+    Tbuf = torch.full((ld,), -7.0, device="cuda")
+    Tbuf[:n] = dev(g)
+    cp = torch.full((ld,), -7.0, device="cuda")
+    hbuf = torch.zeros(ld, device="cuda")
+    hbuf[:n] = dev(h32)
+    cnt = torch.zeros(1, dtype=torch.int32, device="cuda")
+    B.df_thermo_T_from_h(gm, hbuf, dev(cells.Y), Tbuf, cp=cp, n_unconverged=cnt, n_cells=n)
+    torch.cuda.synchronize()
+    Tg = Tbuf.cpu().numpy()
+    assert np.abs(Tg[:n].astype(np.float64) - T_ref).max() <= 1e-3
+    assert int(cnt.item()) == 0
+    assert (Tg[n:] == -7.0).all() and (cp.cpu().numpy()[n:] == -7.0).all()
+    cp_ref, _ = om.mixture_cp_h(Tg[:n], cells.Y[:, :n])
+    assert helpers.rel_err(cp.cpu().numpy()[:n], cp_ref).max() <= 1e-5
+
+
 def test_T_from_h_empty_and_errors(B):
     mech, _, cells, om = make_case(1, 64)
     gm = B.Mech(mech)
