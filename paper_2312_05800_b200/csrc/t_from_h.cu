@@ -218,11 +218,19 @@ t_from_h_sorted_kernel(MechScalars sc, const float* __restrict__ th32, const dou
     const int c0 = tid, c1 = tid + kThreads;  // this thread's cells before the sort
     const bool in0 = base + c0 < n, in1 = base + c1 < n;
     const long long i0 = in0 ? base + c0 : 0, i1 = in1 ? base + c1 : 0;
-    float2 y[K];
+    float2 y[K], hin, tg;
+    if (base + kSCells <= n) {  // whole block in range: one pointer, the second cell at a constant offset
+        const float* yp = Y + i0;
 #pragma unroll
-    for (int k = 0; k < K; ++k) y[k] = make_float2(__ldg(Y + (size_t)k * ld + i0), __ldg(Y + (size_t)k * ld + i1));
-    float2 hin = make_float2(__ldg(h + i0), __ldg(h + i1));
-    float2 tg = make_float2(T[i0], T[i1]);
+        for (int k = 0; k < K; ++k, yp += ld) y[k] = make_float2(__ldg(yp), __ldg(yp + kThreads));
+        hin = make_float2(__ldg(h + i0), __ldg(h + i0 + kThreads));
+        tg = make_float2(T[i0], T[i0 + kThreads]);
+    } else {
+#pragma unroll
+        for (int k = 0; k < K; ++k) y[k] = make_float2(__ldg(Y + (size_t)k * ld + i0), __ldg(Y + (size_t)k * ld + i1));
+        hin = make_float2(__ldg(h + i0), __ldg(h + i1));
+        tg = make_float2(T[i0], T[i1]);
+    }
     for (int i = tid; i < K * 12; i += kThreads) s64[i] = th64[i];
     if (tid < K) s0[tid] = th32[tid * 12 + 6];
     __syncthreads();
