@@ -249,6 +249,24 @@ def run_gpu(args):
     value = aggregate_value(world, n, ms_step)
     k_ms = [float(np.mean([e[i].elapsed_time(e[i + 1]) for e in marks])) for i in range(3)]
 
+    # ---- optional: each kernel timed alone (its own launches back to back, the board not power-limited by the MLP) ----
+    alone_ms = None
+    if args.kernels_alone:
+        def alone(launch, reps=12):
+            ts = []
+            for _ in range(reps):
+                dT.copy_(dTg)
+                a, b = ev(), ev()
+                a.record(stream); launch(); b.record(stream)
+                torch.cuda.synchronize()
+                ts.append(a.elapsed_time(b))
+            return float(np.median(ts[2:]))
+        time.sleep(2.0)
+        alone_ms = {"T_from_h": alone(lambda: B.df_thermo_T_from_h(gm, dh, dY, dT))}
+        B.df_thermo_T_from_h(gm, dh, dY, dT)
+        alone_ms["properties"] = alone(lambda: B.df_thermo_properties(gm, dT0, dp, dY, cp=cp, mu=mu, lam=lam, D=D))
+        alone_ms["ann_bf16"] = alone(lambda: B.df_chem_ann_source(ga, gm, dT0, dp, dY, omega=om, workspace=ws), reps=5)
+
     # ---- e2e: the same step through df_step_host with pinned HOST buffers ----
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     hh, hp, hg, hY = pin(dh.cpu().numpy()), pin(cells.p), pin(cells.T_guess), pin(cells.Y)
@@ -289,6 +307,7 @@ def run_gpu(args):
                    "cells_per_gpu": n, "l2": "inputs (176 MB/step at the full size) exceed the 126 MB L2; no explicit flush",
                    "parallelism": f"replicas x{world} (no collective in the data path)"},
         "kernel_ms": {"T_from_h": k_ms[0], "properties": k_ms[1], "ann_bf16": k_ms[2]},
+        **({"kernel_alone_ms": alone_ms} if alone_ms else {}),
         "roofline": {"bound": "tensor", "kernel": "ann_bf16_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                      "frac": achieved / peak,
                      # dram__bytes_read.sum + dram__bytes_write.sum of one launch at the full size (profiles/r1_summary.md)
@@ -316,6 +335,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-cells", type=int, default=262144, help="cells per oracle pass (cpu_baseline / reference arm)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--kernels-alone", action="store_true",
+                    help="also time each kernel alone (median of its own launches), reported as kernel_alone_ms")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
