@@ -311,7 +311,7 @@ def run_gpu(args):
         "roofline": {"bound": "tensor", "kernel": "ann_bf16_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                      "frac": achieved / peak,
                      # dram__bytes_read.sum + dram__bytes_write.sum of one launch at the full size (profiles/r1_summary.md)
-                     "traffic": 326.1e6 if n == 2097152 else None,
+                     "traffic": 325.7e6 if n == 2097152 else None,
                      "peak_source": peak_src, "frac_vs_burst": achieved / pk["bf16"],
                      "frac_vs_sustained": achieved / pk["bf16_sust"],
                      "algorithmic": f"{FLOPS_PER_CELL_MLP} flop/cell x {n} cells/launch"},
