@@ -1,11 +1,13 @@
 // t_from_h.cu -- K1: temperature from enthalpy by Newton on NASA-7 (NS (1)).
 //
-// HBM-bound: 4(K+2) bytes in + 4 (T) [+ 4 (cp)] out per cell.  One thread owns 4 consecutive cells
-// (float4 SoA loads, coalesced across the warp).  For fixed Y, h(T,Y) is itself one polynomial in
-// tau = (T - T_mid)/S with mixture coefficients C_m = sum_k Y_k c_{k,m}: the K-loop runs once
-// (12 FMAs per species per cell, both ranges), every Newton iteration is then K-independent.
-// fp32 iterations bring T to within a few mK; one fp64 Newton step on the species-level
-// polynomials (fp64 tables, the selected range only) removes the fp32 cancellation error.
+// HBM-bound: 4(K+2) bytes in + 4 (T) [+ 4 (cp)] out per cell.  For fixed Y, h(T,Y) is itself one polynomial in
+// tau = (T - T_mid)/S with mixture coefficients C_m = sum_k Y_k c_{k,m}: the K-loop runs once, every Newton
+// iteration is then K-independent.  Two kernels:
+//  * t_from_h_sorted_kernel<K> (K = 9, 19: the configs' species counts): all fp64, one range per cell, the block's
+//    cells sorted by range through shared memory so that the table reads are warp-uniform (see its header below);
+//  * t_from_h_kernel (any K): one thread owns 4 consecutive cells (float4 SoA loads); fp32 mixture coefficients of
+//    both ranges (12 FMAs per species per cell), fp32 iterations to a few mK, then one fp64 Newton step on the
+//    species-level polynomials (fp64 tables, the selected range only) that removes the fp32 cancellation error.
 #include "common.cuh"
 
 namespace {

@@ -99,6 +99,27 @@ def test_T_from_h_range_sorted_blocks(B, n, ld, side):
     assert helpers.rel_err(cp.cpu().numpy()[:n], cp_ref).max() <= 1e-5
 
 
+def test_T_from_h_nan_cells_do_not_spread(B):
+    """A18: NaN in h or Y must neither hang nor fault, is counted as unconverged, and leaves the other cells of the
+    block (which share threads and shared-memory slots with it after the range sort) at the oracle's root."""
+    n = 1500
+    mech, _, cells, om = make_case(3, n)
+    h32 = h_from_T(om, cells)
+    Y = cells.Y.copy()
+    bad = np.zeros(n, bool)
+    bad[[0, 1, 130, 255, 256, 700, 1499]] = True
+    h32[[0, 130, 256, 1499]] = np.nan
+    Y[3, [1, 255, 700]] = np.nan
+    T_ref = om.T_from_h(h32[~bad], np.ascontiguousarray(cells.Y[:, ~bad]), cells.T_guess[~bad])
+    gm = B.Mech(mech)
+    T = dev(cells.T_guess)
+    cnt = torch.zeros(1, dtype=torch.int32, device="cuda")
+    B.df_thermo_T_from_h(gm, dev(h32), dev(Y), T, n_unconverged=cnt)
+    torch.cuda.synchronize()
+    assert np.abs(T.cpu().numpy()[~bad].astype(np.float64) - T_ref).max() <= 1e-3
+    assert int(cnt.item()) == int(bad.sum())
+
+
 def test_T_from_h_empty_and_errors(B):
     mech, _, cells, om = make_case(1, 64)
     gm = B.Mech(mech)
