@@ -18,9 +18,11 @@
 // are re-tiled at create time into the exact 128B-swizzled K-major shared-memory images the UMMA descriptors
 // expect, in streaming order, so every TMA transfer is one contiguous cp.async.bulk of 8-26 KB.
 //
-// Warp roles (128 + 128 kGroups threads): 0 = weight-ring TMA producer, 1 = layer-2/3/4 MMA issuer, 2 = TMEM
-// allocator and layer-1 MMA issuer, 3 = auxiliary TMA producer (W1 quads, H2 chunks, W4), 4.. = kGroups epilogue
-// groups of four warps (warp w owns TMEM lanes 32 (w % 4) .. +31); group g takes every kGroups-th layer-1 chunk.
+// Warp roles (20 warps): 0 = the two TMA producers (lane 0: weight ring; lane 1: W4, W1 quads, H2 chunks -- the two
+// sides of one divergent branch), 1 and 3 = the two alternating layer-2/3 MMA issuers (warp 1 also issues layer 4),
+// 2 = TMEM allocator and layer-1 MMA issuer, 4..15 = kGroups epilogue groups of four warps (warp w owns TMEM lanes
+// 32 (w % 4) .. +31; group g takes every kGroups-th layer-1 chunk), 16..19 = four cell-I/O warps (next tile's
+// Box-Cox features -> A0, previous tile's D4 -> inverse Box-Cox -> omega).
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
@@ -35,10 +37,7 @@ namespace {
 
 // ---- geometry ---------------------------------------------------------------------------------
 constexpr int kTileM = 128;
-#ifndef KGROUPS
-#define KGROUPS 3
-#endif
-constexpr int kGroups = KGROUPS;                  // epilogue groups of 4 warps (one warp per TMEM lane quarter)
+constexpr int kGroups = 3;                     // epilogue groups of 4 warps (one warp per TMEM lane quarter)
 constexpr int kIssuer2Warp = 3;                // second layer-2/3 MMA issuer
 constexpr int kIoWarp = 4 + 4 * kGroups;       // four cell-I/O warps: next tile's features -> A0, this tile's D4 -> omega
 constexpr int kThreads = 32 * (kIoWarp + 4);
@@ -52,7 +51,6 @@ constexpr int kSmallBufs = 3;
 constexpr int kTmemCols = 512;
 
 struct NetGeom {
-    int b_fmt;               // UMMA B (weight) format: 1 = bf16, 0 = fp16
     int K, K0steps;          // species, k-steps (of 16) over the K+4 layer-1 inputs (features, 2 bias columns)
     int d1, d2, d3;          // hidden widths
     int NC;                  // d1 / 32 chunks of layer 1 (one 32-wide K stage of layer 2 each)
@@ -82,7 +80,6 @@ struct Bf16Plan {
     Bf16Dev d;
     float b4_host[32] = {0};
     void* blob = nullptr;
-    int num_sms = 0;
 };
 
 namespace {
@@ -147,10 +144,10 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
     return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) |
            ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
 }
-// kind::f16 instruction descriptor: D = f32, A = fp16 activations (format 0), B = bf16 weights (format 1),
-// both K-major, M = 128.
-__device__ __forceinline__ uint32_t umma_idesc(int N, int b_fmt) {
-    return (1u << 4) | (0u << 7) | ((uint32_t)b_fmt << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
+// kind::f16 instruction descriptor: D = f32 (bit 4), A and B = fp16 (format 0 in bits 7.. and 10..: kind::f16 wants
+// both operands in one format, A21), both K-major, N >> 3 in bits 17.., M >> 4 in bits 24..
+__device__ __forceinline__ uint32_t umma_idesc(int N) {
+    return (1u << 4) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
 }
 __device__ __forceinline__ bool elect_one() {
     uint32_t pred;
@@ -184,29 +181,28 @@ __device__ __forceinline__ float tanh_approx(float x) {
     asm("tanh.approx.f32 %0, %1;" : "=f"(r) : "f"(x));
     return r;
 }
-// GELU in its tanh form (within 5e-4 of x Phi(x); the bf16 rounding that follows is 4e-3 relative).
-__device__ __forceinline__ float gelu_fast(float v) {
-#ifdef DF_DBG_NO_GELU
-    return v;
-#endif
-    const float u = v * fmaf(0.0356774081f, v * v, 0.7978845608f);
-    const float hv = 0.5f * v;
-    return fmaf(hv, tanh_approx(u), hv);
-}
-// GELU (tanh form) on two packed fp16 values: 6 half2 instructions + 1 MUFU for two activations.  The inputs are the
-// fp32 accumulators rounded to fp16 (2^-11), the arithmetic adds ~1e-3 relative: well inside the 2e-2 budget (A12).
-__device__ __forceinline__ uint32_t gelu_h2(uint32_t v) {
+// two fp32 -> packed fp16x2 (first argument in the low half = lower K index); saturates at +-65504 instead of inf
+__device__ __forceinline__ uint32_t pack_act(float lo, float hi) {
     uint32_t r;
-    asm("{\n\t.reg .b32 vv, t, u, th, hv;\n\t"
-        "mul.f16x2 vv, %1, %1;\n\t"
-        "fma.rn.f16x2 t, vv, %2, %3;\n\t"
-        "mul.f16x2 u, t, %1;\n\t"
-        "tanh.approx.f16x2 th, u;\n\t"
-        "mul.f16x2 hv, %1, %4;\n\t"
-        "fma.rn.f16x2 %0, hv, th, hv;\n\t}"
-        : "=r"(r)
-        : "r"(v), "r"(0x28912891u) /* 0.035677 */, "r"(0x3A623A62u) /* 0.79788 */, "r"(0x38003800u) /* 0.5 */);
+    asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
     return r;
+}
+// GELU (A13) of two fp32 accumulators -> packed fp16x2.  Tanh form v/2 (1 + tanh(sqrt(2/pi) (v + 0.044715 v^3))),
+// evaluated in packed fp32 (FFMA2) with MUFU.TANH in fp32 (measured 3e-6 rms on this part) and rounded to fp16 once,
+// at the end: next to an exactly rounded fp16 activation the only error left is that of the tanh form (<= 4.7e-4
+// at |v| ~ 2-3, but third-order exact at v = 0 where the pre-activations live: it moves the network output by 3e-6
+// rms against 2e-5 from the fp16 roundings).  A minimax refit of the two constants halves the maximum error and was
+// tried: it is WORSE (its slope error at v = 0 is systematic and adds up coherently over 1600 units: 4.6e-5 rms at
+// the output).  The earlier all-fp16x2 evaluation (fp16 v, three fp16 roundings inside the tanh argument,
+// tanh.approx.f16x2) had 2-3x the rounding error of the result's own fp16 rounding, and its v*v overflowed for
+// |v| > 255.
+__device__ __forceinline__ uint32_t gelu_pair(float a, float b) {
+    const float2 v = make_float2(a, b);
+    const float2 t = __ffma2_rn(__fmul2_rn(v, v), make_float2(0.0356774081f, 0.0356774081f), make_float2(0.7978845608f, 0.7978845608f));
+    const float2 u = __fmul2_rn(t, v);
+    const float2 hv = __fmul2_rn(v, make_float2(0.5f, 0.5f));
+    const float2 r = __ffma2_rn(hv, make_float2(tanh_approx(u.x), tanh_approx(u.y)), hv);
+    return pack_act(r.x, r.y);
 }
 // dY*_k of ann_common.cuh with MUFU-grade transcendentals (ex2/lg2/rcp.approx): 5 MUFU + a few FMA per species
 // instead of powf/log1pf/expm1f (~400 instructions).  Its error (<= 2e-4 relative for |lambda Delta| >= 1e-3 Y^lambda)
@@ -220,12 +216,6 @@ __device__ __forceinline__ float ann_dystar_fast(float y, float delta, float lam
     const float base = lambda * delta;
     const float zero = base > 0.f ? exp2f(__log2f(base) * inv_lambda) : 0.f;
     return y > 0.f ? ((z > -1.0f) ? pos : -y) : zero;
-}
-// two fp32 -> packed fp16x2 (first argument in the low half = lower K index)
-__device__ __forceinline__ uint32_t pack_act(float lo, float hi) {
-    uint32_t r;
-    asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
-    return r;
 }
 // byte offset of 16-byte chunk c16 (0..7) of row r inside a 128B-swizzled [rows x 64] bf16 tile
 __device__ __forceinline__ uint32_t swz(int r, int c16) { return (uint32_t)(r * 128 + ((c16 ^ (r & 7)) << 4)); }
@@ -241,19 +231,6 @@ __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&r)[32]) {
         : "r"(taddr)
         : "memory");
 }
-
-#ifdef DF_DBG_PROGRESS
-__device__ volatile int* g_prog = nullptr;   // mapped host memory: [role][8] progress counters of block 0
-#define PROG(role, slot, val) do { if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && g_prog) g_prog[(role) * 8 + (slot)] = (val); } while (0)
-#else
-#define PROG(role, slot, val) do { } while (0)
-#endif
-#ifdef DF_DBG_CLK
-__device__ long long g_dbg[16][128];
-#define DBG_REC(row, idx, cond) do { if ((cond) && blockIdx.x == 0 && (idx) < 128) g_dbg[row][idx] = clock64(); } while (0)
-#else
-#define DBG_REC(row, idx, cond) do { } while (0)
-#endif
 
 // barrier indices
 enum {
@@ -320,12 +297,8 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             auto load = [&](const uint8_t* src, uint32_t bytes) {
                 const uint32_t slot = cnt % kWStages, par = (cnt / kWStages) & 1;
                 mbar_poll(bar(B_W_EMPTY + slot), par ^ 1);
-#ifdef DF_DBG_NO_TMA
-                mbar_arrive(bar(B_W_FULL + slot));
-#else
                 mbar_expect_tx(bar(B_W_FULL + slot), bytes);
                 tma_bulk_g2s(s_w + slot * g.w_slot_bytes, src, bytes, bar(B_W_FULL + slot));
-#endif
                 ++cnt;
             };
             for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
@@ -364,7 +337,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
         // Layer 1 has its own issuing warp so that neither issuer has more than two mbarrier round trips per
         // 32-column chunk: it runs ahead of layer 2 as far as the three D1 buffers allow.  Whole warp convergent,
         // one elected lane issues (ptxas then keeps descriptors and barrier addresses in uniform registers).
-        const uint32_t id32 = umma_idesc(32, g.b_fmt);
+        const uint32_t id32 = umma_idesc(32);
         const uint64_t dA0 = umma_desc(s_r2), dW1 = umma_desc(s_r2 + kChunkBytes);
         uint32_t w1c = 0, gs = 0, ac = 0, tc = 0;
         for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tc) {
@@ -373,10 +346,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                 for (int c = 0; c < g.NC; ++c, ++gs, ++ac) {
                     const uint32_t slot = w1c & 1, sb = gs % kSmallBufs;
                     if ((c & 3) == 0) mbar_wait(bar(B_W1_FULL + slot), (w1c >> 1) & 1);
-                    PROG(0, 0, (int)gs);
                     mbar_wait(bar(B_SMALL_EMPTY + sb), ((gs / kSmallBufs) & 1) ^ 1);
-                    PROG(0, 1, (int)gs);
-                    DBG_REC(0, gs - 150, lane == 0 && gs >= 150);
                     tc_fence_after();
                     const bool quad_done = (c & 3) == 3 || c == g.NC - 1;
                     if (elect_one()) {
@@ -388,7 +358,6 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                         if (quad_done) tc_commit(bar(B_W1_EMPTY + slot));
                     }
                     __syncwarp();
-                    DBG_REC(1, gs - 150, lane == 0 && gs >= 150);
                     if (quad_done) ++w1c;
                 }
             ++gs;  // the D4 accumulation of this tile (issued by warp 1) takes the next buffer of the ring
@@ -401,9 +370,9 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
         // accumulation (the bias stage, accumulate = 0) is announced on B_ACC_START before the other issuer adds to it;
         // barriers that follow a whole accumulation / H2 tile (ACC_FULL, H2C_EMPTY) take one commit from each issuer.
         const int id = (warp == 1) ? 0 : 1;
-        const uint32_t id32 = umma_idesc(32, g.b_fmt);
-        const uint32_t id2a = umma_idesc(g.na2, g.b_fmt), id2b = umma_idesc(g.nb2 > 0 ? g.nb2 : 16, g.b_fmt);
-        const uint32_t id3a = umma_idesc(g.n3a, g.b_fmt), id3b = umma_idesc(g.n3b > 0 ? g.n3b : 16, g.b_fmt);
+        const uint32_t id32 = umma_idesc(32);
+        const uint32_t id2a = umma_idesc(g.na2), id2b = umma_idesc(g.nb2 > 0 ? g.nb2 : 16);
+        const uint32_t id3a = umma_idesc(g.n3a), id3b = umma_idesc(g.n3b > 0 ? g.n3b : 16);
         const uint64_t dR2 = umma_desc(s_r2), dR1 = umma_desc(s_r1), dW = umma_desc(s_w), dW4 = umma_desc(s_w4);
         const uint32_t w_slot16 = (uint32_t)g.w_slot_bytes >> 4;
         // st: stages of the weight ring; gs: uses of the small-accumulator ring; ac: uses of the A1 slots;
@@ -447,13 +416,9 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                 for (int c = 0; c < g.NC; ++c, ++ac, ++st) {
                     if ((int)(st & 1) != id) continue;
                     const uint32_t slot = ac % kA1Slots;
-                    PROG(1 + id, 0, (int)ac);
                     mbar_wait(bar(B_A1_FULL + slot), (ac / kA1Slots) & 1);
-                    PROG(1 + id, 1, (int)ac);
-                    DBG_REC(2, ac - 150, lane == 0 && ac >= 150);
                     issue_stage(dR1 + (((slot >> 1) * kChunkBytes + (slot & 1) * 64) >> 4), g.na2, g.nb2, id2a, id2b, false,
                                 bar(B_A1_EMPTY + slot));
-                    DBG_REC(3, ac - 150, lane == 0 && ac >= 150);
                 }
                 if (elect_one()) tc_commit(bar(B_ACC_FULL));
                 __syncwarp();
@@ -516,24 +481,19 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
         // GELU on 16 accumulators (biases are already in them) -> 8 packed fp16x2 words
         auto gelu16 = [&](const uint32_t* r, uint32_t (&o)[8]) {
 #pragma unroll
-            for (int i = 0; i < 8; ++i) o[i] = gelu_h2(pack_act(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1])));
+            for (int i = 0; i < 8; ++i) o[i] = gelu_pair(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1]));
         };
 
         uint32_t tcnt = 0;
         for (long long tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tcnt) {
-            DBG_REC(12, tcnt * 16 + 0, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
             // the H3 ring lives in R1: the previous tile's layer-4 MMAs must be done before A1 chunks go there again
             if (tcnt > 0) mbar_wait(bar(B_TILE_DONE), (tcnt - 1) & 1);
-            DBG_REC(12, tcnt * 16 + 1, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
             // ---- phase A ----
             for (int h = 0; h < 2; ++h) {
                 for (int c = 0; c < g.NC; ++c, ++gs, ++ac) {
                     if ((int)(ac % kGroups) != grp) continue;
                     const uint32_t sb = gs % kSmallBufs;
-                    if (q == 0) PROG(3 + grp, 0, (int)gs);
                     mbar_wait(bar(B_SMALL_FULL + grp), (ac / kGroups) & 1);
-                    if (q == 0) PROG(3 + grp, 1, (int)gs);
-                    DBG_REC(4, gs - 150, lane == 0 && q == 0 && gs >= 150);
                     tc_fence_after();
                     uint32_t r[32];
                     tc_ld32(t_lane + kSmallCol + sb * 32, r);
@@ -541,16 +501,12 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar(B_SMALL_EMPTY + sb));
-                    DBG_REC(5, gs - 150, lane == 0 && q == 0 && gs >= 150);
                     uint32_t o[16];
 #pragma unroll
                     for (int i = 0; i < 16; ++i)   // b1 is already in the accumulator (bias columns of W1)
-                        o[i] = gelu_h2(pack_act(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1])));
+                        o[i] = gelu_pair(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1]));
                     const uint32_t slot = ac % kA1Slots;
-                    DBG_REC(6, ac - 150, lane == 0 && q == 0 && ac >= 150);
-                    if (q == 0) PROG(3 + grp, 2, (int)ac);
                     mbar_wait(bar(B_A1_EMPTY + slot), ((ac / kA1Slots) & 1) ^ 1);
-                    if (q == 0) PROG(3 + grp, 3, (int)ac);
                     const uint32_t base = s_r1 + (slot >> 1) * kChunkBytes;
 #pragma unroll
                     for (int c4 = 0; c4 < 4; ++c4)
@@ -558,15 +514,10 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                     fence_proxy_async_smem();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar(B_A1_FULL + slot));
-                    DBG_REC(7, ac - 150, lane == 0 && q == 0 && ac >= 150);
                 }
                 // drain D2 (this half): +b2, GELU, fp16 -> H2 scratch in the chunk images phase B loads
-                DBG_REC(12, tcnt * 16 + 3 + 3 * h, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
-                if (q == 0) PROG(3 + grp, 4, (int)af);
                 mbar_wait(bar(B_ACC_FULL), af & 1);
                 ++af;
-                if (q == 0) PROG(3 + grp, 5, (int)af);
-                DBG_REC(12, tcnt * 16 + 4 + 3 * h, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
                 tc_fence_after();
                 {
                     // software-pipelined: the TMEM load of the next 16-column unit is in flight during the math
@@ -601,7 +552,6 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                         c0 += kStep;
                     }
                 }
-                DBG_REC(12, tcnt * 16 + 15, lane == 0 && q == 0 && grp == 0 && tcnt < 8 && h == 1);
                 tc_fence_before();
                 // generic-proxy stores to the scratch -> async-proxy (TMA) reads by warp 3 of this CTA: the proxy fence for
                 // the global space, then the release/acquire pair of the mbarrier.  (A preceding __threadfence and the
@@ -612,13 +562,10 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
                     mbar_arrive(bar(B_ACC_EMPTY));
                     mbar_arrive(bar(B_H2_FULL));
                 }
-                DBG_REC(12, tcnt * 16 + 5 + 3 * h, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
             }
             // ---- phase B: drain D3 in 64-wide chunks -> H3 ring (feeds layer 4); group grp owns 16-column unit grp ----
-            DBG_REC(12, tcnt * 16 + 9, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
             mbar_wait(bar(B_ACC_FULL), af & 1);
             ++af;
-            DBG_REC(12, tcnt * 16 + 10, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
             tc_fence_after();
             for (int jj = 0; jj < g.NJ; ++jj, ++h3c) {
                 // the four 16-column units of this 64-wide chunk go round-robin over the groups, continuing from the
@@ -654,7 +601,6 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(B_ACC_EMPTY));
-            DBG_REC(12, tcnt * 16 + 11, lane == 0 && q == 0 && grp == 0 && tcnt < 8);
             ++gs;   // the D4 accumulation of this tile takes the next buffer of the small ring (read by the I/O warps)
         }
     } else if (warp >= kIoWarp && warp < kIoWarp + 4) {
@@ -783,27 +729,21 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
 // ---- host side: geometry, weight re-tiling, launch ------------------------------------------------
 namespace {
 
-uint16_t bf16_bits(float x) {  // round to nearest even
-    uint32_t u;
-    memcpy(&u, &x, 4);
-    if ((u & 0x7F800000u) == 0x7F800000u) return (uint16_t)(u >> 16);
-    u += 0x7FFFu + ((u >> 16) & 1u);
-    return (uint16_t)(u >> 16);
-}
-
 uint16_t fp16_bits(float x) {  // round to nearest even, via the compiler's __half conversion on the host
     const __half h = __float2half_rn(x);
     uint16_t b;
     memcpy(&b, &h, 2);
     return b;
 }
+float fp16_value(float x) {
+    const __half h = __float2half_rn(x);
+    return __half2float(h);
+}
 
-int g_put_fmt = 1;  // 1 = bf16, 0 = fp16 (set by ann_bf16_create before packing)
-
-// element (row r, column c < 64) of a 128B-swizzled K-major 16-bit tile
+// element (row r, column c < 64) of a 128B-swizzled K-major fp16 tile
 inline void put(uint8_t* tile, int r, int c, float v) {
     const size_t off = (size_t)r * 128 + (size_t)((((c >> 3) ^ (r & 7)) << 4) + (c & 7) * 2);
-    const uint16_t b = g_put_fmt ? bf16_bits(v) : fp16_bits(v);
+    const uint16_t b = fp16_bits(v);
     memcpy(tile + off, &b, 2);
 }
 
@@ -823,13 +763,30 @@ df_status ann_bf16_create(df_ann* ann, const float* const* W, const float* const
     if (d2 % 32 || d2 < 64 || d2 > 800) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: dims[2] %% 32 == 0, 64..800 (got %d)", d2);
     if (d3 % 16 || d3 < 32 || d3 > 400) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: dims[3] %% 16 == 0, 32..400 (got %d)", d3);
 
+    // The contract of precision 1 (include/df_thermo.h): weights are bf16-valued and, like the biases, inside the
+    // fp16 range, because the tensor path holds them in fp16 (A21) -- exact for bf16 values in [2^-14, 65504], within
+    // 2^-25 absolute below that.  Anything else would be re-rounded silently (or become inf): refuse it.
+    for (int l = 0; l < 4; ++l) {
+        const size_t nw = (size_t)ann->dims[l] * ann->dims[l + 1];
+        for (size_t i = 0; i < nw; ++i) {
+            const float w = W[l][i];
+            uint32_t bits;
+            memcpy(&bits, &w, 4);
+            if (!(fabsf(w) <= 65504.0f))
+                return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: W[%d][%zu] = %g is outside the fp16 range the tensor path holds weights in", l, i, (double)w);
+            if (bits & 0xFFFFu)
+                return df_set_error(DF_ERR_INVALID_ARG, "bf16 path: W[%d][%zu] = %.9g is not bf16-valued (round the weights to bf16 first)", l, i, (double)w);
+        }
+        for (int i = 0; i < ann->dims[l + 1]; ++i)
+            if (!(fabsf(b[l][i]) <= 65504.0f))
+                return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: b[%d][%d] = %g is outside the fp16 range", l, i, (double)b[l][i]);
+    }
+
     Bf16Plan* P = new (std::nothrow) Bf16Plan;
     if (!P) return df_set_error(DF_ERR_ALLOC, "bf16 path: out of host memory");
     ann->bf16 = P;
     NetGeom& g = P->g;
     g.K = K;
-    g.b_fmt = 0;  // tcgen05 kind::f16 needs A and B in one format (fp16 x bf16 is an illegal instruction): fp16 x fp16
-    g_put_fmt = g.b_fmt;
     g.K0steps = (K + 4 <= 16) ? 1 : 2;  // features + 2 bias columns, fp16
     g.d1 = d1; g.d2 = d2; g.d3 = d3;
     g.NC = d1 / 32;
@@ -852,10 +809,6 @@ df_status ann_bf16_create(df_ann* ann, const float* const* W, const float* const
     g.smem_bytes = g.off_bar + B_COUNT * 8 + 16 + 1024;
     if (g.smem_bytes > 227 * 1024) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: layer widths need %d B of shared memory", g.smem_bytes);
 
-    int dev = 0;
-    DF_CUDA_TRY(cudaGetDevice(&dev));
-    DF_CUDA_TRY(cudaDeviceGetAttribute(&P->num_sms, cudaDevAttrMultiProcessorCount, dev));
-
     const int nquads = (g.NC + 3) / 4;
     const size_t sz_w1 = (size_t)nquads * kW1QuadBytes, sz_w2 = (size_t)2 * (g.NC + 1) * g.w2_tile_bytes,
                  sz_w3 = (size_t)(g.NKS + 1) * g.w3_tile_bytes, sz_w4 = (size_t)g.w4_bytes;
@@ -863,47 +816,24 @@ df_status ann_bf16_create(df_ann* ann, const float* const* W, const float* const
     const size_t o_w1 = 0, o_w2 = o_w1 + sz_w1, o_w3 = o_w2 + sz_w2, o_w4 = o_w3 + sz_w3, o_b = o_w4 + sz_w4;
     std::vector<uint8_t> blob(o_b + sz_b, 0);
     const int din = K + 2;
-    auto put_bias_w1 = [&](uint8_t* t, int r, int col0, float bv) {
-        const uint16_t hb = g.b_fmt ? bf16_bits(bv) : fp16_bits(bv);
-        float hf;
-        if (g.b_fmt) {
-            const uint32_t hu = (uint32_t)hb << 16;
-            memcpy(&hf, &hu, 4);
-        } else {
-            __half hh;
-            memcpy(&hh, &hb, 2);
-            hf = __half2float(hh);
-        }
+    // a bias rides in the accumulator as two weight columns (fp16 hi + lo parts) against the ones columns of A0
+    auto put_bias = [&](uint8_t* t, int r, int col0, float bv) {
+        const float hf = fp16_value(bv);
         put(t, r, col0 + din, hf);
         put(t, r, col0 + din + 1, bv - hf);
     };
     // W1: chunk c (32 outputs) sits in quad c/4 at rows 32*((c&3)>>1).., K columns 32*(c&1)..; columns K+2 and
-    // K+3 carry the bf16 hi and lo parts of b1 (the A0 tile holds 1.0 there).
+    // K+3 carry the fp16 hi and lo parts of b1 (the A0 tile holds 1.0 there).
     for (int c = 0; c < g.NC; ++c) {
         uint8_t* t = blob.data() + o_w1 + (size_t)(c >> 2) * kW1QuadBytes;
         const int r0 = ((c & 3) >> 1) * 32, k0 = (c & 1) * 32;
         for (int r = 0; r < 32; ++r) {
             const int o = c * 32 + r;
             for (int k = 0; k < din; ++k) put(t, r0 + r, k0 + k, W[0][(size_t)o * din + k]);
-            put_bias_w1(t, r0 + r, k0, b[0][o]);
+            put_bias(t, r0 + r, k0, b[0][o]);
         }
     }
     // bias tiles: zero except K rows din, din + 1 (the ones columns of A0) = hi / lo parts of the bias
-    auto put_bias = [&](uint8_t* t, int r, int col0, float bv) {
-        g_put_fmt = g.b_fmt;
-        const uint16_t hb = g.b_fmt ? bf16_bits(bv) : fp16_bits(bv);
-        float hf;
-        if (g.b_fmt) {
-            const uint32_t hu = (uint32_t)hb << 16;
-            memcpy(&hf, &hu, 4);
-        } else {
-            __half hh;
-            memcpy(&hh, &hb, 2);
-            hf = __half2float(hh);
-        }
-        put(t, r, col0 + din, hf);
-        put(t, r, col0 + din + 1, bv - hf);
-    };
     for (int h = 0; h < 2; ++h) {
         uint8_t* t = blob.data() + o_w2 + (size_t)(h * (g.NC + 1)) * g.w2_tile_bytes;
         for (int r = 0; r < g.na2; ++r) put_bias(t, r, 0, b[1][h * g.NH + r]);
@@ -954,7 +884,6 @@ df_status ann_bf16_create(df_ann* ann, const float* const* W, const float* const
     P->d.b2 = db + d1;
     P->d.b3 = db + d1 + d2;
     P->d.b4 = db + d1 + d2 + d3;
-    DF_CUDA_TRY(cudaFuncSetAttribute(ann_bf16_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, g.smem_bytes));
     return DF_OK;
 }
 
@@ -965,20 +894,27 @@ void ann_bf16_destroy(df_ann* ann) {
     ann->bf16 = nullptr;
 }
 
-static long long bf16_grid(const Bf16Plan* P, long long n) {
+// one CTA per SM of the device the call runs on (persistent kernel), fewer when there are fewer tiles
+static long long bf16_grid(long long n) {
     const long long tiles = (n + kTileM - 1) / kTileM;
-    return tiles < P->num_sms ? tiles : P->num_sms;
+    const int sms = df_device_sm_count();
+    return tiles < sms ? tiles : (sms > 0 ? sms : 1);
 }
 
 size_t ann_bf16_workspace(const df_ann* ann, long long n) {
-    const Bf16Plan* P = ann->bf16;
-    return (size_t)bf16_grid(P, n) * P->g.NKC * kChunkBytes;
+    return (size_t)bf16_grid(n) * ann->bf16->g.NKC * kChunkBytes;
 }
 
 df_status launch_ann_bf16(const df_ann* ann, const df_mech* mech, long long n, long long ld, const float* T,
                           const float* p, const float* Y, float* omega, float* dY, void* ws, size_t ws_bytes,
                           cudaStream_t s) {
     const Bf16Plan* P = ann->bf16;
+    const long long grid = bf16_grid(n);
+    if (ws_bytes < (size_t)grid * P->g.NKC * kChunkBytes)
+        return df_set_error(DF_ERR_INVALID_ARG, "df_chem_ann_source: workspace too small for this device");
+    static DfPerDevice smem_attr;   // the attribute is per device; every handle shape fits the fixed maximum
+    df_status st = df_ensure_dyn_smem((const void*)ann_bf16_kernel, 227 * 1024, &smem_attr);
+    if (st != DF_OK) return st;
     KArgs a;
     a.g = P->g;
     a.d = P->d;
@@ -989,23 +925,7 @@ df_status launch_ann_bf16(const df_ann* ann, const df_mech* mech, long long n, l
     a.T = T; a.p = p; a.Y = Y;
     a.omega = omega; a.dY = dY;
     a.scratch = static_cast<uint8_t*>(ws);
-    (void)ws_bytes;
-    ann_bf16_kernel<<<(unsigned)bf16_grid(P, n), kThreads, P->g.smem_bytes, s>>>(a, ann->norm);
+    ann_bf16_kernel<<<(unsigned)grid, kThreads, P->g.smem_bytes, s>>>(a, ann->norm);
     DF_CUDA_TRY(cudaGetLastError());
     return DF_OK;
 }
-
-
-#ifdef DF_DBG_CLK
-extern "C" __attribute__((visibility("default"))) int df_debug_read(long long* out) {
-    return (int)cudaMemcpyFromSymbol(out, g_dbg, sizeof(g_dbg));
-}
-#endif
-
-#ifdef DF_DBG_PROGRESS
-extern "C" __attribute__((visibility("default"))) int df_debug_set_progress(int* host_mapped) {
-    int* dptr = nullptr;
-    if (cudaHostGetDevicePointer((void**)&dptr, host_mapped, 0) != cudaSuccess) return -1;
-    return (int)cudaMemcpyToSymbol(g_prog, &dptr, sizeof(dptr));
-}
-#endif

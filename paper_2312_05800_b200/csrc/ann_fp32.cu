@@ -106,11 +106,9 @@ df_status launch_ann_fp32(const df_ann* ann, const df_mech* mech, long long n, l
         net.b[l] = ann->w32 + ann->b32_off[l];
     }
     const size_t smem = (size_t)2 * net.max_dim * kThreads * sizeof(float);
-    static bool attr_set = false;
-    if (!attr_set) {
-        DF_CUDA_TRY(cudaFuncSetAttribute(ann_fp32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_set = true;
-    }
+    static DfPerDevice smem_attr;
+    const df_status st = df_ensure_dyn_smem((const void*)ann_fp32_kernel, 200 * 1024, &smem_attr);
+    if (st != DF_OK) return st;
     const long long blocks = (n + kThreads - 1) / kThreads;
     if (blocks > 0x7fffffffLL) return df_set_error(DF_ERR_UNSUPPORTED, "df_chem_ann_source: n_cells too large");
     ann_fp32_kernel<<<(unsigned)blocks, kThreads, smem, s>>>(net, ann->norm, ann->K, mech->dev.invW, n, ld, T, p, Y,

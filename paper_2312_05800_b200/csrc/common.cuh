@@ -2,6 +2,7 @@
 // Product code: nothing here is used by, or uses, oracle/.
 #pragma once
 #include <cuda_runtime.h>
+#include <atomic>
 #include <cstdarg>
 #include <cstdint>
 #include <cstdio>
@@ -21,6 +22,15 @@ df_status df_set_error(df_status code, const char* fmt, ...);
             return df_set_error(DF_ERR_CUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), \
                                 __FILE__, __LINE__);                                              \
     } while (0)
+
+// ---- per-device launch prerequisites (runtime.cu) ------------------------------------------------
+// cudaFuncSetAttribute applies to the device that is current when it is called, so "done once" must be tracked per
+// device, not per process (a second GPU in the same process would otherwise launch without the attribute).
+struct DfPerDevice {
+    std::atomic<unsigned long long> done[2] = {{0ull}, {0ull}};   // one bit per device ordinal (up to 128)
+};
+df_status df_ensure_dyn_smem(const void* kernel, int bytes, DfPerDevice* state);
+int df_device_sm_count();   // multiprocessors of the current device (cached per device); 0 on error
 
 // ---- species tables, repacked at create time (mech.cu) ---------------------------------------
 // Thermo: h_k(T)/W_k = sum_{m<6} th[k][r][m] tau^m with tau = (T - T_mid) * inv_S, r = 0 (lo) / 1 (hi).

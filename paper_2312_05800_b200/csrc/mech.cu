@@ -9,19 +9,6 @@
 
 #include "common.cuh"
 
-static thread_local char g_err[512] = "";
-
-df_status df_set_error(df_status code, const char* fmt, ...) {
-    va_list ap;
-    va_start(ap, fmt);
-    vsnprintf(g_err, sizeof(g_err), fmt, ap);
-    va_end(ap);
-    return code;
-}
-
-extern "C" const char* df_last_error(void) { return g_err; }
-extern "C" int df_abi_version(void) { return 1; }
-
 namespace {
 
 // q(x) = p(c + s x): coefficients of the shifted/scaled polynomial, degree n-1.

@@ -256,11 +256,9 @@ df_status launch_properties_tiled(const df_mech* mech, long long n, long long ld
                                   const float* Y, float* cp, float* h, float* mu, float* lam, float* D, cudaStream_t s) {
     const MechDev& md = mech->dev;
     const size_t smem = (size_t)2 * md.Kp * kTT * sizeof(float2) + ((size_t)md.Kp * md.Kp + 1024) * sizeof(float);
-    static bool attr_set = false;
-    if (!attr_set) {
-        DF_CUDA_TRY(cudaFuncSetAttribute(props_tiled_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_set = true;
-    }
+    static DfPerDevice smem_attr;
+    const df_status st = df_ensure_dyn_smem((const void*)props_tiled_kernel, 200 * 1024, &smem_attr);
+    if (st != DF_OK) return st;
     const long long blocks = (n + 2 * kTT - 1) / (2 * kTT);
     if (blocks > 0x7fffffffLL) return df_set_error(DF_ERR_UNSUPPORTED, "df_thermo_properties: n_cells too large");
     props_tiled_kernel<<<(unsigned)blocks, kTT, smem, s>>>(md, n, ld, T, p, Y, cp, h, mu, lam, D);

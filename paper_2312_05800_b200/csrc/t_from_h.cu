@@ -337,9 +337,9 @@ df_status launch_fixed(const df_mech* mech, long long n, long long ld, const flo
                        int* n_unconv, cudaStream_t s) {
     const long long blocks = (n + kSCells - 1) / kSCells;
     if (blocks > 0x7fffffffLL) return df_set_error(DF_ERR_UNSUPPORTED, "df_thermo_T_from_h: n_cells too large");
-    static const cudaError_t attr = cudaFuncSetAttribute(t_from_h_sorted_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                         (int)sorted_smem_bytes<K>());
-    DF_CUDA_TRY(attr);
+    static DfPerDevice smem_attr;
+    const df_status st = df_ensure_dyn_smem((const void*)t_from_h_sorted_kernel<K>, (int)sorted_smem_bytes<K>(), &smem_attr);
+    if (st != DF_OK) return st;
     t_from_h_sorted_kernel<K><<<(unsigned)blocks, kThreads, sorted_smem_bytes<K>(), s>>>(mech->dev.sc, mech->dev.th32,
                                                                                          mech->dev.th64, n, ld, h, Y, T, cp, n_unconv);
     DF_CUDA_TRY(cudaGetLastError());

@@ -80,3 +80,43 @@ def mixed_err(got, ref, axis=-1):
     mixed = np.abs(d) / (np.abs(ref) + rms + 1e-300)
     norm = np.sqrt(np.sum(d * d, axis=axis)) / (np.sqrt(np.sum(ref * ref, axis=axis)) + 1e-300)
     return float(mixed.max()), float(norm.max())
+
+
+def mixed_err_table(got, ref):
+    """Per-species A12 figures of a [K, n] result: element-wise mixed maximum (with the cell it occurs at) and the
+    normwise error."""
+    got = np.asarray(got, np.float64)
+    ref = np.asarray(ref, np.float64)
+    d = got - ref
+    rms = np.sqrt(np.mean(ref * ref, axis=1, keepdims=True))
+    mixed = np.abs(d) / (np.abs(ref) + rms + 1e-300)
+    norm = np.sqrt(np.sum(d * d, axis=1)) / (np.sqrt(np.sum(ref * ref, axis=1)) + 1e-300)
+    worst = mixed.argmax(axis=1)
+    return [dict(k=int(k), mixed=float(mixed[k, worst[k]]), cell=int(worst[k]), normwise=float(norm[k]),
+                 p999=float(np.quantile(mixed[k], 0.999)), rms_ref=float(rms[k, 0]))
+            for k in range(got.shape[0])]
+
+
+def record(tag, payload):
+    """Append one JSON line of measured errors to gpurun_out/parity_measured.jsonl (the folder a GPU run brings
+    back); the summaries under profiles/ are copied from there.  Silent when the folder cannot be written."""
+    import json
+    import os
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    try:
+        os.makedirs(os.path.join(root, "gpurun_out"), exist_ok=True)
+        with open(os.path.join(root, "gpurun_out", "parity_measured.jsonl"), "a") as f:
+            f.write(json.dumps(dict(tag=tag, **payload)) + "\n")
+    except OSError:
+        pass
+
+
+FLOOR_FACTOR = 1.25
+
+
+def bounds_16bit(ref, ideal, tol=2e-2):
+    """Per-species element-wise (mixed-form) bound on the 16-bit tensor path: north_star's 2e-2, or, for a species
+    whose exactly rounded fp16 chain (tests/ideal16.py) already exceeds 0.8 x that, 1.25 x that floor (A12).
+    Returns (bounds[K], floor_table)."""
+    floor = mixed_err_table(ideal, ref)
+    return np.array([max(tol, FLOOR_FACTOR * t["mixed"]) for t in floor]), floor

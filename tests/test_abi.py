@@ -37,7 +37,7 @@ def test_library_exports_every_declared_symbol(lib_path):
 def test_binding_symbol_list_matches_header(lib_path):
     from paper_2312_05800_b200 import binding
     assert sorted(binding.SYMBOLS) == declared_symbols()
-    assert binding.abi_version() == 1
+    assert binding.abi_version() == 2
 
 
 def test_no_cpu_fallback(lib_path):

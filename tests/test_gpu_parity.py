@@ -198,9 +198,9 @@ def test_properties_subset_outputs(B):
 # --------------------------------------------------------------------------------------------
 # H3: ANN source, fp32 path
 # --------------------------------------------------------------------------------------------
-def check_source(B, mech, ann, cells, n, tol, sample=None, tol_mixed=None):
-    """tol bounds the per-species normwise error; tol_mixed (default: tol) the element-wise mixed form (A12)."""
-    tol_mixed = tol if tol_mixed is None else tol_mixed
+def check_source(B, mech, ann, cells, n, tol, sample=None, tag=None):
+    """tol bounds both A12 forms per species: the element-wise mixed error and the normwise error.  The measured
+    figures are recorded (gpurun_out/parity_measured.jsonl) whether the test passes or not."""
     from oracle import oracle
     gm, ga = B.Mech(mech), B.Ann(ann)
     K, ld = cells.Y.shape
@@ -213,19 +213,35 @@ def check_source(B, mech, ann, cells, n, tol, sample=None, tol_mixed=None):
     om_g, dY_g = om_g.cpu().numpy(), dY_g.cpu().numpy()
     # sum_k (Y_k + dY_k) = 1 on every cell (A11 / P:86)
     s = (cells.Y[:, :n].astype(np.float64) + dY_g[:, :n]).sum(axis=0)
-    assert np.abs(s - 1.0).max() <= 2e-6, np.abs(s - 1.0).max()
+    sum_err = float(np.abs(s - 1.0).max())
     idx = np.arange(n) if sample is None else sample
     o_mech, o_ann = oracle.Mech(mech), oracle.Ann(ann)
     om_r, dY_r = o_ann.source(o_mech, cells.T[idx], cells.p[idx], np.ascontiguousarray(cells.Y[:, idx]))
+    ideal = None
+    if ann.precision == 1:   # the floor an exactly rounded fp16 chain has on these cells (tests/ideal16.py, A12)
+        from tests import ideal16
+        ideal = dict(zip(("omega", "dY"), ideal16.ideal_chain_source(mech, ann, cells.T[idx], cells.p[idx],
+                                                                      np.ascontiguousarray(cells.Y[:, idx]), "fp16")))
+    failures = []
     for name, got, ref in (("dY", dY_g[:, idx], dY_r), ("omega", om_g[:, idx], om_r)):
-        mixed, norm = helpers.mixed_err(got, ref[:, :len(idx)])
-        assert mixed <= tol_mixed and norm <= tol, f"{name}: mixed {mixed:.3e} normwise {norm:.3e} (tol {tol_mixed}/{tol})"
+        ref = ref[:, :len(idx)]
+        table = helpers.mixed_err_table(got, ref)
+        bound, floor = (np.full(K, tol), None) if ideal is None else helpers.bounds_16bit(ref, ideal[name], tol)
+        helpers.record(tag or "check_source", dict(quantity=name, dims=list(ann.dims), precision=int(ann.precision), n=int(n),
+                                                   cells_compared=int(len(idx)), sum_to_one=sum_err, tol=tol,
+                                                   per_species=table, ideal_fp16_chain=floor))
+        for t in table:
+            if t["mixed"] > bound[t["k"]] or t["normwise"] > tol:
+                failures.append(f"{name}[k={t['k']}]: mixed {t['mixed']:.3e} (bound {bound[t['k']]:.3e}) normwise "
+                                f"{t['normwise']:.3e} (bound {tol})")
+    assert sum_err <= 1e-6, sum_err
+    assert not failures, "; ".join(failures)
     return dY_g, om_g
 
 
 def test_ann_source_fp32_cfg1(B):
     mech, ann, cells, _ = make_case(1, 4096)
-    check_source(B, mech, ann, cells, 4096, 1e-5)
+    check_source(B, mech, ann, cells, 4096, 1e-5, tag="fp32_cfg1")
 
 
 def test_ann_source_fp32_ragged_and_degenerate(B):
@@ -233,7 +249,7 @@ def test_ann_source_fp32_ragged_and_degenerate(B):
     mech, ann, cells, _ = make_case(1, 1003, 1004)
     cells.Y[:, :8] = 0.0
     cells.Y[np.arange(8), np.arange(8)] = 1.0   # one-hot cells: Y_k = 0 branch of the inverse transform
-    check_source(B, mech, ann, cells, 1003, 1e-5)
+    check_source(B, mech, ann, cells, 1003, 1e-5, tag="fp32_ragged_degenerate")
 
 
 def test_ann_K_mismatch(B):
@@ -249,11 +265,8 @@ def test_ann_K_mismatch(B):
 # --------------------------------------------------------------------------------------------
 # H3: ANN source, bf16 / tcgen05 path (tolerance 2e-2, A12)
 # --------------------------------------------------------------------------------------------
-# north_star: "2e-2 relative on the bf16 path".  DESIGN.md A12: the error of a bf16-operand chain is rounding
-# noise, so "relative" is read per species in the norm sense (||d_k||/||ref_k|| <= 2e-2); a single element is
-# then bounded by the tail of that noise, sqrt(2 ln N) ~ 5 sigma for N ~ 1e5..1e6 samples -> 1e-1 of
-# (|ref| + RMS_k).
-BF16_MIXED = 1e-1
+# north_star: "2e-2 relative on the bf16 path"; A12 reads it per species both element-wise, as
+# |d| <= 2e-2 (|ref| + RMS_cells(ref_k)), and normwise.  Both at 2e-2; the measured figures are recorded.
 @pytest.mark.parametrize("hidden,n,ld", [([128, 64, 32], 1000, 1000), ([64, 64, 48], 131, 132), ([192, 96, 80], 700, 704)])
 def test_ann_source_bf16_small_nets(B, hidden, n, ld):
     """Small layer widths exercise the chunk/piece bookkeeping of the chain at sizes the oracle does in full."""
@@ -261,14 +274,14 @@ def test_ann_source_bf16_small_nets(B, hidden, n, ld):
     mech = synth.make_mechanism(19, synth.config_seed(2))
     ann = synth.make_ann(19, hidden, 1, synth.config_seed(2))
     cells = synth.cells_stratified(19, n, synth.config_seed(2), ld=ld)
-    check_source(B, mech, ann, cells, n, 2e-2, tol_mixed=BF16_MIXED)
+    check_source(B, mech, ann, cells, n, 2e-2, tag=f"bf16_small_{hidden[0]}_{hidden[1]}_{hidden[2]}")
 
 
 @pytest.mark.parametrize("n", [128, 2077])
 def test_ann_source_bf16_paper_net(B, n):
     """21 -> 1600 -> 800 -> 400 -> 19, every cell against the oracle; 2077 = 16 tiles + ragged tail."""
     mech, ann, cells, _ = make_case(2, n, (n + 3) // 4 * 4)
-    check_source(B, mech, ann, cells, n, 2e-2, tol_mixed=BF16_MIXED)
+    check_source(B, mech, ann, cells, n, 2e-2, tag=f"bf16_paper_net_n{n}")
 
 
 def test_ann_source_bf16_multi_tile_per_cta(B):
@@ -276,7 +289,48 @@ def test_ann_source_bf16_multi_tile_per_cta(B):
     n = 148 * 128 * 2 + 77
     mech, ann, cells, _ = make_case(2, n, (n + 3) // 4 * 4)
     sample = np.unique(np.concatenate([np.arange(0, n, 97), np.arange(n - 130, n)]))
-    check_source(B, mech, ann, cells, n, 2e-2, sample=sample, tol_mixed=BF16_MIXED)
+    check_source(B, mech, ann, cells, n, 2e-2, sample=sample, tag="bf16_paper_net_multi_tile")
+
+
+def test_ann_create_precision1_contract(B):
+    """include/df_thermo.h: precision 1 takes bf16-valued weights inside the fp16 range (the tensor path holds them
+    in fp16, A21); anything else is refused instead of being re-rounded silently."""
+    from paper_2312_05800_b200 import synth
+    ann = synth.make_ann(19, [64, 64, 32], 1, 5)
+    B.Ann(ann)                                   # the generator's bf16-rounded weights are accepted
+    ann.W[1][3, 5] = np.float32(7.0e4)           # bf16-valued, but above 65504
+    with pytest.raises(B.DfError) as e:
+        B.Ann(ann)
+    assert e.value.code == B.DF_ERR_UNSUPPORTED
+    ann.W[1][3, 5] = np.float32(0.1)             # 0.1 is not bf16-representable
+    with pytest.raises(B.DfError) as e:
+        B.Ann(ann)
+    assert e.value.code == B.DF_ERR_INVALID_ARG
+    ann.W[1][3, 5] = np.float32(0.125)
+    ann.b[2][0] = np.float32(np.inf)
+    with pytest.raises(B.DfError) as e:
+        B.Ann(ann)
+    assert e.value.code == B.DF_ERR_UNSUPPORTED
+
+
+def test_ann_two_live_handles_of_different_shapes(B):
+    """Creating a small net after a large one must not break launches of the large one (the dynamic shared-memory
+    attribute of the kernel is per device and fixed, not per handle)."""
+    from paper_2312_05800_b200 import synth
+    seed = synth.config_seed(2)
+    mech = synth.make_mechanism(19, seed)
+    big, small = synth.make_ann(19, [1600, 800, 400], 1, seed), synth.make_ann(19, [64, 64, 32], 1, seed)
+    cells = synth.cells_stratified(19, 300, seed)
+    gm, gb = B.Mech(mech), B.Ann(big)
+    gs = B.Ann(small)
+    T, p, Y = dev(cells.T), dev(cells.p), dev(cells.Y)
+    o1, o2, o3 = (torch.zeros(19, 300, device="cuda") for _ in range(3))
+    B.df_chem_ann_source(gb, gm, T, p, Y, omega=o1, workspace=B.alloc_workspace(gb, 300))
+    B.df_chem_ann_source(gs, gm, T, p, Y, omega=o2, workspace=B.alloc_workspace(gs, 300))
+    B.df_chem_ann_source(gb, gm, T, p, Y, omega=o3, workspace=B.alloc_workspace(gb, 300))
+    torch.cuda.synchronize()
+    assert float((o1 - o3).abs().max()) <= 1e-3 * float(o1.abs().max())
+    assert float(o2.abs().max()) > 0
 
 
 # --------------------------------------------------------------------------------------------
