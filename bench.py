@@ -3,9 +3,14 @@
 
 A "step" is one pass of the whole hot path over one batch of synthetic cells:
 df_thermo_T_from_h -> df_thermo_properties -> df_chem_ann_source (bf16 21-1600-800-400-19 MLP)
-on BASELINE.json configs[2] (the headline: 2,097,152 cells, K = 19), through the C ABI.
+on BASELINE.json configs[2] (the headline: 2,097,152 cells, K = 19), through the C ABI.  The same line carries
+  kernels   one roofline entry per kernel of that step (T_from_h: hbm, properties: alu, ann_bf16: tensor),
+  fp32_peak the FFMA-chain peak measured in this run (df_probe_fp32_peak), next to the nominal figure,
+  configs   short timed runs of the other BASELINE configs (1, 2, 4, 5) with their own roofline fractions,
+  e2e       the step through df_step_host with pinned HOST buffers,
+  cpu_baseline  the fp64 oracle on the host cores (bounded sample).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--cells n] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--cells n] [--impl reference] [--no-configs]
 
 N > 1: launched by torchrun, one rank per GPU, every rank runs the same per-GPU workload on its
 own cells (weak scaling; the path has no exchange step, so there is no collective in the data
@@ -31,6 +36,13 @@ UNIT = "cells/s"
 CFG = 3                      # BASELINE.json configs[2] (1-based numbering in synth.CONFIGS)
 FLOPS_PER_CELL_MLP = 3282400  # 2 * (21*1600 + 1600*800 + 800*400 + 400*19)
 HIDDEN = [1600, 800, 400]
+FP32_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x FP32 lanes x 2 (FMA) x clocks.max.sm = 74.45
+
+
+def props_flops(K: int) -> float:
+    """minimum-formulation flops per cell of the property pass, F(K) = 12.5 K^2 + 51.5 K + 10."""
+    return 12.5 * K * K + 51.5 * K + 10.0
+
 
 
 def peaks():
@@ -101,6 +113,48 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+
+
+# ---- DRAM traffic per launch from the committed ncu export -------------------------------------
+NCU_RAW = os.path.join(ROOT, "profiles", "r2_ncu_raw.csv")   # `ncu -i ... --page raw --csv`, see profiles/r2_summary.md
+_UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+
+
+def ncu_traffic(kernel_substr: str, grid_x=None):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the captured launch of `kernel_substr` whose grid is grid_x
+    blocks (None: its largest captured grid), read from the committed ncu raw-page export (wide CSV: a header row, a
+    units row, one row per launch).  None when the export or the launch is not there."""
+    import csv
+    if not os.path.exists(NCU_RAW):
+        return None
+    with open(NCU_RAW, newline="") as f:
+        rows = [r for r in csv.reader(f) if r]
+    hdr = next((i for i, r in enumerate(rows) if "Kernel Name" in r), None)
+    if hdr is None or hdr + 1 >= len(rows):
+        return None
+    names, units = rows[hdr], rows[hdr + 1]
+    try:
+        ck, cg = names.index("Kernel Name"), names.index("Grid Size")
+        cr, cw = names.index("dram__bytes_read.sum"), names.index("dram__bytes_write.sum")
+    except ValueError:
+        return None
+    best = None
+    for r in rows[hdr + 2:]:
+        if len(r) <= max(ck, cg, cr, cw) or kernel_substr not in r[ck]:
+            continue
+        try:
+            gx = int(r[cg].strip("() ").split(",")[0])
+            val = (float(r[cr].replace(",", "")) * _UNIT.get(units[cr], 1.0)
+                   + float(r[cw].replace(",", "")) * _UNIT.get(units[cw], 1.0))
+        except ValueError:
+            continue
+        if grid_x is not None and gx == grid_x:
+            return val
+        if grid_x is None and (best is None or gx > best[0]):
+            best = (gx, val)
+    return best[1] if best else None
+
+
 def make_inputs(n: int, rank: int):
     """Seeded synthetic cfg3 fields (DESIGN.md input recipe); rank shifts the cell seed only."""
     from paper_2312_05800_b200 import synth
@@ -111,30 +165,47 @@ def make_inputs(n: int, rank: int):
     return mech, ann, cells
 
 
-def run_reference(args):
-    """The oracle (as it stands) timed on the host cores on a bounded sample of the same workload."""
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
-        return
+def cpu_model() -> str:
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def _oracle_step(om, oa, cells, h32):
+    T32 = om.T_from_h(h32, cells.Y, cells.T_guess).astype(np.float32)
+    om.properties(T32, cells.p, cells.Y)
+    oa.source(om, T32, cells.p, cells.Y)
+
+
+def _oracle_setup(ns):
+    """The oracle as it stands (oracle/oracle.cpp, never tuned), compiled for THIS host: g++ -O3 -march=native
+    -ffp-contract=off (the tests use the portable -O2 build of the same source)."""
     from oracle import oracle
-    # bounded sample per step: about 2e6 cell-updates in total (~2 minutes on 16 cores), never above --ref-cells
-    ns = max(4096, min(args.ref_cells, int(2.0e6 / max(1, args.steps + args.warmup))))
+    oracle.use_native_build()
     mech, ann, cells = make_inputs(ns, 0)
     om, oa = oracle.Mech(mech), oracle.Ann(ann)
     _, h = om.mixture_cp_h(cells.T, cells.Y)
-    h32 = h.astype(np.float32)
+    return oracle, om, oa, cells, h.astype(np.float32)
 
-    def step():
-        T = om.T_from_h(h32, cells.Y, cells.T_guess)
-        T32 = T.astype(np.float32)
-        om.properties(T32, cells.p, cells.Y)
-        oa.source(om, T32, cells.p, cells.Y)
 
+def run_reference(args):
+    """The oracle timed on the host cores on a bounded sample of the same workload (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    # bounded sample per step: about 2e6 cell-updates in total (~2 minutes on 16 cores), never above --ref-cells
+    ns = max(4096, min(args.ref_cells, int(2.0e6 / max(1, args.steps + args.warmup))))
+    oracle, om, oa, cells, h32 = _oracle_setup(ns)
     for _ in range(args.warmup):
-        step()
+        _oracle_step(om, oa, cells, h32)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        step()
+        _oracle_step(om, oa, cells, h32)
     dt = (time.perf_counter() - t0) / args.steps
     val = ns / dt
     cores = oracle.get_threads()
@@ -144,7 +215,8 @@ def run_reference(args):
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"configs[2] sample: {ns} of 2097152 cells, K=19, T_from_h+properties+MLP 21-1600-800-400-19"},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
-                         "sample": f"{ns} cells per step (the full config is 2097152)"},
+                         "sample": f"{ns} cells per step (the full config is 2097152)",
+                         "build": oracle.build_flags(), "cpu": cpu_model()},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
@@ -166,19 +238,168 @@ def aggregate_value(world: int, cells_per_gpu: int, ms_per_step: float) -> float
 
 
 def cpu_baseline(ns: int):
-    """cpu_baseline leg: the fp64 oracle on a bounded sample, all host cores (rank 0, N = 1 only)."""
-    from oracle import oracle
-    mech, ann, cells = make_inputs(ns, 0)
-    om, oa = oracle.Mech(mech), oracle.Ann(ann)
-    _, h = om.mixture_cp_h(cells.T, cells.Y)
-    h32 = h.astype(np.float32)
+    """cpu_baseline leg: the fp64 oracle on a bounded sample of the workload, all host cores, plus the same on one
+    thread over a sixteenth of the sample (rank 0, N = 1 only)."""
+    oracle, om, oa, cells, h32 = _oracle_setup(ns)
+    cores = oracle.get_threads()
     t0 = time.perf_counter()
-    T32 = om.T_from_h(h32, cells.Y, cells.T_guess).astype(np.float32)
-    om.properties(T32, cells.p, cells.Y)
-    oa.source(om, T32, cells.p, cells.Y)
+    _oracle_step(om, oa, cells, h32)
     dt = time.perf_counter() - t0
-    return {"value": ns / dt, "unit": UNIT, "cores": oracle.get_threads(), "kind": "oracle",
-            "sample": f"first {ns} cells of the workload, one pass, {dt:.1f} s"}
+    n1 = max(1024, ns // 16)
+    from paper_2312_05800_b200 import synth
+    sub = synth.Cells(n1, cells.T[:n1], cells.p[:n1], np.ascontiguousarray(cells.Y[:, :n1]), cells.T_guess[:n1])
+    oracle.set_threads(1)
+    t0 = time.perf_counter()
+    _oracle_step(om, oa, sub, h32[:n1])
+    dt1 = time.perf_counter() - t0
+    oracle.set_threads(cores)
+    return {"value": ns / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {ns} cells of the workload, one pass, {dt:.1f} s",
+            "one_thread": {"value": n1 / dt1, "unit": UNIT, "sample": f"first {n1} cells, one pass, {dt1:.1f} s"},
+            "build": oracle.build_flags(), "cpu": cpu_model()}
+
+
+# ---- GPU legs ---------------------------------------------------------------------------------------
+def _median_launch_ms(torch, stream, launch, reps, before=None, warm=3):
+    """Median and minimum CUDA-event time of `launch`, each launch bracketed by its own pair of events on the
+    launching stream; `before` (untimed) restores in/out arguments, e.g. the Newton guess."""
+    ts = []
+    for i in range(warm + reps):
+        if before is not None:
+            before(i)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        launch(i)
+        b.record(stream)
+        torch.cuda.synchronize()
+        if i >= warm:
+            ts.append(a.elapsed_time(b))
+    return float(np.median(ts)), float(np.min(ts))
+
+
+def measure_fp32_peak(torch, B, stream):
+    """FFMA-chain peak of this board, now: scalar FFMA and packed FFMA2 variants."""
+    out = {}
+    blocks, iters = 148 * 16, 8192
+    for name, variant in (("ffma", 0), ("ffma2", 1)):
+        flops = [0.0]
+
+        def launch(_i):
+            flops[0] = B.df_probe_fp32_peak(variant, blocks, iters)
+        med, mn = _median_launch_ms(torch, stream, launch, reps=5, warm=2)
+        out[name] = flops[0] / (mn * 1e-3) / 1e12
+    out["measured"] = max(out["ffma"], out["ffma2"])
+    out["nominal"] = FP32_NOMINAL_TFLOPS
+    out["unit"] = "TFLOP/s"
+    out["how"] = ("df_probe_fp32_peak: 148 x 16 blocks x 256 threads, 16 register-only dependent FMA chains per thread "
+                  "x 8192 iterations, best of 5 (CUDA events); nominal = 148 SM x 128 lanes x 2 x 1.965 GHz")
+    return out
+
+
+def alu_entry(kernel, flops_per_cell, n, ms, fp32, extra=None):
+    ach = flops_per_cell * n / (ms * 1e-3) / 1e12
+    e = {"kernel": kernel, "bound": "alu", "achieved": ach, "peak": fp32["measured"], "unit": "TFLOP/s",
+         "frac": ach / fp32["measured"], "frac_vs_nominal": ach / fp32["nominal"], "ms": ms,
+         "peak_source": "FP32 FMA peak measured in this run (fp32_peak.measured)",
+         "algorithmic": f"{flops_per_cell:.0f} flop/cell x {n} cells/launch"}
+    e.update(extra or {})
+    return e
+
+
+def hbm_entry(kernel, bytes_per_cell, n, ms, pk, extra=None):
+    ach = bytes_per_cell * n / (ms * 1e-3) / 1e9
+    e = {"kernel": kernel, "bound": "hbm", "achieved": ach, "peak": pk["hbm"], "unit": "GB/s", "frac": ach / pk["hbm"],
+         "ms": ms, "peak_source": f"{pk['src']} HBM copy bandwidth",
+         "algorithmic": f"{bytes_per_cell} B/cell x {n} cells/launch"}
+    e.update(extra or {})
+    return e
+
+
+def bench_configs(torch, B, stream, pk, fp32, quick=False):
+    """Short timed runs of BASELINE configs 1, 2, 4, 5 (the headline is configs[2] = cfg3)."""
+    from paper_2312_05800_b200 import synth
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    out = {}
+
+    # ---- cfg1: 4096 cells, K = 9, fp32 MLP 11-64-64-9: launch-latency bound, reported in microseconds per call ----
+    mech, ann, cells = synth.make_config(1)
+    gm, ga = B.Mech(mech), B.Ann(ann)
+    n, K = cells.n, mech.K
+    T0, p, Y, Tg = dev(cells.T), dev(cells.p), dev(cells.Y), dev(cells.T_guess)
+    h = torch.empty(n, device="cuda")
+    B.df_thermo_properties(gm, T0, p, Y, h=h)
+    T, cp, mu, lam = (torch.empty(n, device="cuda") for _ in range(4))
+    D, om = torch.empty(K, n, device="cuda"), torch.empty(K, n, device="cuda")
+    t1, _ = _median_launch_ms(torch, stream, lambda i: B.df_thermo_T_from_h(gm, h, Y, T), 20, before=lambda i: T.copy_(Tg))
+    t2, _ = _median_launch_ms(torch, stream, lambda i: B.df_thermo_properties(gm, T, p, Y, cp=cp, mu=mu, lam=lam, D=D), 20)
+    t3, _ = _median_launch_ms(torch, stream, lambda i: B.df_chem_ann_source(ga, gm, T, p, Y, omega=om), 20)
+    out["cfg1"] = {"workload": "configs[0]: 4096 cells, K=9, T_from_h + properties + fp32 MLP 11-64-64-9",
+                   "us_per_call": {"T_from_h": 1e3 * t1, "properties": 1e3 * t2, "ann_fp32": 1e3 * t3},
+                   "cells_per_s": n / ((t1 + t2 + t3) * 1e-3), "note": "launch-latency bound (problem < 1 MB): no roofline fraction"}
+    del gm, ga
+
+    # ---- cfg2: 262,144 cells, K = 19, the tensor-path MLP alone; 6 rotating buffer sets (the 42 MB of one set would
+    # sit in the 126 MB L2) ----
+    mech, ann, cells = synth.make_config(2)
+    gm, ga = B.Mech(mech), B.Ann(ann)
+    n, K = cells.n, mech.K
+    sets = []
+    for s_ in range(6):
+        sets.append((dev(np.roll(cells.T, 4096 * s_)), dev(cells.p), dev(np.roll(cells.Y, 4096 * s_, axis=1)),
+                     torch.empty(K, n, device="cuda")))
+    ws = B.alloc_workspace(ga, n)
+
+    def ann_launch(i):
+        T_, p_, Y_, o_ = sets[i % len(sets)]
+        B.df_chem_ann_source(ga, gm, T_, p_, Y_, omega=o_, workspace=ws)
+    med, mn = _median_launch_ms(torch, stream, ann_launch, 12)
+    ach = FLOPS_PER_CELL_MLP * n / (med * 1e-3) / 1e12
+    out["cfg2"] = {"workload": "configs[1]: 262144 cells, K=19, bf16 MLP 21-1600-800-400-19 alone, 6 rotating buffer sets",
+                   "ms": med, "ms_min": mn, "cells_per_s": n / (med * 1e-3),
+                   "roofline": {"kernel": "ann_bf16_kernel", "bound": "tensor", "achieved": ach, "peak": pk["bf16"], "unit": "TFLOP/s",
+                                "frac": ach / pk["bf16"], "peak_source": f"{pk['src']} bf16 burst (kernel timed alone)",
+                                "algorithmic": f"{FLOPS_PER_CELL_MLP} flop/cell x {n} cells/launch",
+                                "note": "2048 tiles over 148 CTAs = 13.8 waves: 1 - 13.84/14 = 1.1 % tail"}}
+    del gm, ga, sets, ws
+    torch.cuda.empty_cache()
+
+    # ---- cfg4: 2,097,152 cells, K = 53, property pass only ----
+    mech, _, cells = synth.make_config(4)
+    gm = B.Mech(mech)
+    n, K = cells.n, mech.K
+    T0, p, Y = dev(cells.T), dev(cells.p), dev(cells.Y)
+    cp, hh, mu, lam = (torch.empty(n, device="cuda") for _ in range(4))
+    D = torch.empty(K, n, device="cuda")
+    med, mn = _median_launch_ms(torch, stream, lambda i: B.df_thermo_properties(gm, T0, p, Y, cp=cp, h=hh, mu=mu, lam=lam, D=D),
+                                3 if quick else 8)
+    out["cfg4"] = {"workload": "configs[3]: 2097152 cells, K=53, properties (cp, h, mu, lambda, D[53])", "ms": med, "ms_min": mn,
+                   "cells_per_s": n / (med * 1e-3),
+                   "roofline": alu_entry("props_kernel (K=53)", props_flops(K), n, med, fp32,
+                                         {"hbm_bytes_per_cell": 4 * (2 * K + 6), "traffic": ncu_traffic("props_tiled")})}
+    del gm, T0, p, Y, cp, hh, mu, lam, D
+    torch.cuda.empty_cache()
+
+    # ---- cfg5: 16,777,216 cells, K = 19, T_from_h (+ cp at the root) on the robustness field, warm and cold guess ----
+    mech, _, cells = synth.make_config(5, n=(1 << 21) if quick else None)
+    gm = B.Mech(mech)
+    n, K = cells.n, mech.K
+    Y = dev(cells.Y)
+    h = torch.empty(n, device="cuda")
+    B.df_thermo_properties(gm, dev(cells.T), None, Y, h=h)
+    warm, cold = dev(cells.T_guess), torch.full((n,), 1000.0, device="cuda")
+    T, cp = torch.empty(n, device="cuda"), torch.empty(n, device="cuda")
+    cnt = torch.zeros(1, dtype=torch.int32, device="cuda")
+    res = {}
+    for name, g in (("warm", warm), ("cold", cold)):
+        med, mn = _median_launch_ms(torch, stream, lambda i: B.df_thermo_T_from_h(gm, h, Y, T, cp=cp, n_unconverged=cnt), 8,
+                                    before=lambda i, g=g: T.copy_(g))
+        res[name] = hbm_entry("t_from_h kernel (K=19)", 4 * (K + 2) + 8, n, med, pk,
+                              {"ms_min": mn, "cells_per_s": n / (med * 1e-3),
+                               "max_abs_T_error_vs_drawn_K": float((T - dev(cells.T)).abs().max())})
+    out["cfg5"] = {"workload": f"configs[4]: {n} cells, K=19, robustness field (T 250-3500 K, near-pure and 1e-20-trace cells), "
+                               "df_thermo_T_from_h with cp written: 4(K+2) B in + T + cp out = 92 B/cell",
+                   "unconverged": int(cnt.item()), "warm": res["warm"], "cold": res["cold"]}
+    return out
 
 
 def run_gpu(args):
@@ -249,23 +470,18 @@ def run_gpu(args):
     value = aggregate_value(world, n, ms_step)
     k_ms = [float(np.mean([e[i].elapsed_time(e[i + 1]) for e in marks])) for i in range(3)]
 
-    # ---- optional: each kernel timed alone (its own launches back to back, the board not power-limited by the MLP) ----
-    alone_ms = None
-    if args.kernels_alone:
-        def alone(launch, reps=12):
-            ts = []
-            for _ in range(reps):
-                dT.copy_(dTg)
-                a, b = ev(), ev()
-                a.record(stream); launch(); b.record(stream)
-                torch.cuda.synchronize()
-                ts.append(a.elapsed_time(b))
-            return float(np.median(ts[2:]))
-        time.sleep(2.0)
-        alone_ms = {"T_from_h": alone(lambda: B.df_thermo_T_from_h(gm, dh, dY, dT))}
-        B.df_thermo_T_from_h(gm, dh, dY, dT)
-        alone_ms["properties"] = alone(lambda: B.df_thermo_properties(gm, dT0, dp, dY, cp=cp, mu=mu, lam=lam, D=D))
-        alone_ms["ann_bf16"] = alone(lambda: B.df_chem_ann_source(ga, gm, dT0, dp, dY, omega=om, workspace=ws), reps=5)
+    # ---- each kernel of the step timed alone (its own launches back to back, the board not power-limited by the MLP) ----
+    time.sleep(1.0)
+    alone_ms = {}
+    alone_ms["T_from_h"], _ = _median_launch_ms(torch, stream, lambda i: B.df_thermo_T_from_h(gm, dh, dY, dT), 10,
+                                                before=lambda i: dT.copy_(dTg))
+    alone_ms["properties"], _ = _median_launch_ms(torch, stream,
+                                                  lambda i: B.df_thermo_properties(gm, dT, dp, dY, cp=cp, mu=mu, lam=lam, D=D), 10)
+    alone_ms["ann_bf16"], _ = _median_launch_ms(torch, stream,
+                                                lambda i: B.df_chem_ann_source(ga, gm, dT, dp, dY, omega=om, workspace=ws), 4, warm=1)
+
+    pk = peaks()
+    fp32 = measure_fp32_peak(torch, B, stream) if rank == 0 else None
 
     # ---- e2e: the same step through df_step_host with pinned HOST buffers ----
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -289,7 +505,8 @@ def run_gpu(args):
         if dist is not None:
             dist.destroy_process_group()
         return
-    pk = peaks()
+    ctx.close()
+    del ctx, hh, hp, hg, hY, oT, ocp, omu, olam, oD, oom
     achieved = FLOPS_PER_CELL_MLP * n / (k_ms[2] * 1e-3) / 1e12
     clocks = clk.summary(w0, w1)
     # B200_PROFILING.md: burst peak for a kernel timed alone, sustained peak for one timed inside a long step; the
@@ -299,6 +516,29 @@ def run_gpu(args):
     peak = pk["bf16_sust"] if capped else pk["bf16"]
     why = "power-limited clocks in the timed region: " + (", ".join(clocks["reasons"]) or "SM clock below 95 % of max")
     peak_src = f"{pk['src']} bf16 {'sustained (' + why + ')' if capped else 'burst'}"
+    blocks256 = (n + 255) // 256
+    ann_roof = {"bound": "tensor", "kernel": "ann_bf16_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                "frac": achieved / peak,
+                # dram__bytes_read.sum + dram__bytes_write.sum of one launch at this size, from the committed ncu export
+                "traffic": ncu_traffic("ann_bf16_kernel", min(148, (n + 127) // 128)) if n == 2097152 else None,
+                "peak_source": peak_src, "frac_vs_burst": achieved / pk["bf16"],
+                "frac_vs_sustained": achieved / pk["bf16_sust"],
+                "algorithmic": f"{FLOPS_PER_CELL_MLP} flop/cell x {n} cells/launch"}
+    a_alone = FLOPS_PER_CELL_MLP * n / (alone_ms["ann_bf16"] * 1e-3) / 1e12
+    kernels = {
+        # bytes the timed call really moves: h, T guess, Y[19] in; T out (no cp requested in the step)
+        "t_from_h": hbm_entry("t_from_h kernel (K=19)", 4 * (K + 2) + 4, n, k_ms[0], pk,
+                              {"ms_alone": alone_ms["T_from_h"],
+                               "frac_alone": (4 * (K + 2) + 4) * n / (alone_ms["T_from_h"] * 1e-3) / 1e9 / pk["hbm"],
+                               "traffic": ncu_traffic("t_from_h", blocks256) if n == 2097152 else None,
+                               "note": "2.1 M cells: 184.5 MB per launch; configs.cfg5 has the 16.8 M-cell figure"}),
+        "properties": alu_entry("props kernel (K=19)", props_flops(K), n, k_ms[1], fp32,
+                                {"ms_alone": alone_ms["properties"],
+                                 "frac_alone": props_flops(K) * n / (alone_ms["properties"] * 1e-3) / 1e12 / fp32["measured"],
+                                 "hbm_bytes_per_cell": 4 * (2 * K + 6),
+                                 "traffic": ncu_traffic("props_fixed", None) if n == 2097152 else None}),
+        "ann_bf16": dict(ann_roof, ms=k_ms[2], ms_alone=alone_ms["ann_bf16"], frac_alone_vs_burst=a_alone / pk["bf16"]),
+    }
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
@@ -307,18 +547,18 @@ def run_gpu(args):
                    "cells_per_gpu": n, "l2": "inputs (176 MB/step at the full size) exceed the 126 MB L2; no explicit flush",
                    "parallelism": f"replicas x{world} (no collective in the data path)"},
         "kernel_ms": {"T_from_h": k_ms[0], "properties": k_ms[1], "ann_bf16": k_ms[2]},
-        **({"kernel_alone_ms": alone_ms} if alone_ms else {}),
-        "roofline": {"bound": "tensor", "kernel": "ann_bf16_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                     "frac": achieved / peak,
-                     # dram__bytes_read.sum + dram__bytes_write.sum of one launch at the full size (profiles/r1_summary.md)
-                     "traffic": 325.7e6 if n == 2097152 else None,
-                     "peak_source": peak_src, "frac_vs_burst": achieved / pk["bf16"],
-                     "frac_vs_sustained": achieved / pk["bf16_sust"],
-                     "algorithmic": f"{FLOPS_PER_CELL_MLP} flop/cell x {n} cells/launch"},
+        "kernel_alone_ms": alone_ms,
+        "roofline": ann_roof,
+        "kernels": kernels,
+        "fp32_peak": fp32,
         "e2e": {"value": world * n / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
         "gpu_launches": 3 * args.steps,
         "clocks": clocks,
     }
+    if world == 1 and not args.no_configs:
+        del dT0, dp, dY, dh, dTg, dT, cp, mu, lam, D, om, ws
+        torch.cuda.empty_cache()
+        out["configs"] = bench_configs(torch, B, stream, pk, fp32, quick=args.quick_configs)
     if world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(args.ref_cells)
     print(json.dumps(out))
@@ -335,8 +575,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-cells", type=int, default=262144, help="cells per oracle pass (cpu_baseline / reference arm)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--kernels-alone", action="store_true",
-                    help="also time each kernel alone (median of its own launches), reported as kernel_alone_ms")
+    ap.add_argument("--no-configs", action="store_true", help="skip the configs block (BASELINE configs 1, 2, 4, 5)")
+    ap.add_argument("--quick-configs", action="store_true", help="configs block at reduced repetitions / cfg5 at 2 M cells")
+    ap.add_argument("--kernels-alone", action="store_true", help="accepted for compatibility: kernel_alone_ms is always reported")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
@@ -346,4 +587,3 @@ def main():
 
 if __name__ == "__main__":
     main()
-

@@ -83,9 +83,11 @@ DF_API int df_mech_num_species(const df_mech* mech);
  * n_layers linear layers, dims[0] = K+2 inputs (T, p, F(Y_0..K-1)), dims[n_layers] = K outputs,
  * GELU after every layer but the last.  W[l] is [dims[l+1]][dims[l]] row-major (y = x W^T + b).
  * precision 0: fp32 FFMA path (any n_layers >= 1, every dims[l] <= 256).
- * precision 1: 16-bit tensor-core path (tcgen05, fp32 accumulate in TMEM).  Weights are expected to be
- *              bf16-valued (as BASELINE's "bf16 weights"); tcgen05 kind::f16 needs both operands in one format,
- *              so they are held in fp16 (exact for |w| >= 2^-14) and activations are rounded to fp16 (A21).
+ * precision 1: 16-bit tensor-core path (tcgen05, fp32 accumulate in TMEM).  Weights MUST be bf16-valued (BASELINE's
+ *              "bf16 weights": low 16 bits of the fp32 pattern zero, else DF_ERR_INVALID_ARG) and, like the biases,
+ *              finite with magnitude <= 65504 (else DF_ERR_UNSUPPORTED): tcgen05 kind::f16 needs both operands in one
+ *              format, so the weights are held in fp16 (exact for bf16 values >= 2^-14, within 2^-25 below) and the
+ *              activations are rounded to fp16, saturating at +-65504 (A21).
  *              n_layers == 4, dims[1] % 64 == 0, dims[2] % 32 == 0 with 64 <= dims[2] <= 800,
  *              dims[3] % 16 == 0 with 32 <= dims[3] <= 400, K <= 28.
  * x_mean/x_std [K+2] and u_mean/u_std [K] are the Z-score statistics; the network output
@@ -97,9 +99,9 @@ DF_API df_status df_ann_create(df_ann** out, int n_layers, const int* dims,
                         const double* u_mean, const double* u_std,
                         double boxcox_lambda, double dt);
 DF_API df_status df_ann_destroy(df_ann* ann);
-/* Device scratch df_chem_ann_source needs for n_cells cells (0 on the fp32 path).  The bf16
- * path keeps one layer's activations (bf16) for a bounded chunk of cells, so the value does not
- * grow with n_cells beyond that chunk. */
+/* Device scratch df_chem_ann_source needs for n_cells cells on the CURRENT device (0 on the fp32 path).  The
+ * tensor path parks one 128-cell tile of layer-2 activations (fp16) per resident CTA (one per SM), so the value
+ * does not grow with n_cells beyond 128 x SM-count cells. */
 DF_API size_t df_ann_workspace_bytes(const df_ann* ann, long long n_cells);
 
 /* ---- hot call 1: temperature from enthalpy (NS (1); A3, A4) ------------------------------
@@ -144,6 +146,13 @@ DF_API df_status df_host_ctx_destroy(df_host_ctx* ctx);
 DF_API df_status df_step_host(df_host_ctx* ctx, long long n_cells, long long ld,
                        const float* h, const float* p, const float* T_guess, const float* Y,
                        float* T, float* cp, float* mu, float* lambda, float* D, float* omega);
+
+/* ---- measurement helper (not part of the hot path) -------------------------------------------
+ * Launches a register-only dependent-FMA kernel on `stream` (blocks x 256 threads, 16 FMAs per thread per iteration):
+ * variant 0 = scalar FFMA, 1 = packed FFMA2 (the form the property kernels use).  *flops (host, optional) receives
+ * the floating-point operations of the launch (FMA = 2); out (device, optional) receives blocks*256 floats.
+ * bench.py times it with CUDA events: the FP32 "alu" roofline peak measured in the same run. */
+DF_API df_status df_probe_fp32_peak(int variant, int blocks, long long iters, float* out, double* flops, void* stream);
 
 #ifdef __cplusplus
 }

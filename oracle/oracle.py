@@ -16,21 +16,39 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "oracle.cpp")
 _LIB = os.path.join(_HERE, "liboracle.so")
+_LIB_NATIVE = os.path.join(_HERE, "liboracle_native.so")
 _lib = None
+_native = False
+_FLAGS = ["-std=c++17", "-O2", "-ffp-contract=off", "-fopenmp"]
+_FLAGS_NATIVE = ["-std=c++17", "-O3", "-march=native", "-ffp-contract=off", "-fopenmp"]
 
 
 def build(force: bool = False) -> str:
     """g++ -O2 (generic x86-64: the .so travels to another host), OpenMP over cells."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", _SRC, "-o", _LIB]
+        cmd = ["g++", *_FLAGS, "-fPIC", "-shared", _SRC, "-o", _LIB]
         subprocess.run(cmd, check=True)
     return _LIB
+
+
+def use_native_build() -> None:
+    """bench.py's timed legs only: the same source compiled on, and for, the host it is timed
+    on (-O3 -march=native; still -ffp-contract=off, so the arithmetic is the tests').  Always rebuilt: a library
+    carried over from another host could hold instructions this CPU lacks.  Must be called before the first use."""
+    global _native
+    assert _lib is None, "use_native_build() must come before the library is loaded"
+    subprocess.run(["g++", *_FLAGS_NATIVE, "-fPIC", "-shared", _SRC, "-o", _LIB_NATIVE], check=True)
+    _native = True
+
+
+def build_flags() -> str:
+    return "g++ " + " ".join(_FLAGS_NATIVE if _native else _FLAGS)
 
 
 def lib():
     global _lib
     if _lib is None:
-        _lib = C.CDLL(build())
+        _lib = C.CDLL(_LIB_NATIVE if _native else build())
         d, i, ll, vp = C.c_double, C.c_int, C.c_longlong, C.c_void_p
         P = C.c_void_p
         _lib.oracle_mech_create.restype = vp

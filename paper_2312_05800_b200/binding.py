@@ -23,6 +23,7 @@ SYMBOLS = (
     "df_ann_create", "df_ann_destroy", "df_ann_workspace_bytes",
     "df_thermo_T_from_h", "df_thermo_properties", "df_chem_ann_source",
     "df_host_ctx_create", "df_host_ctx_destroy", "df_step_host",
+    "df_probe_fp32_peak",
 )
 
 DF_OK, DF_ERR_INVALID_ARG, DF_ERR_UNSUPPORTED, DF_ERR_ALLOC, DF_ERR_CUDA = range(5)
@@ -55,6 +56,7 @@ _lib.df_chem_ann_source.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp, _vp, _vp, _vp,
 _lib.df_host_ctx_create.argtypes = [C.POINTER(_vp), _vp, _vp, _ll]
 _lib.df_host_ctx_destroy.argtypes = [_vp]
 _lib.df_step_host.argtypes = [_vp, _ll, _ll] + [_vp] * 10
+_lib.df_probe_fp32_peak.argtypes = [_i, _i, _ll, _vp, C.POINTER(_d), _vp]
 
 
 def _check(code: int) -> None:
@@ -195,3 +197,10 @@ class HostCtx:
             self.handle = None
 
     __del__ = close
+
+
+def df_probe_fp32_peak(variant: int, blocks: int, iters: int, out=None, stream=None) -> float:
+    """Launch the FMA-chain probe; returns the flops of the launch (time it with CUDA events)."""
+    fl = _d(0.0)
+    _check(_lib.df_probe_fp32_peak(int(variant), int(blocks), int(iters), _dp(out), C.byref(fl), _stream(stream)))
+    return float(fl.value)
