@@ -54,13 +54,18 @@ struct MechDev {
     float* ddiag;    // [K][5]
     float* dfull;    // [K][K][5] symmetric, generic path
     float* wilkeB;   // [K][K]   B_kj = 1/sqrt(8 (1 + W_k/W_j))
-    // padded / tiled copies for the tiled any-K kernel (properties_tiled.cu); Kp = K rounded up to 8
+    // padded / tiled copies for the any-K kernel (properties_group.cu); Kp = K rounded up to 8, nt = Kp / 8
     int Kp;
-    float* small_p;  // [Kp][24]: invW, sqrtW, visc[5], cond[5], ddiag[5], pad(7); padding species: visc = 1, rest 0
+    float* small_p;  // [Kp][24]: invW, sqrtW, visc[5], cond[5], ddiag[5], W, pad(6); padding species: visc = cond = ddiag = 1, rest 0
     float* thp;      // [Kp][2][6] fp32 thermo (padding: 0)
     double* h0p;     // [Kp][2]   fp64 constant terms
-    float* BT;       // [Kp][Kp]  BT[j][k] = B_kj (padding 1)
-    float* dtile;    // [tiles (kt <= jt)][8][8][8]: coefficients of D_{k0+a, j0+b} (5 used; padding pairs: 1,0,0,0,0)
+    float* BW;       // [4][Kp][16]: BW[w][j][a] = B_{k,j} for k = w Kp/4 + a (Wilke rows of warp w; padding 1)
+    float* dtile;    // [tiles (kt <= jt)][8][8][5]: coefficients of D_{kt 8 + a, jt 8 + b} (padding pairs: 1,0,0,0,0)
+    // diffusion schedule: rounds of up to four species-tile pairs with pairwise disjoint tile indices (round-robin
+    // tournament), one pair per warp; kt < 0 = idle
+    int n_rounds;
+    signed char sched_kt[12][4], sched_jt[12][4];
+    short sched_tile[12][4];
 };
 
 // Fixed-K tables passed as a __grid_constant__ kernel parameter: every coefficient becomes a
@@ -119,7 +124,7 @@ __device__ __forceinline__ float poly4(const float* c, float u) {
 // launchers implemented in the kernel translation units
 df_status launch_T_from_h(const df_mech*, long long n, long long ld, const float* h, const float* Y, float* T,
                           float* cp, int* n_unconv, cudaStream_t s);
-df_status launch_properties_tiled(const df_mech*, long long n, long long ld, const float* T, const float* p, const float* Y,
+df_status launch_properties_group(const df_mech*, long long n, long long ld, const float* T, const float* p, const float* Y,
                                   float* cp, float* h, float* mu, float* lam, float* D, cudaStream_t s);
 df_status launch_properties(const df_mech*, long long n, long long ld, const float* T, const float* p, const float* Y,
                             float* cp, float* h, float* mu, float* lam, float* D, cudaStream_t s);

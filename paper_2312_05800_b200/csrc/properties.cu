@@ -7,7 +7,7 @@
 //   * Wilke: Phi_kj = B_kj (1 + g_k/g_j)^2 with g = sqrt(mu)/(T W)^(1/4) and B_kj = [8 (1 + W_k/W_j)]^(-1/2) tabulated;
 //   * binary diffusion uses each symmetric pair once (4 FFMA Horner + 1 MUFU.RCP + 2 FFMA);
 //   * the formation-enthalpy part of h is accumulated in fp64 (K DFMA), the sensible part in fp32.
-// Other K (e.g. 53) go to the tiled any-K kernel in properties_tiled.cu.
+// Other K (e.g. 53) go to the any-K kernel in properties_group.cu.
 #include "common.cuh"
 
 namespace {
@@ -224,5 +224,5 @@ df_status launch_properties(const df_mech* mech, long long n, long long ld, cons
         return df_set_error(DF_ERR_UNSUPPORTED, "df_thermo_properties: n_cells too large");
     if (mech->t9) return launch_fixed<9>(mech->t9, n, ld, T, p, Y, cp, h, mu, lam, D, s);
     if (mech->t19) return launch_fixed<19>(mech->t19, n, ld, T, p, Y, cp, h, mu, lam, D, s);
-    return launch_properties_tiled(mech, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+    return launch_properties_group(mech, n, ld, T, p, Y, cp, h, mu, lam, D, s);
 }

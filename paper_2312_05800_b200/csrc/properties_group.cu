@@ -1,0 +1,397 @@
+// properties_group.cu -- K2 for any species count K <= 64 (BASELINE config 4: K = 53).  NS (2); A5-A7.
+//
+// At K = 53 the per-cell vectors (X, 1/g, S: 53 values each) do not fit in registers.  Kept per thread in shared
+// memory they cap a thread-owns-its-cells kernel at 6 warps per SM (round 1: 26 % of the FP32 roofline, every
+// O(K) phase exposed to global-memory latency).  Here FOUR WARPS SHARE ONE GROUP OF 64 CELLS: lane l of every warp
+// holds cells 2l, 2l+1 of the group as a float2 (packed FFMA2 arithmetic), the per-cell vectors live once per group
+// in shared memory ([species][lane] float2: 0.5 KB per species), and the species dimension of every phase is split
+// over the four warps -- a quarter of the shared memory per warp (12 warps per SM) and a quarter of the serial work
+// per thread:
+//   phase 1  thermo + x_k = Y_k/W_k            species k = w, w+4, ...; partial sums combined through shared memory
+//   phase 2  X_k, r_k = 1/ghat_k, conductivity  same split
+//   phase 3  Wilke: warp w owns rows k in [w Kp/4, (w+1) Kp/4) (accumulators in registers) and streams all j:
+//            den_k += B_kj (X_j + g_k (2 X_j r_j + g_k X_j r_j^2)) -- three FFMA2 per (k, j), B_kj from a table re-tiled
+//            per warp so that a row segment is four broadcast LDS.128
+//   phase 4  mixture-averaged diffusion over 8 x 8 species tiles, each symmetric pair evaluated once (4 FFMA2 Horner,
+//            one MUFU.RCP for both cells, 2 FFMA2).  The tile pairs of a round come from a round-robin tournament
+//            (mech.cu): they touch disjoint rows of the S accumulators, so the four warps add into shared memory
+//            without atomics; one block barrier per round.  A warp stages its own coefficient tile (1280 B, in
+//            loop order) with cp.async one round ahead.
+//   final    D_k = N_k / S_k with N_k = sum_{j != k} Y_j from tile totals + in-tile sums of Y_j = X_j W_j sum(x)
+//            (direct sums, never 1 - Y_k: A7), self-diffusion D_kk when S_k = 0.
+// A block is one group; it loops over groups (grid-stride) so the tables are staged once per block.
+#include "common.cuh"
+
+namespace {
+
+constexpr int kGT = 128;       // threads per block = 4 warps sharing 64 cells
+constexpr int kGroupCells = 64;
+typedef float2 f2;
+__device__ __forceinline__ f2 bc(float s) { return make_float2(s, s); }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ f2 fma2(f2 a, float s, f2 c) { return __ffma2_rn(a, bc(s), c); }
+__device__ __forceinline__ f2 fma2(f2 a, float s, float c) { return __ffma2_rn(a, bc(s), bc(c)); }
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ f2 mul2(f2 a, float s) { return __fmul2_rn(a, bc(s)); }
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
+// reciprocals of both halves from one MUFU: 1/x = y/(xy), 1/y = x/(xy)
+__device__ __forceinline__ f2 rcp2(f2 a) {
+    const float r = rcp_approx(a.x * a.y);
+    return make_float2(r * a.y, r * a.x);
+}
+__device__ __forceinline__ f2 poly4_2(float c0, float c1, float c2, float c3, float c4, f2 u) {
+    return fma2(fma2(fma2(fma2(u, c4, c3), u, bc(c2)), u, bc(c1)), u, bc(c0));
+}
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+constexpr int kTileFloats = 64 * 5;   // one 8 x 8 tile of pair coefficients
+
+// One 8 x 8 tile of species pairs.  coef: [a][b][5] in shared memory (warp-uniform addresses: broadcast loads).
+template <bool DIAG>
+__device__ __forceinline__ void diff_tile(const float* __restrict__ coef, f2 u, const f2 (&Xk)[8], const f2 (&Xj)[8],
+                                          f2 (&Sk)[8], f2 (&Sj)[8]) {
+#pragma unroll
+    for (int a = 0; a < (DIAG ? 7 : 8); ++a) {
+        float q[40];
+#pragma unroll
+        for (int i = 0; i < 10; ++i) {
+            const float4 v = reinterpret_cast<const float4*>(coef + a * 40)[i];
+            q[4 * i] = v.x; q[4 * i + 1] = v.y; q[4 * i + 2] = v.z; q[4 * i + 3] = v.w;
+        }
+#pragma unroll
+        for (int b = DIAG ? a + 1 : 0; b < 8; ++b) {
+            const f2 r = rcp2(poly4_2(q[5 * b], q[5 * b + 1], q[5 * b + 2], q[5 * b + 3], q[5 * b + 4], u));
+            Sk[a] = fma2(Xj[b], r, Sk[a]);
+            if (DIAG) Sk[b] = fma2(Xk[a], r, Sk[b]);
+            else Sj[b] = fma2(Xk[a], r, Sj[b]);
+        }
+    }
+}
+
+struct GroupSmem {   // byte offsets into the dynamic shared memory of a block
+    int sX, sR, small, thp, h0p, BW, ring, scr, total;
+};
+__host__ __device__ inline GroupSmem group_smem(int Kp) {
+    GroupSmem g;
+    int o = 0;
+    g.sX = o; o += Kp * 32 * 8;
+    g.sR = o; o += Kp * 32 * 8;
+    g.h0p = o; o += Kp * 2 * 8;
+    g.small = o; o += Kp * 24 * 4;
+    g.thp = o; o += Kp * 12 * 4;
+    g.BW = o; o += 4 * Kp * 16 * 4;
+    g.ring = o; o += 4 * 2 * kTileFloats * 4;   // per warp: two coefficient tiles
+    g.scr = o; o += 4 * 12 * 32 * 8;            // per warp: 12 float2-sized slots per lane
+    g.total = o;
+    return g;
+}
+
+template <int KW>   // Wilke rows per warp = Kp / 4
+__global__ void __launch_bounds__(kGT, 3)
+props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld, const float* __restrict__ Tg,
+                   const float* __restrict__ pg, const float* __restrict__ Yg, float* __restrict__ cp_o,
+                   float* __restrict__ h_o, float* __restrict__ mu_o, float* __restrict__ lam_o, float* __restrict__ D_o) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    constexpr int Kp = 4 * KW, nt = Kp / 8;
+    const int K = md.K;
+    const GroupSmem L = group_smem(Kp);
+    f2* sX = reinterpret_cast<f2*>(smem + L.sX);
+    f2* sR = reinterpret_cast<f2*>(smem + L.sR);
+    const double* sH0 = reinterpret_cast<const double*>(smem + L.h0p);
+    const float* sSmall = reinterpret_cast<const float*>(smem + L.small);
+    const float* sTh = reinterpret_cast<const float*>(smem + L.thp);
+    const float* sBW = reinterpret_cast<const float*>(smem + L.BW);
+    float* sRing = reinterpret_cast<float*>(smem + L.ring);
+    f2* sScr = reinterpret_cast<f2*>(smem + L.scr);
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+
+    // ---- stage the tables once per block ----
+    for (int e = tid; e < Kp * 2; e += kGT) reinterpret_cast<double*>(smem + L.h0p)[e] = md.h0p[e];
+    for (int e = tid; e < Kp * 24 / 4; e += kGT)
+        reinterpret_cast<float4*>(smem + L.small)[e] = __ldg(reinterpret_cast<const float4*>(md.small_p) + e);
+    for (int e = tid; e < Kp * 12 / 4; e += kGT)
+        reinterpret_cast<float4*>(smem + L.thp)[e] = __ldg(reinterpret_cast<const float4*>(md.thp) + e);
+    for (int e = tid; e < 4 * Kp * 16 / 4; e += kGT)
+        reinterpret_cast<float4*>(smem + L.BW)[e] = __ldg(reinterpret_cast<const float4*>(md.BW) + e);
+    __syncthreads();
+
+    const bool want_thermo = cp_o || h_o, want_transport = mu_o || lam_o || D_o;
+    const long long ngroups = (n + kGroupCells - 1) / kGroupCells;
+    for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+        // every thread stays alive through the barriers; lanes past the end of the field work on cell 0 and do not store
+        const long long i_raw = grp * kGroupCells + 2 * lane;
+        const bool valid = i_raw < n;
+        const long long i = valid ? i_raw : 0;
+        const bool two = valid && (i + 1 < n);
+        auto ld2 = [&](const float* p) -> f2 {
+            if (two) return __ldg(reinterpret_cast<const float2*>(p + i));
+            const float v = __ldg(p + i);
+            return make_float2(v, v);
+        };
+        auto st2 = [&](float* p, f2 v) {
+            if (two) *reinterpret_cast<float2*>(p + i) = v;
+            else if (valid) p[i] = v.x;
+        };
+        const f2 T = ld2(Tg);
+        const f2 tau = mul2(add2(T, bc(-md.sc.T_mid)), md.sc.inv_S);
+        const bool lo0 = T.x < md.sc.T_mid, lo1 = T.y < md.sc.T_mid;   // A2: hi for T >= T_mid
+
+        // ---- phase 1: x_k = Y_k / W_k and the thermo sums of this warp's species --------------------------------
+        {
+            f2 C[5];
+#pragma unroll
+            for (int m = 0; m < 5; ++m) C[m] = bc(0.f);
+            double H0a = 0.0, H0b = 0.0;
+            f2 sumx = bc(0.f);
+#pragma unroll 4
+            for (int k = w; k < Kp; k += 4) {
+                const f2 y = (k < K) ? ld2(Yg + (size_t)k * ld) : bc(0.f);
+                const f2 x = mul2(y, sSmall[k * 24]);
+                sX[k * 32 + lane] = x;
+                sumx = add2(sumx, x);
+                if (want_thermo) {
+                    const float4 a = *reinterpret_cast<const float4*>(sTh + k * 12), b = *reinterpret_cast<const float4*>(sTh + k * 12 + 4),
+                                 c = *reinterpret_cast<const float4*>(sTh + k * 12 + 8);   // lo c0..c5 | hi c0..c5
+                    C[0] = fma2(y, make_float2(lo0 ? a.y : b.w, lo1 ? a.y : b.w), C[0]);
+                    C[1] = fma2(y, make_float2(lo0 ? a.z : c.x, lo1 ? a.z : c.x), C[1]);
+                    C[2] = fma2(y, make_float2(lo0 ? a.w : c.y, lo1 ? a.w : c.y), C[2]);
+                    C[3] = fma2(y, make_float2(lo0 ? b.x : c.z, lo1 ? b.x : c.z), C[3]);
+                    C[4] = fma2(y, make_float2(lo0 ? b.y : c.w, lo1 ? b.y : c.w), C[4]);
+                    if (h_o) {   // formation-enthalpy term in fp64 (|h| ~ 1e7 J/kg against a 1e-5 tolerance)
+                        const double hl = sH0[2 * k], hh = sH0[2 * k + 1];
+                        H0a = fma((double)y.x, lo0 ? hl : hh, H0a);
+                        H0b = fma((double)y.y, lo1 ? hl : hh, H0b);
+                    }
+                }
+            }
+            f2* my = sScr + (w * 12) * 32 + lane;
+            my[0] = sumx;
+            if (want_thermo) {
+#pragma unroll
+                for (int m = 0; m < 5; ++m) my[(1 + m) * 32] = C[m];
+                reinterpret_cast<double*>(my)[6 * 32] = H0a;
+                reinterpret_cast<double*>(my)[7 * 32] = H0b;
+            }
+        }
+        __syncthreads();
+        f2 sumx = bc(0.f);
+#pragma unroll
+        for (int v = 0; v < 4; ++v) sumx = add2(sumx, sScr[(v * 12) * 32 + lane]);
+        if (want_thermo && w == 1) {
+            f2 q[5];
+#pragma unroll
+            for (int m = 0; m < 5; ++m) {
+                q[m] = bc(0.f);
+#pragma unroll
+                for (int v = 0; v < 4; ++v) q[m] = add2(q[m], sScr[(v * 12 + 1 + m) * 32 + lane]);
+            }
+            if (cp_o)
+                st2(cp_o, mul2(fma2(fma2(fma2(fma2(mul2(q[4], 5.f), tau, mul2(q[3], 4.f)), tau, mul2(q[2], 3.f)), tau,
+                                         mul2(q[1], 2.f)), tau, q[0]),
+                               md.sc.inv_S));
+            if (h_o) {
+                double Ha = 0.0, Hb = 0.0;
+#pragma unroll
+                for (int v = 0; v < 4; ++v) {
+                    Ha += reinterpret_cast<const double*>(sScr + (v * 12) * 32 + lane)[6 * 32];
+                    Hb += reinterpret_cast<const double*>(sScr + (v * 12) * 32 + lane)[7 * 32];
+                }
+                const f2 sens = mul2(tau, fma2(fma2(fma2(fma2(q[4], tau, q[3]), tau, q[2]), tau, q[1]), tau, q[0]));
+                st2(h_o, make_float2((float)(Ha + (double)sens.x), (float)(Hb + (double)sens.y)));
+            }
+        }
+        if (!want_transport) {   // block-uniform
+            __syncthreads();     // the scratch is rewritten by the next group
+            continue;
+        }
+
+        // ---- phase 2: X_k, r_k = 1/ghat_k, conductivity sums -----------------------------------------------------
+        const f2 inv_sumx = make_float2(1.0f / sumx.x, 1.0f / sumx.y);
+        const f2 u = mul2(add2(make_float2(logf(T.x), logf(T.y)), bc(-md.sc.Lc)), md.sc.inv_Ls);
+        const f2 sqrtT = make_float2(sqrtf(T.x), sqrtf(T.y));
+        {
+            f2 s1 = bc(0.f), s2 = bc(0.f);
+#pragma unroll 2
+            for (int k = w; k < Kp; k += 4) {
+                const f2 X = mul2(sX[k * 32 + lane], inv_sumx);
+                sX[k * 32 + lane] = X;
+                const float4 a = *reinterpret_cast<const float4*>(sSmall + k * 24), b = *reinterpret_cast<const float4*>(sSmall + k * 24 + 4),
+                             c = *reinterpret_cast<const float4*>(sSmall + k * 24 + 8);   // invW sqrtW v0 v1 | v2 v3 v4 c0 | c1 c2 c3 c4
+                sR[k * 32 + lane] = rcp2(poly4_2(a.z, a.w, b.x, b.y, b.z, u));
+                const f2 lk = poly4_2(b.w, c.x, c.y, c.z, c.w, u);
+                s1 = fma2(X, lk, s1);
+                s2 = fma2(X, rcp2(lk), s2);
+            }
+            f2* my = sScr + (w * 12 + 8) * 32 + lane;   // slots 8, 9 (slot 0..7 may still be read by warp 1)
+            my[0] = s1;
+            my[32] = s2;
+        }
+        __syncthreads();
+        if (lam_o && w == 0) {
+            f2 s1 = bc(0.f), s2 = bc(0.f);
+#pragma unroll
+            for (int v = 0; v < 4; ++v) {
+                s1 = add2(s1, sScr[(v * 12 + 8) * 32 + lane]);
+                s2 = add2(s2, sScr[(v * 12 + 9) * 32 + lane]);
+            }
+            st2(lam_o, mul2(mul2(sqrtT, 0.5f), add2(s1, rcp2(s2))));   // A6
+        }
+
+        // ---- phase 3: Wilke; this warp owns rows k0 .. k0 + KW - 1 ------------------------------------------------
+        if (mu_o) {
+            const int k0 = w * KW;
+            f2 gk[KW], den[KW];
+#pragma unroll
+            for (int a = 0; a < KW; ++a) {
+                gk[a] = rcp2(sR[(k0 + a) * 32 + lane]);
+                den[a] = bc(0.f);
+            }
+            const float* bw = sBW + (size_t)w * Kp * 16;
+#pragma unroll 2
+            for (int j = 0; j < Kp; ++j) {
+                const f2 xj = sX[j * 32 + lane], rj = sR[j * 32 + lane];
+                const f2 xr = mul2(xj, rj);
+                const f2 b2 = add2(xr, xr), c = mul2(xr, rj);
+                float B[16];
+#pragma unroll
+                for (int q4 = 0; q4 < (KW + 3) / 4; ++q4) {
+                    const float4 v = *reinterpret_cast<const float4*>(bw + j * 16 + 4 * q4);
+                    B[4 * q4] = v.x; B[4 * q4 + 1] = v.y; B[4 * q4 + 2] = v.z; B[4 * q4 + 3] = v.w;
+                }
+#pragma unroll
+                for (int a = 0; a < KW; ++a)   // B_kj X_j (1 + g_k r_j)^2, expanded: all terms positive
+                    den[a] = fma2(fma2(gk[a], fma2(gk[a], c, b2), xj), B[a], den[a]);
+            }
+            f2 acc = bc(0.f);
+#pragma unroll
+            for (int a = 0; a < KW; ++a)
+                acc = fma2(mul2(mul2(sX[(k0 + a) * 32 + lane], sSmall[(k0 + a) * 24 + 1]), mul2(gk[a], gk[a])), rcp2(den[a]), acc);
+            sScr[(w * 12 + 10) * 32 + lane] = acc;
+        }
+        __syncthreads();   // every warp is done reading r: sR becomes the S accumulators
+        if (mu_o && w == 0) {
+            f2 acc = bc(0.f);
+#pragma unroll
+            for (int v = 0; v < 4; ++v) acc = add2(acc, sScr[(v * 12 + 10) * 32 + lane]);
+            st2(mu_o, mul2(sqrtT, acc));
+        }
+        if (!D_o) continue;   // block-uniform; the barrier above also protects the scratch
+
+        // ---- phase 4: mixture-averaged diffusivities ---------------------------------------------------------------
+        for (int k = w; k < Kp; k += 4) sR[k * 32 + lane] = bc(0.f);
+        float* ring = sRing + w * 2 * kTileFloats;
+        auto stage = [&](int round, int buf) {
+            if (md.sched_kt[round][w] >= 0) {
+                const float* src = md.dtile + (size_t)md.sched_tile[round][w] * kTileFloats;
+                for (int c16 = lane; c16 < kTileFloats / 4; c16 += 32) cp_async16(ring + buf * kTileFloats + 4 * c16, src + 4 * c16);
+            }
+            cp_async_commit();
+        };
+        stage(0, 0);
+        __syncthreads();   // S is zeroed everywhere
+        for (int r = 0; r < md.n_rounds; ++r) {
+            if (r + 1 < md.n_rounds) stage(r + 1, (r + 1) & 1);
+            else cp_async_commit();
+            cp_async_wait<1>();
+            __syncwarp();
+            const int kt = md.sched_kt[r][w], jt = md.sched_jt[r][w];
+            if (kt >= 0) {   // warp-uniform
+                const float* coef = ring + (r & 1) * kTileFloats;
+                f2 Xk[8], Xj[8], Sk[8], Sj[8];
+#pragma unroll
+                for (int a = 0; a < 8; ++a) {
+                    Xk[a] = sX[(kt * 8 + a) * 32 + lane];
+                    Xj[a] = sX[(jt * 8 + a) * 32 + lane];
+                    Sk[a] = Sj[a] = bc(0.f);
+                }
+                if (kt == jt) diff_tile<true>(coef, u, Xk, Xj, Sk, Sj);
+                else diff_tile<false>(coef, u, Xk, Xj, Sk, Sj);
+                // rows kt and jt of S belong to this warp alone in this round
+#pragma unroll
+                for (int a = 0; a < 8; ++a) sR[(kt * 8 + a) * 32 + lane] = add2(sR[(kt * 8 + a) * 32 + lane], Sk[a]);
+                if (kt != jt) {
+#pragma unroll
+                    for (int a = 0; a < 8; ++a) sR[(jt * 8 + a) * 32 + lane] = add2(sR[(jt * 8 + a) * 32 + lane], Sj[a]);
+                }
+            }
+            __syncthreads();
+        }
+        cp_async_wait<0>();
+
+        // ---- final: D_k = N_k / S_k, species a = w and w + 4 of every tile ------------------------------------------
+        {
+            const f2 p = ld2(pg);
+            const f2 scale = make_float2(T.x * sqrtT.x / p.x, T.y * sqrtT.y / p.y);
+            f2 TT[nt];   // tile totals of Y_j = X_j W_j sum(x)
+#pragma unroll
+            for (int t = 0; t < nt; ++t) {
+                TT[t] = bc(0.f);
+#pragma unroll
+                for (int a = 0; a < 8; ++a) TT[t] = fma2(sX[(t * 8 + a) * 32 + lane], sSmall[(t * 8 + a) * 24 + 17], TT[t]);
+            }
+#pragma unroll
+            for (int t = 0; t < nt; ++t) {
+                f2 others = bc(0.f);
+#pragma unroll
+                for (int t2 = 0; t2 < nt; ++t2)
+                    if (t2 != t) others = add2(others, TT[t2]);
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int a = w + 4 * h, k = t * 8 + a;
+                    if (k < K) {
+                        f2 Nk = others;
+#pragma unroll
+                        for (int b = 0; b < 8; ++b)
+                            if (b != a) Nk = fma2(sX[(t * 8 + b) * 32 + lane], sSmall[(t * 8 + b) * 24 + 17], Nk);
+                        Nk = mul2(Nk, sumx);
+                        const f2 S = sR[k * 32 + lane];
+                        const float* dd = sSmall + k * 24 + 12;
+                        const f2 dk = poly4_2(dd[0], dd[1], dd[2], dd[3], dd[4], u);
+                        const f2 q = mul2(Nk, rcp2(make_float2(S.x > 0.f ? S.x : 1.f, S.y > 0.f ? S.y : 1.f)));
+                        const f2 Dk = make_float2(S.x > 0.f ? q.x : dk.x, S.y > 0.f ? q.y : dk.y);   // A7
+                        st2(D_o + (size_t)k * ld, mul2(Dk, scale));
+                    }
+                }
+            }
+        }
+        __syncthreads();   // sX / sR / scratch are rewritten by the next group
+    }
+}
+
+template <int KW>
+df_status launch_kw(const MechDev& md, long long n, long long ld, const float* T, const float* p, const float* Y, float* cp,
+                    float* h, float* mu, float* lam, float* D, cudaStream_t s) {
+    const int smem = group_smem(4 * KW).total;
+    static DfPerDevice smem_attr;
+    const df_status st = df_ensure_dyn_smem((const void*)props_group_kernel<KW>, smem, &smem_attr);
+    if (st != DF_OK) return st;
+    const long long ngroups = (n + kGroupCells - 1) / kGroupCells;
+    const long long cap = (long long)df_device_sm_count() * 3 * 4;   // 3 resident blocks per SM, ~4 waves
+    const long long blocks = ngroups < cap ? ngroups : cap;
+    props_group_kernel<KW><<<(unsigned)(blocks > 0 ? blocks : 1), kGT, smem, s>>>(md, n, ld, T, p, Y, cp, h, mu, lam, D);
+    DF_CUDA_TRY(cudaGetLastError());
+    return DF_OK;
+}
+
+}  // namespace
+
+df_status launch_properties_group(const df_mech* mech, long long n, long long ld, const float* T, const float* p,
+                                  const float* Y, float* cp, float* h, float* mu, float* lam, float* D, cudaStream_t s) {
+    const MechDev& md = mech->dev;
+    switch (md.Kp / 8) {
+        case 1: return launch_kw<2>(md, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+        case 2: return launch_kw<4>(md, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+        case 3: return launch_kw<6>(md, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+        case 4: return launch_kw<8>(md, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+        case 5: return launch_kw<10>(md, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+        case 6: return launch_kw<12>(md, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+        case 7: return launch_kw<14>(md, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+        case 8: return launch_kw<16>(md, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+    }
+    return df_set_error(DF_ERR_UNSUPPORTED, "df_thermo_properties: K = %d", md.K);
+}
