@@ -39,6 +39,8 @@ __device__ __forceinline__ f2 rcp2(f2 a) {
     const float r = rcp_approx(a.x * a.y);
     return make_float2(r * a.y, r * a.x);
 }
+// one MUFU per half: in the FMA-bound pair loop the XU pipe is idle and the three multiplies of rcp2 are not
+__device__ __forceinline__ f2 rcp2x(f2 a) { return make_float2(rcp_approx(a.x), rcp_approx(a.y)); }
 __device__ __forceinline__ f2 poly4_2(float c0, float c1, float c2, float c3, float c4, f2 u) {
     return fma2(fma2(fma2(fma2(u, c4, c3), u, bc(c2)), u, bc(c1)), u, bc(c0));
 }
@@ -65,7 +67,7 @@ __device__ __forceinline__ void diff_tile(const float* __restrict__ coef, f2 u, 
         }
 #pragma unroll
         for (int b = DIAG ? a + 1 : 0; b < 8; ++b) {
-            const f2 r = rcp2(poly4_2(q[5 * b], q[5 * b + 1], q[5 * b + 2], q[5 * b + 3], q[5 * b + 4], u));
+            const f2 r = rcp2x(poly4_2(q[5 * b], q[5 * b + 1], q[5 * b + 2], q[5 * b + 3], q[5 * b + 4], u));
             Sk[a] = fma2(Xj[b], r, Sk[a]);
             if (DIAG) Sk[b] = fma2(Xk[a], r, Sk[b]);
             else Sj[b] = fma2(Xk[a], r, Sj[b]);
@@ -122,6 +124,18 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
 
     const bool want_thermo = cp_o || h_o, want_transport = mu_o || lam_o || D_o;
     const long long ngroups = (n + kGroupCells - 1) / kGroupCells;
+    // T and p of a group are loaded one group ahead (their latency would otherwise open every group)
+    auto ld2_at = [&](const float* p, long long grp) -> f2 {
+        const long long ir = grp * kGroupCells + 2 * lane;
+        if (ir + 1 < n) return __ldg(reinterpret_cast<const float2*>(p + ir));
+        const float v = __ldg(p + (ir < n ? ir : 0));
+        return make_float2(v, v);
+    };
+    f2 T_next = bc(1000.f), p_next = bc(1.f);
+    if ((long long)blockIdx.x < ngroups) {
+        T_next = ld2_at(Tg, blockIdx.x);
+        if (D_o) p_next = ld2_at(pg, blockIdx.x);
+    }
     for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
         // every thread stays alive through the barriers; lanes past the end of the field work on cell 0 and do not store
         const long long i_raw = grp * kGroupCells + 2 * lane;
@@ -137,7 +151,15 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
             if (two) *reinterpret_cast<float2*>(p + i) = v;
             else if (valid) p[i] = v.x;
         };
-        const f2 T = ld2(Tg);
+        const f2 T = T_next, p_cell = p_next;
+        // all of this warp's Y rows in flight at once, then the next group's T and p
+        f2 yv[KW];
+#pragma unroll
+        for (int a = 0; a < KW; ++a) yv[a] = (w + 4 * a < K) ? ld2(Yg + (size_t)(w + 4 * a) * ld) : bc(0.f);
+        if (grp + gridDim.x < ngroups) {
+            T_next = ld2_at(Tg, grp + gridDim.x);
+            if (D_o) p_next = ld2_at(pg, grp + gridDim.x);
+        }
         const f2 tau = mul2(add2(T, bc(-md.sc.T_mid)), md.sc.inv_S);
         const bool lo0 = T.x < md.sc.T_mid, lo1 = T.y < md.sc.T_mid;   // A2: hi for T >= T_mid
 
@@ -148,9 +170,10 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
             for (int m = 0; m < 5; ++m) C[m] = bc(0.f);
             double H0a = 0.0, H0b = 0.0;
             f2 sumx = bc(0.f);
-#pragma unroll 4
-            for (int k = w; k < Kp; k += 4) {
-                const f2 y = (k < K) ? ld2(Yg + (size_t)k * ld) : bc(0.f);
+#pragma unroll
+            for (int a = 0; a < KW; ++a) {
+                const int k = w + 4 * a;
+                const f2 y = yv[a];
                 const f2 x = mul2(y, sSmall[k * 24]);
                 sX[k * 32 + lane] = x;
                 sumx = add2(sumx, x);
@@ -325,8 +348,7 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
 
         // ---- final: D_k = N_k / S_k, species a = w and w + 4 of every tile ------------------------------------------
         {
-            const f2 p = ld2(pg);
-            const f2 scale = make_float2(T.x * sqrtT.x / p.x, T.y * sqrtT.y / p.y);
+            const f2 scale = make_float2(T.x * sqrtT.x / p_cell.x, T.y * sqrtT.y / p_cell.y);
             f2 TT[nt];   // tile totals of Y_j = X_j W_j sum(x)
 #pragma unroll
             for (int t = 0; t < nt; ++t) {
