@@ -56,16 +56,12 @@ struct MechDev {
     float* wilkeB;   // [K][K]   B_kj = 1/sqrt(8 (1 + W_k/W_j))
     // padded / tiled copies for the any-K kernel (properties_group.cu); Kp = K rounded up to 8, nt = Kp / 8
     int Kp;
-    float* small_p;  // [Kp][24]: invW, sqrtW, visc[5], cond[5], ddiag[5], W, pad(6); padding species: visc = cond = ddiag = 1, rest 0
+    float* small_p;  // [Kp][20]: invW, sqrtW, visc[5], cond[5], ddiag[5], pad(3); padding species: visc = cond = ddiag = 1, rest 0
     float* thp;      // [Kp][2][6] fp32 thermo (padding: 0)
     double* h0p;     // [Kp][2]   fp64 constant terms
     float* BW;       // [4][Kp][16]: BW[w][j][a] = B_{k,j} for k = w Kp/4 + a (Wilke rows of warp w; padding 1)
-    float* dtile;    // [tiles (kt <= jt)][8][8][5]: coefficients of D_{kt 8 + a, jt 8 + b} (padding pairs: 1,0,0,0,0)
-    // diffusion schedule: rounds of up to four species-tile pairs with pairwise disjoint tile indices (round-robin
-    // tournament), one pair per warp; kt < 0 = idle
-    int n_rounds;
-    signed char sched_kt[12][4], sched_jt[12][4];
-    short sched_tile[12][4];
+    float* dtile;    // eight species tiles of TS = Kp/8: [36 tile pairs (kt <= jt)][TS][row of TS x 5, padded to 4 floats]
+                     // = coefficients of D_{kt TS + a, jt TS + b} (padding pairs: 1,0,0,0,0)
 };
 
 // Fixed-K tables passed as a __grid_constant__ kernel parameter: every coefficient becomes a

@@ -164,13 +164,13 @@ extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const
         return st;
     }
     {   // padded / tiled tables of the any-K kernel (properties_group.cu)
-        const int Kp = (K + 7) / 8 * 8, nt = Kp / 8, KW = Kp / 4;
+        const int Kp = (K + 7) / 8 * 8, KW = Kp / 4, TS = Kp / 8, RS = (TS * 5 + 3) / 4 * 4;
         d.Kp = Kp;
-        std::vector<float> small((size_t)Kp * 24, 0.f), thp((size_t)Kp * 12, 0.f), BW((size_t)4 * Kp * 16, 1.f);
+        std::vector<float> small((size_t)Kp * 20, 0.f), thp((size_t)Kp * 12, 0.f), BW((size_t)4 * Kp * 16, 1.f);
         std::vector<double> h0p((size_t)Kp * 2, 0.0);
-        std::vector<float> dt((size_t)nt * (nt + 1) / 2 * 64 * 5, 0.f);
+        std::vector<float> dt((size_t)36 * TS * RS, 0.f);
         for (int k = 0; k < Kp; ++k) {
-            float* sp = &small[(size_t)k * 24];
+            float* sp = &small[(size_t)k * 20];
             if (k < K) {
                 sp[0] = t.invW[k];
                 sp[1] = t.sqrtW[k];
@@ -179,7 +179,6 @@ extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const
                     sp[7 + m] = t.cond[k * 5 + m];
                     sp[12 + m] = t.ddiag[k * 5 + m];
                 }
-                sp[17] = (float)W[k];
                 for (int i = 0; i < 12; ++i) thp[(size_t)k * 12 + i] = t.th32[(size_t)k * 12 + i];
                 h0p[k * 2] = t.th64[(size_t)(k * 2) * 6];
                 h0p[k * 2 + 1] = t.th64[(size_t)(k * 2 + 1) * 6];
@@ -195,69 +194,19 @@ extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const
                     const int k = w * KW + a;
                     if (k < K) BW[((size_t)w * Kp + j) * 16 + a] = t.wilkeB[(size_t)k * K + j];
                 }
-        std::vector<int> tile_of((size_t)nt * nt, -1);
+        // eight species tiles of TS; tile pair (kt <= jt) number kt*8 - kt(kt-1)/2 + (jt - kt): [a][b][5], rows padded to RS
         size_t tix = 0;
-        for (int kt = 0; kt < nt; ++kt)
-            for (int jt = kt; jt < nt; ++jt, ++tix) {
-                tile_of[(size_t)kt * nt + jt] = (int)tix;
-                for (int a = 0; a < 8; ++a)
-                    for (int b = 0; b < 8; ++b) {
-                        float* c = &dt[((tix * 8 + a) * 8 + b) * 5];
-                        const int k = kt * 8 + a, j = jt * 8 + b;
+        for (int kt = 0; kt < 8; ++kt)
+            for (int jt = kt; jt < 8; ++jt, ++tix)
+                for (int a = 0; a < TS; ++a)
+                    for (int b = 0; b < TS; ++b) {
+                        float* c = &dt[(tix * TS + a) * RS + (size_t)b * 5];
+                        const int k = kt * TS + a, j = jt * TS + b;
                         if (k < K && j < K)
                             for (int m = 0; m < 5; ++m) c[m] = t.dfull[((size_t)k * K + j) * 5 + m];
                         else
                             c[0] = 1.f;
                     }
-            }
-        // Round-robin tournament over the species tiles (plus a dummy when their number is odd: its partner gets
-        // its diagonal tile): every round pairs each tile with exactly one other, so the <= 4 tile pairs of a round
-        // touch disjoint rows of the S accumulators.  Diagonal tiles not covered that way follow, four per round.
-        std::vector<std::pair<int, int>> rounds_flat;
-        int n_rounds = 0;
-        auto add_round = [&](const std::vector<std::pair<int, int>>& m) {
-            for (int w = 0; w < 4; ++w) {
-                const bool on = w < (int)m.size();
-                int kt = on ? m[w].first : -1, jt = on ? m[w].second : -1;
-                if (on && kt > jt) std::swap(kt, jt);
-                d.sched_kt[n_rounds][w] = (signed char)kt;
-                d.sched_jt[n_rounds][w] = (signed char)jt;
-                d.sched_tile[n_rounds][w] = (short)(on ? tile_of[(size_t)kt * nt + jt] : 0);
-            }
-            ++n_rounds;
-        };
-        const int teams = (nt % 2) ? nt + 1 : nt;   // team index nt (when odd) is the dummy
-        std::vector<bool> diag_done(nt, false);
-        if (nt == 1) {
-            add_round({{0, 0}});
-            diag_done[0] = true;
-        } else {
-            std::vector<int> ring(teams);
-            for (int i = 0; i < teams; ++i) ring[i] = i;
-            for (int r = 0; r < teams - 1; ++r) {
-                std::vector<std::pair<int, int>> m;
-                for (int i = 0; i < teams / 2; ++i) {
-                    int x = ring[i], y = ring[teams - 1 - i];
-                    if (x >= nt) { x = y; diag_done[y] = true; }
-                    else if (y >= nt) { y = x; diag_done[x] = true; }
-                    m.push_back({x, y});
-                }
-                add_round(m);
-                const int last = ring[teams - 1];   // rotate all but the first
-                for (int i = teams - 1; i > 1; --i) ring[i] = ring[i - 1];
-                ring[1] = last;
-            }
-        }
-        {
-            std::vector<std::pair<int, int>> m;
-            for (int x = 0; x < nt; ++x)
-                if (!diag_done[x]) {
-                    m.push_back({x, x});
-                    if (m.size() == 4) { add_round(m); m.clear(); }
-                }
-            if (!m.empty()) add_round(m);
-        }
-        d.n_rounds = n_rounds;
         if ((st = to_device(&d.small_p, small)) || (st = to_device(&d.thp, thp)) || (st = to_device(&d.h0p, h0p)) ||
             (st = to_device(&d.BW, BW)) || (st = to_device(&d.dtile, dt))) {
             df_mech_destroy(mech);

@@ -12,13 +12,15 @@
 //   phase 3  Wilke: warp w owns rows k in [w Kp/4, (w+1) Kp/4) (accumulators in registers) and streams all j:
 //            den_k += B_kj (X_j + g_k (2 X_j r_j + g_k X_j r_j^2)) -- three FFMA2 per (k, j), B_kj from a table re-tiled
 //            per warp so that a row segment is four broadcast LDS.128
-//   phase 4  mixture-averaged diffusion over 8 x 8 species tiles, each symmetric pair evaluated once (4 FFMA2 Horner,
-//            one MUFU.RCP for both cells, 2 FFMA2).  The tile pairs of a round come from a round-robin tournament
-//            (mech.cu): they touch disjoint rows of the S accumulators, so the four warps add into shared memory
-//            without atomics; one block barrier per round.  A warp stages its own coefficient tile (1280 B, in
-//            loop order) with cp.async one round ahead.
-//   final    D_k = N_k / S_k with N_k = sum_{j != k} Y_j from tile totals + in-tile sums of Y_j = X_j W_j sum(x)
-//            (direct sums, never 1 - Y_k: A7), self-diffusion D_kk when S_k = 0.
+//   phase 4  mixture-averaged diffusion: the Kp species form EIGHT tiles of TS = Kp/8, each symmetric pair of species is
+//            evaluated once (4 FFMA2 Horner, two MUFU.RCP, 2 FFMA2).  The 28 off-diagonal tile pairs are played as a
+//            round-robin tournament of 8 teams: 7 rounds x 4 pairs with pairwise disjoint tiles, one pair per warp, so
+//            the four warps add into the shared S accumulators without atomics and every round is balanced; two more
+//            rounds take the 8 diagonal tiles.  One block barrier per round.  A warp stages its own coefficient tile
+//            (<= 1280 B, in loop order) with cp.async one round ahead.
+//   final    D_k = N_k / S_k, N_k = sum_{j != k} Y_j evaluated as (sum_j Y_j) - Y_k IN FP64 on the exact fp32 Y (the
+//            fp32 form of that difference is the cancellation A7 warns of; in fp64 it is exact to 1e-16 sum Y),
+//            self-diffusion D_kk when S_k = 0.
 // A block is one group; it loops over groups (grid-stride) so the tables are staged once per block.
 #include "common.cuh"
 
@@ -51,22 +53,30 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-constexpr int kTileFloats = 64 * 5;   // one 8 x 8 tile of pair coefficients
+constexpr int kTileFloatsMax = 8 * 40;   // ring slot: the largest tile (TS = 8: 8 rows of 8 pairs x 5 coefficients)
+__host__ __device__ constexpr int tile_row_floats(int TS) { return (TS * 5 + 3) / 4 * 4; }   // rows start 16-byte aligned
 
-// One 8 x 8 tile of species pairs.  coef: [a][b][5] in shared memory (warp-uniform addresses: broadcast loads).
-template <bool DIAG>
-__device__ __forceinline__ void diff_tile(const float* __restrict__ coef, f2 u, const f2 (&Xk)[8], const f2 (&Xj)[8],
-                                          f2 (&Sk)[8], f2 (&Sj)[8]) {
+// round-robin tournament of the 8 species tiles (circle method), then the diagonal tiles: [round][warp]
+__constant__ signed char kSchedK[9][4] = {{0, 1, 2, 3}, {0, 5, 1, 2}, {0, 4, 3, 1}, {0, 3, 2, 1}, {0, 2, 1, 6}, {0, 1, 4, 5}, {0, 2, 3, 4}, {0, 1, 2, 3}, {4, 5, 6, 7}};
+__constant__ signed char kSchedJ[9][4] = {{7, 6, 5, 4}, {6, 7, 4, 3}, {5, 6, 7, 2}, {4, 5, 6, 7}, {3, 4, 5, 7}, {2, 3, 7, 6}, {1, 7, 6, 5}, {0, 1, 2, 3}, {4, 5, 6, 7}};
+constexpr int kRounds = 9;
+__device__ __forceinline__ int tile_index(int kt, int jt) { return kt * 8 - kt * (kt - 1) / 2 + (jt - kt); }   // kt <= jt
+
+// One TS x TS tile of species pairs.  coef: [a][b][5] in shared memory (warp-uniform addresses: broadcast loads).
+template <int TS, bool DIAG>
+__device__ __forceinline__ void diff_tile(const float* __restrict__ coef, f2 u, const f2 (&Xk)[TS], const f2 (&Xj)[TS],
+                                          f2 (&Sk)[TS], f2 (&Sj)[TS]) {
+    constexpr int RS = tile_row_floats(TS);
 #pragma unroll
-    for (int a = 0; a < (DIAG ? 7 : 8); ++a) {
-        float q[40];
+    for (int a = 0; a < (DIAG ? TS - 1 : TS); ++a) {
+        float q[RS];
 #pragma unroll
-        for (int i = 0; i < 10; ++i) {
-            const float4 v = reinterpret_cast<const float4*>(coef + a * 40)[i];
+        for (int i = 0; i < RS / 4; ++i) {
+            const float4 v = reinterpret_cast<const float4*>(coef + a * RS)[i];
             q[4 * i] = v.x; q[4 * i + 1] = v.y; q[4 * i + 2] = v.z; q[4 * i + 3] = v.w;
         }
 #pragma unroll
-        for (int b = DIAG ? a + 1 : 0; b < 8; ++b) {
+        for (int b = DIAG ? a + 1 : 0; b < TS; ++b) {
             const f2 r = rcp2x(poly4_2(q[5 * b], q[5 * b + 1], q[5 * b + 2], q[5 * b + 3], q[5 * b + 4], u));
             Sk[a] = fma2(Xj[b], r, Sk[a]);
             if (DIAG) Sk[b] = fma2(Xk[a], r, Sk[b]);
@@ -74,6 +84,9 @@ __device__ __forceinline__ void diff_tile(const float* __restrict__ coef, f2 u, 
         }
     }
 }
+
+constexpr int kScrSlots = 14;   // per warp and lane: float2-sized exchange slots (sum x, 5 C, 2 H0, s1, s2, acc, 2 sum Y)
+constexpr int kSmallStride = 20;
 
 struct GroupSmem {   // byte offsets into the dynamic shared memory of a block
     int sX, sR, small, thp, h0p, BW, ring, scr, total;
@@ -84,11 +97,11 @@ __host__ __device__ inline GroupSmem group_smem(int Kp) {
     g.sX = o; o += Kp * 32 * 8;
     g.sR = o; o += Kp * 32 * 8;
     g.h0p = o; o += Kp * 2 * 8;
-    g.small = o; o += Kp * 24 * 4;
+    g.small = o; o += Kp * kSmallStride * 4;
     g.thp = o; o += Kp * 12 * 4;
     g.BW = o; o += 4 * Kp * 16 * 4;
-    g.ring = o; o += 4 * 2 * kTileFloats * 4;   // per warp: two coefficient tiles
-    g.scr = o; o += 4 * 12 * 32 * 8;            // per warp: 12 float2-sized slots per lane
+    g.ring = o; o += 4 * 2 * kTileFloatsMax * 4;   // per warp: two coefficient tiles
+    g.scr = o; o += 4 * kScrSlots * 32 * 8;
     g.total = o;
     return g;
 }
@@ -99,7 +112,7 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
                    const float* __restrict__ pg, const float* __restrict__ Yg, float* __restrict__ cp_o,
                    float* __restrict__ h_o, float* __restrict__ mu_o, float* __restrict__ lam_o, float* __restrict__ D_o) {
     extern __shared__ __align__(16) unsigned char smem[];
-    constexpr int Kp = 4 * KW, nt = Kp / 8;
+    constexpr int Kp = 4 * KW, TS = KW / 2;   // eight species tiles of TS
     const int K = md.K;
     const GroupSmem L = group_smem(Kp);
     f2* sX = reinterpret_cast<f2*>(smem + L.sX);
@@ -114,7 +127,7 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
 
     // ---- stage the tables once per block ----
     for (int e = tid; e < Kp * 2; e += kGT) reinterpret_cast<double*>(smem + L.h0p)[e] = md.h0p[e];
-    for (int e = tid; e < Kp * 24 / 4; e += kGT)
+    for (int e = tid; e < Kp * kSmallStride / 4; e += kGT)
         reinterpret_cast<float4*>(smem + L.small)[e] = __ldg(reinterpret_cast<const float4*>(md.small_p) + e);
     for (int e = tid; e < Kp * 12 / 4; e += kGT)
         reinterpret_cast<float4*>(smem + L.thp)[e] = __ldg(reinterpret_cast<const float4*>(md.thp) + e);
@@ -168,15 +181,19 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
             f2 C[5];
 #pragma unroll
             for (int m = 0; m < 5; ++m) C[m] = bc(0.f);
-            double H0a = 0.0, H0b = 0.0;
+            double H0a = 0.0, H0b = 0.0, Yta = 0.0, Ytb = 0.0;
             f2 sumx = bc(0.f);
 #pragma unroll
             for (int a = 0; a < KW; ++a) {
                 const int k = w + 4 * a;
                 const f2 y = yv[a];
-                const f2 x = mul2(y, sSmall[k * 24]);
+                const f2 x = mul2(y, sSmall[k * kSmallStride]);
                 sX[k * 32 + lane] = x;
                 sumx = add2(sumx, x);
+                if (D_o) {   // sum_j Y_j in fp64 (exact on fp32 inputs up to 1e-16): N_k = sum - Y_k without cancellation
+                    Yta += (double)y.x;
+                    Ytb += (double)y.y;
+                }
                 if (want_thermo) {
                     const float4 a = *reinterpret_cast<const float4*>(sTh + k * 12), b = *reinterpret_cast<const float4*>(sTh + k * 12 + 4),
                                  c = *reinterpret_cast<const float4*>(sTh + k * 12 + 8);   // lo c0..c5 | hi c0..c5
@@ -192,8 +209,12 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
                     }
                 }
             }
-            f2* my = sScr + (w * 12) * 32 + lane;
+            f2* my = sScr + (w * kScrSlots) * 32 + lane;
             my[0] = sumx;
+            if (D_o) {
+                reinterpret_cast<double*>(my)[11 * 32] = Yta;
+                reinterpret_cast<double*>(my)[12 * 32] = Ytb;
+            }
             if (want_thermo) {
 #pragma unroll
                 for (int m = 0; m < 5; ++m) my[(1 + m) * 32] = C[m];
@@ -204,14 +225,14 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
         __syncthreads();
         f2 sumx = bc(0.f);
 #pragma unroll
-        for (int v = 0; v < 4; ++v) sumx = add2(sumx, sScr[(v * 12) * 32 + lane]);
+        for (int v = 0; v < 4; ++v) sumx = add2(sumx, sScr[(v * kScrSlots) * 32 + lane]);
         if (want_thermo && w == 1) {
             f2 q[5];
 #pragma unroll
             for (int m = 0; m < 5; ++m) {
                 q[m] = bc(0.f);
 #pragma unroll
-                for (int v = 0; v < 4; ++v) q[m] = add2(q[m], sScr[(v * 12 + 1 + m) * 32 + lane]);
+                for (int v = 0; v < 4; ++v) q[m] = add2(q[m], sScr[(v * kScrSlots + 1 + m) * 32 + lane]);
             }
             if (cp_o)
                 st2(cp_o, mul2(fma2(fma2(fma2(fma2(mul2(q[4], 5.f), tau, mul2(q[3], 4.f)), tau, mul2(q[2], 3.f)), tau,
@@ -221,8 +242,8 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
                 double Ha = 0.0, Hb = 0.0;
 #pragma unroll
                 for (int v = 0; v < 4; ++v) {
-                    Ha += reinterpret_cast<const double*>(sScr + (v * 12) * 32 + lane)[6 * 32];
-                    Hb += reinterpret_cast<const double*>(sScr + (v * 12) * 32 + lane)[7 * 32];
+                    Ha += reinterpret_cast<const double*>(sScr + (v * kScrSlots) * 32 + lane)[6 * 32];
+                    Hb += reinterpret_cast<const double*>(sScr + (v * kScrSlots) * 32 + lane)[7 * 32];
                 }
                 const f2 sens = mul2(tau, fma2(fma2(fma2(fma2(q[4], tau, q[3]), tau, q[2]), tau, q[1]), tau, q[0]));
                 st2(h_o, make_float2((float)(Ha + (double)sens.x), (float)(Hb + (double)sens.y)));
@@ -243,14 +264,14 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
             for (int k = w; k < Kp; k += 4) {
                 const f2 X = mul2(sX[k * 32 + lane], inv_sumx);
                 sX[k * 32 + lane] = X;
-                const float4 a = *reinterpret_cast<const float4*>(sSmall + k * 24), b = *reinterpret_cast<const float4*>(sSmall + k * 24 + 4),
-                             c = *reinterpret_cast<const float4*>(sSmall + k * 24 + 8);   // invW sqrtW v0 v1 | v2 v3 v4 c0 | c1 c2 c3 c4
+                const float4 a = *reinterpret_cast<const float4*>(sSmall + k * kSmallStride), b = *reinterpret_cast<const float4*>(sSmall + k * kSmallStride + 4),
+                             c = *reinterpret_cast<const float4*>(sSmall + k * kSmallStride + 8);   // invW sqrtW v0 v1 | v2 v3 v4 c0 | c1 c2 c3 c4
                 sR[k * 32 + lane] = rcp2(poly4_2(a.z, a.w, b.x, b.y, b.z, u));
                 const f2 lk = poly4_2(b.w, c.x, c.y, c.z, c.w, u);
                 s1 = fma2(X, lk, s1);
                 s2 = fma2(X, rcp2(lk), s2);
             }
-            f2* my = sScr + (w * 12 + 8) * 32 + lane;   // slots 8, 9 (slot 0..7 may still be read by warp 1)
+            f2* my = sScr + (w * kScrSlots + 8) * 32 + lane;   // slots 8, 9 (slot 0..7 may still be read by warp 1)
             my[0] = s1;
             my[32] = s2;
         }
@@ -259,8 +280,8 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
             f2 s1 = bc(0.f), s2 = bc(0.f);
 #pragma unroll
             for (int v = 0; v < 4; ++v) {
-                s1 = add2(s1, sScr[(v * 12 + 8) * 32 + lane]);
-                s2 = add2(s2, sScr[(v * 12 + 9) * 32 + lane]);
+                s1 = add2(s1, sScr[(v * kScrSlots + 8) * 32 + lane]);
+                s2 = add2(s2, sScr[(v * kScrSlots + 9) * 32 + lane]);
             }
             st2(lam_o, mul2(mul2(sqrtT, 0.5f), add2(s1, rcp2(s2))));   // A6
         }
@@ -293,91 +314,87 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
             f2 acc = bc(0.f);
 #pragma unroll
             for (int a = 0; a < KW; ++a)
-                acc = fma2(mul2(mul2(sX[(k0 + a) * 32 + lane], sSmall[(k0 + a) * 24 + 1]), mul2(gk[a], gk[a])), rcp2(den[a]), acc);
-            sScr[(w * 12 + 10) * 32 + lane] = acc;
+                acc = fma2(mul2(mul2(sX[(k0 + a) * 32 + lane], sSmall[(k0 + a) * kSmallStride + 1]), mul2(gk[a], gk[a])), rcp2(den[a]), acc);
+            sScr[(w * kScrSlots + 10) * 32 + lane] = acc;
         }
         __syncthreads();   // every warp is done reading r: sR becomes the S accumulators
         if (mu_o && w == 0) {
             f2 acc = bc(0.f);
 #pragma unroll
-            for (int v = 0; v < 4; ++v) acc = add2(acc, sScr[(v * 12 + 10) * 32 + lane]);
+            for (int v = 0; v < 4; ++v) acc = add2(acc, sScr[(v * kScrSlots + 10) * 32 + lane]);
             st2(mu_o, mul2(sqrtT, acc));
         }
         if (!D_o) continue;   // block-uniform; the barrier above also protects the scratch
 
         // ---- phase 4: mixture-averaged diffusivities ---------------------------------------------------------------
         for (int k = w; k < Kp; k += 4) sR[k * 32 + lane] = bc(0.f);
-        float* ring = sRing + w * 2 * kTileFloats;
-        auto stage = [&](int round, int buf) {
-            if (md.sched_kt[round][w] >= 0) {
-                const float* src = md.dtile + (size_t)md.sched_tile[round][w] * kTileFloats;
-                for (int c16 = lane; c16 < kTileFloats / 4; c16 += 32) cp_async16(ring + buf * kTileFloats + 4 * c16, src + 4 * c16);
+        // the next group's Y rows on their way from HBM to L2 while this group's pair loops run
+        if (grp + gridDim.x < ngroups && (lane & 7) == 0) {
+            const long long in = (grp + gridDim.x) * kGroupCells + 2 * lane;
+            if (in < n) {
+#pragma unroll
+                for (int a = 0; a < KW; ++a)
+                    if (w + 4 * a < K) asm volatile("prefetch.global.L2 [%0];" ::"l"(Yg + (size_t)(w + 4 * a) * ld + in));
             }
+        }
+        constexpr int kTileFloats = TS * tile_row_floats(TS);
+        float* ring = sRing + w * 2 * kTileFloatsMax;
+        auto stage = [&](int round, int buf) {
+            const float* src = md.dtile + (size_t)tile_index(kSchedK[round][w], kSchedJ[round][w]) * kTileFloats;
+            for (int c16 = lane; c16 < kTileFloats / 4; c16 += 32) cp_async16(ring + buf * kTileFloatsMax + 4 * c16, src + 4 * c16);
             cp_async_commit();
         };
         stage(0, 0);
         __syncthreads();   // S is zeroed everywhere
-        for (int r = 0; r < md.n_rounds; ++r) {
-            if (r + 1 < md.n_rounds) stage(r + 1, (r + 1) & 1);
+        for (int r = 0; r < kRounds; ++r) {
+            if (r + 1 < kRounds) stage(r + 1, (r + 1) & 1);
             else cp_async_commit();
             cp_async_wait<1>();
             __syncwarp();
-            const int kt = md.sched_kt[r][w], jt = md.sched_jt[r][w];
-            if (kt >= 0) {   // warp-uniform
-                const float* coef = ring + (r & 1) * kTileFloats;
-                f2 Xk[8], Xj[8], Sk[8], Sj[8];
+            const int kt = kSchedK[r][w], jt = kSchedJ[r][w];
+            const float* coef = ring + (r & 1) * kTileFloatsMax;
+            f2 Xk[TS], Xj[TS], Sk[TS], Sj[TS];
 #pragma unroll
-                for (int a = 0; a < 8; ++a) {
-                    Xk[a] = sX[(kt * 8 + a) * 32 + lane];
-                    Xj[a] = sX[(jt * 8 + a) * 32 + lane];
-                    Sk[a] = Sj[a] = bc(0.f);
-                }
-                if (kt == jt) diff_tile<true>(coef, u, Xk, Xj, Sk, Sj);
-                else diff_tile<false>(coef, u, Xk, Xj, Sk, Sj);
-                // rows kt and jt of S belong to this warp alone in this round
+            for (int a = 0; a < TS; ++a) {
+                Xk[a] = sX[(kt * TS + a) * 32 + lane];
+                Xj[a] = sX[(jt * TS + a) * 32 + lane];
+                Sk[a] = Sj[a] = bc(0.f);
+            }
+            if (r >= 7) diff_tile<TS, true>(coef, u, Xk, Xj, Sk, Sj);    // block-uniform: the two diagonal rounds
+            else diff_tile<TS, false>(coef, u, Xk, Xj, Sk, Sj);
+            // tiles kt and jt of S belong to this warp alone in this round
 #pragma unroll
-                for (int a = 0; a < 8; ++a) sR[(kt * 8 + a) * 32 + lane] = add2(sR[(kt * 8 + a) * 32 + lane], Sk[a]);
-                if (kt != jt) {
+            for (int a = 0; a < TS; ++a) sR[(kt * TS + a) * 32 + lane] = add2(sR[(kt * TS + a) * 32 + lane], Sk[a]);
+            if (r < 7) {
 #pragma unroll
-                    for (int a = 0; a < 8; ++a) sR[(jt * 8 + a) * 32 + lane] = add2(sR[(jt * 8 + a) * 32 + lane], Sj[a]);
-                }
+                for (int a = 0; a < TS; ++a) sR[(jt * TS + a) * 32 + lane] = add2(sR[(jt * TS + a) * 32 + lane], Sj[a]);
             }
             __syncthreads();
         }
         cp_async_wait<0>();
 
-        // ---- final: D_k = N_k / S_k, species a = w and w + 4 of every tile ------------------------------------------
+        // ---- final: D_k = N_k / S_k for this warp's species k = w, w + 4, ... (its Y rows again: L2 hits) ------------
         {
-            const f2 scale = make_float2(T.x * sqrtT.x / p_cell.x, T.y * sqrtT.y / p_cell.y);
-            f2 TT[nt];   // tile totals of Y_j = X_j W_j sum(x)
 #pragma unroll
-            for (int t = 0; t < nt; ++t) {
-                TT[t] = bc(0.f);
+            for (int a = 0; a < KW; ++a) yv[a] = (w + 4 * a < K) ? ld2(Yg + (size_t)(w + 4 * a) * ld) : bc(0.f);
+            double ta = 0.0, tb = 0.0;
 #pragma unroll
-                for (int a = 0; a < 8; ++a) TT[t] = fma2(sX[(t * 8 + a) * 32 + lane], sSmall[(t * 8 + a) * 24 + 17], TT[t]);
+            for (int v = 0; v < 4; ++v) {
+                ta += reinterpret_cast<const double*>(sScr + (v * kScrSlots) * 32 + lane)[11 * 32];
+                tb += reinterpret_cast<const double*>(sScr + (v * kScrSlots) * 32 + lane)[12 * 32];
             }
+            const f2 scale = make_float2(T.x * sqrtT.x * rcp_approx(p_cell.x), T.y * sqrtT.y * rcp_approx(p_cell.y));
 #pragma unroll
-            for (int t = 0; t < nt; ++t) {
-                f2 others = bc(0.f);
-#pragma unroll
-                for (int t2 = 0; t2 < nt; ++t2)
-                    if (t2 != t) others = add2(others, TT[t2]);
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const int a = w + 4 * h, k = t * 8 + a;
-                    if (k < K) {
-                        f2 Nk = others;
-#pragma unroll
-                        for (int b = 0; b < 8; ++b)
-                            if (b != a) Nk = fma2(sX[(t * 8 + b) * 32 + lane], sSmall[(t * 8 + b) * 24 + 17], Nk);
-                        Nk = mul2(Nk, sumx);
-                        const f2 S = sR[k * 32 + lane];
-                        const float* dd = sSmall + k * 24 + 12;
-                        const f2 dk = poly4_2(dd[0], dd[1], dd[2], dd[3], dd[4], u);
-                        const f2 q = mul2(Nk, rcp2(make_float2(S.x > 0.f ? S.x : 1.f, S.y > 0.f ? S.y : 1.f)));
-                        const f2 Dk = make_float2(S.x > 0.f ? q.x : dk.x, S.y > 0.f ? q.y : dk.y);   // A7
-                        st2(D_o + (size_t)k * ld, mul2(Dk, scale));
-                    }
+            for (int a = 0; a < KW; ++a) {
+                const int k = w + 4 * a;
+                if (k < K) {
+                    const f2 Nk = make_float2((float)(ta - (double)yv[a].x), (float)(tb - (double)yv[a].y));
+                    const f2 S = sR[k * 32 + lane];
+                    const float* dd = sSmall + k * kSmallStride + 12;
+                    const f2 dk = poly4_2(dd[0], dd[1], dd[2], dd[3], dd[4], u);
+                    const f2 q = mul2(Nk, rcp2x(S));
+                    const f2 Dk = make_float2(S.x > 0.f ? q.x : dk.x, S.y > 0.f ? q.y : dk.y);   // A7
+                    st2(D_o + (size_t)k * ld, mul2(Dk, scale));
                 }
             }
         }
