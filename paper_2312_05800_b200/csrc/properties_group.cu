@@ -18,9 +18,9 @@
 //            the four warps add into the shared S accumulators without atomics and every round is balanced; two more
 //            rounds take the 8 diagonal tiles.  One block barrier per round.  A warp stages its own coefficient tile
 //            (<= 1280 B, in loop order) with cp.async one round ahead.
-//   final    D_k = N_k / S_k, N_k = sum_{j != k} Y_j evaluated as (sum_j Y_j) - Y_k IN FP64 on the exact fp32 Y (the
-//            fp32 form of that difference is the cancellation A7 warns of; in fp64 it is exact to 1e-16 sum Y),
-//            self-diffusion D_kk when S_k = 0.
+//   final    D_k = N_k / S_k, N_k = sum_{j != k} Y_j evaluated as (sum_j Y_j) - Y_k with the sum carried as an
+//            unevaluated float-float pair (TwoSum) over the exact fp32 Y: what A7 warns of is the rounding of the
+//            fp32 sum, amplified by the cancellation; the pair is exact to ~1e-14 sum Y.  Self-diffusion D_kk when S_k = 0.
 // A block is one group; it loops over groups (grid-stride) so the tables are staged once per block.
 #include "common.cuh"
 
@@ -40,6 +40,14 @@ __device__ __forceinline__ f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
 __device__ __forceinline__ f2 rcp2(f2 a) {
     const float r = rcp_approx(a.x * a.y);
     return make_float2(r * a.y, r * a.x);
+}
+// hi + lo += y with the rounding error of the addition kept (Knuth's TwoSum, packed for two cells)
+__device__ __forceinline__ void two_sum_acc(f2& hi, f2& lo, f2 y) {
+    const f2 s = add2(hi, y);
+    const f2 bb = add2(s, make_float2(-hi.x, -hi.y));
+    const f2 e = add2(add2(hi, make_float2(bb.x - s.x, bb.y - s.y)), add2(y, make_float2(-bb.x, -bb.y)));
+    hi = s;
+    lo = add2(lo, e);
 }
 // one MUFU per half: in the FMA-bound pair loop the XU pipe is idle and the three multiplies of rcp2 are not
 __device__ __forceinline__ f2 rcp2x(f2 a) { return make_float2(rcp_approx(a.x), rcp_approx(a.y)); }
@@ -77,7 +85,10 @@ __device__ __forceinline__ void diff_tile(const float* __restrict__ coef, f2 u, 
         }
 #pragma unroll
         for (int b = DIAG ? a + 1 : 0; b < TS; ++b) {
-            const f2 r = rcp2x(poly4_2(q[5 * b], q[5 * b + 1], q[5 * b + 2], q[5 * b + 3], q[5 * b + 4], u));
+            // both pipes at work: two MUFU (XU: 16 clk per pair and SMSP) for five pairs of eight, one MUFU + three
+            // FMUL (FMA pipe: +3 clk) for the rest -- ~13 clk per pair on either pipe
+            const f2 P = poly4_2(q[5 * b], q[5 * b + 1], q[5 * b + 2], q[5 * b + 3], q[5 * b + 4], u);
+            const f2 r = ((a * TS + b) % 8 < 5) ? rcp2x(P) : rcp2(P);
             Sk[a] = fma2(Xj[b], r, Sk[a]);
             if (DIAG) Sk[b] = fma2(Xk[a], r, Sk[b]);
             else Sj[b] = fma2(Xk[a], r, Sj[b]);
@@ -181,7 +192,8 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
             f2 C[5];
 #pragma unroll
             for (int m = 0; m < 5; ++m) C[m] = bc(0.f);
-            double H0a = 0.0, H0b = 0.0, Yta = 0.0, Ytb = 0.0;
+            double H0a = 0.0, H0b = 0.0;
+            f2 Yhi = bc(0.f), Ylo = bc(0.f);   // sum_j Y_j of this warp's species as an unevaluated float-float sum
             f2 sumx = bc(0.f);
 #pragma unroll
             for (int a = 0; a < KW; ++a) {
@@ -190,10 +202,7 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
                 const f2 x = mul2(y, sSmall[k * kSmallStride]);
                 sX[k * 32 + lane] = x;
                 sumx = add2(sumx, x);
-                if (D_o) {   // sum_j Y_j in fp64 (exact on fp32 inputs up to 1e-16): N_k = sum - Y_k without cancellation
-                    Yta += (double)y.x;
-                    Ytb += (double)y.y;
-                }
+                if (D_o) two_sum_acc(Yhi, Ylo, y);
                 if (want_thermo) {
                     const float4 a = *reinterpret_cast<const float4*>(sTh + k * 12), b = *reinterpret_cast<const float4*>(sTh + k * 12 + 4),
                                  c = *reinterpret_cast<const float4*>(sTh + k * 12 + 8);   // lo c0..c5 | hi c0..c5
@@ -212,8 +221,8 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
             f2* my = sScr + (w * kScrSlots) * 32 + lane;
             my[0] = sumx;
             if (D_o) {
-                reinterpret_cast<double*>(my)[11 * 32] = Yta;
-                reinterpret_cast<double*>(my)[12 * 32] = Ytb;
+                my[11 * 32] = Yhi;
+                my[12 * 32] = Ylo;
             }
             if (want_thermo) {
 #pragma unroll
@@ -297,7 +306,7 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
             }
             const float* bw = sBW + (size_t)w * Kp * 16;
 #pragma unroll 2
-            for (int j = 0; j < Kp; ++j) {
+            for (int j = 0; j < K; ++j) {   // padding species have X_j = 0: skipped
                 const f2 xj = sX[j * 32 + lane], rj = sR[j * 32 + lane];
                 const f2 xr = mul2(xj, rj);
                 const f2 b2 = add2(xr, xr), c = mul2(xr, rj);
@@ -377,18 +386,20 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
         {
 #pragma unroll
             for (int a = 0; a < KW; ++a) yv[a] = (w + 4 * a < K) ? ld2(Yg + (size_t)(w + 4 * a) * ld) : bc(0.f);
-            double ta = 0.0, tb = 0.0;
+            f2 thi = bc(0.f), tlo = bc(0.f);
 #pragma unroll
             for (int v = 0; v < 4; ++v) {
-                ta += reinterpret_cast<const double*>(sScr + (v * kScrSlots) * 32 + lane)[11 * 32];
-                tb += reinterpret_cast<const double*>(sScr + (v * kScrSlots) * 32 + lane)[12 * 32];
+                two_sum_acc(thi, tlo, sScr[(v * kScrSlots + 11) * 32 + lane]);
+                tlo = add2(tlo, sScr[(v * kScrSlots + 12) * 32 + lane]);
             }
             const f2 scale = make_float2(T.x * sqrtT.x * rcp_approx(p_cell.x), T.y * sqrtT.y * rcp_approx(p_cell.y));
 #pragma unroll
             for (int a = 0; a < KW; ++a) {
                 const int k = w + 4 * a;
                 if (k < K) {
-                    const f2 Nk = make_float2((float)(ta - (double)yv[a].x), (float)(tb - (double)yv[a].y));
+                    // (hi - Y_k) loses nothing that matters: an fp32 difference is exact to 2^-24 of its RESULT; what
+                    // cancellation would amplify is the rounding of the sum itself, and that sits in lo
+                    const f2 Nk = add2(add2(thi, make_float2(-yv[a].x, -yv[a].y)), tlo);
                     const f2 S = sR[k * 32 + lane];
                     const float* dd = sSmall + k * kSmallStride + 12;
                     const f2 dk = poly4_2(dd[0], dd[1], dd[2], dd[3], dd[4], u);
