@@ -14,6 +14,7 @@
 // The `#pragma omp parallel for` on the per-cell drivers is the only concession to speed:
 // cells are independent ("computation of thermal and transport properties" is
 // per cell; P:79 the ANN is applied per cell).
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -217,6 +218,65 @@ void cell_source(const Ann& a, const Mech& m, double T, double p, const double* 
     }
 }
 
+// ---- NEXT-4: solver-facing extras of the property pass -------------------------------------------
+// P:34-36 "computation of thermal and transport properties" for a compressible solver with non-unity Lewis numbers
+// ("Hirschfelder and Curtiss mixture-averaged transport"): besides cp, h, mu, lambda, D_k the transport
+// equations need rho, psi = d rho / d p at constant T, alpha = lambda / cp, rho D_k, the species enthalpies h_k(T)
+// of the diffusive enthalpy flux sum_k h_k J_k, and (for diagnostics) the mixture entropy.  Reading A22:
+//   rho = p Wbar / (R T)   psi = Wbar / (R T)   alpha = lambda / cp   (rho D)_k = rho D_k   h_k = h_k(T) / W_k  [J/kg]
+//   s = sum_k (Y_k / W_k) [ s_k(T) - R ln X_k ] - (R / Wbar) ln(p / p0),  p0 = 101325 Pa, terms with X_k = 0 drop out
+// (ideal-gas mixture: standard-state species entropies O1, entropy of mixing, pressure correction).
+constexpr double P0 = 101325.0;
+void cell_extras(const Mech& m, double T, double p, const double* Y, long long ld, double cp, double lam, const double* D,
+                 long long ldD, double* rho_o, double* psi_o, double* alpha_o, double* rhoD, double* hk, long long ldo,
+                 double* s_o) {
+    const int K = m.K;
+    double inv_Wbar = 0.0;
+    for (int k = 0; k < K; ++k) inv_Wbar += Y[k * ld] / m.W[k];
+    const double Wbar = 1.0 / inv_Wbar;
+    const double rho = p * Wbar / (R * T);
+    if (rho_o) *rho_o = rho;
+    if (psi_o) *psi_o = Wbar / (R * T);
+    if (alpha_o) *alpha_o = lam / cp;
+    double s = 0.0;
+    for (int k = 0; k < K; ++k) {
+        double hkm, sk;
+        species_thermo(m, k, T, nullptr, &hkm, &sk);
+        if (hk) hk[k * ldo] = hkm / m.W[k];
+        if (rhoD) rhoD[k * ldo] = rho * D[k * ldD];
+        const double X = (Y[k * ld] / m.W[k]) * Wbar;
+        if (X > 0.0) s += (Y[k * ld] / m.W[k]) * (sk - R * std::log(X));
+    }
+    s -= (R / Wbar) * std::log(p / P0);
+    if (s_o) *s_o = s;
+}
+
+// ---- NEXT-3: PaSR scaling of the ANN source and the temperature gate ------------------------------
+// P:113 "the PaSR combustion model wherein the characteristic chemical time is calculated as the slowest formation
+// rate of species and the mixing time scale is calculated as the geometric mean of the Taylor scale and the
+// Kolmogorov scale"; "a minimum temperature threshold of 500 K" (the ANN was never shown colder states).
+// The paper prints no formula.  Reading A23:
+//   tau_c   = max over species with |omega_k| > 0 of rho Y_k / |omega_k|      (slowest species time scale; 0 if none)
+//   tau_mix = sqrt( (k_sgs / eps) * sqrt(nu / eps) ),  nu = mu / rho           (Taylor x Kolmogorov time scales)
+//   kappa   = tau_c / (tau_c + tau_mix)   (0 when tau_c = 0);   omega_k <- kappa omega_k;   T < T_gate => omega_k <- 0
+void cell_pasr(const Mech& m, double T, double p, const double* Y, long long ld, double mu, double ksgs, double eps,
+               double T_gate, const double* om_in, double* om_out, long long ldo, double* kappa_o) {
+    const int K = m.K;
+    double inv_Wbar = 0.0;
+    for (int k = 0; k < K; ++k) inv_Wbar += Y[k * ld] / m.W[k];
+    const double rho = p / (inv_Wbar * R * T);
+    double tau_c = 0.0;
+    for (int k = 0; k < K; ++k) {
+        const double w = std::fabs(om_in[k * ldo]);
+        if (w > 0.0) tau_c = std::max(tau_c, rho * Y[k * ld] / w);
+    }
+    const double tau_mix = std::sqrt((ksgs / eps) * std::sqrt((mu / rho) / eps));
+    double kappa = tau_c > 0.0 ? tau_c / (tau_c + tau_mix) : 0.0;
+    if (T < T_gate) kappa = 0.0;
+    for (int k = 0; k < K; ++k) om_out[k * ldo] = kappa * om_in[k * ldo];
+    if (kappa_o) *kappa_o = kappa;
+}
+
 }  // namespace
 
 extern "C" {
@@ -336,6 +396,27 @@ void oracle_ann_source(const void* av, const void* mv, long long n, long long ld
 #pragma omp parallel for schedule(static)
     for (long long i = 0; i < n; ++i)
         cell_source(a, m, T[i], p[i], Y + i, ld, omega ? omega + i : nullptr, dY ? dY + i : nullptr, ld);
+}
+
+void oracle_extras(const void* mv, long long n, long long ld, const double* T, const double* p, const double* Y,
+                   const double* cp, const double* lam, const double* D, double* rho, double* psi, double* alpha,
+                   double* rhoD, double* hk, double* s) {
+    const Mech& m = *static_cast<const Mech*>(mv);
+#pragma omp parallel for schedule(static)
+    for (long long i = 0; i < n; ++i)
+        cell_extras(m, T[i], p[i], Y + i, ld, cp ? cp[i] : 1.0, lam ? lam[i] : 0.0, D ? D + i : nullptr, ld,
+                    rho ? &rho[i] : nullptr, psi ? &psi[i] : nullptr, (alpha && cp && lam) ? &alpha[i] : nullptr,
+                    (rhoD && D) ? rhoD + i : nullptr, hk ? hk + i : nullptr, ld, s ? &s[i] : nullptr);
+}
+
+void oracle_pasr(const void* mv, long long n, long long ld, const double* T, const double* p, const double* Y,
+                 const double* mu, const double* ksgs, const double* eps, double T_gate, const double* om_in,
+                 double* om_out, double* kappa) {
+    const Mech& m = *static_cast<const Mech*>(mv);
+#pragma omp parallel for schedule(static)
+    for (long long i = 0; i < n; ++i)
+        cell_pasr(m, T[i], p[i], Y + i, ld, mu[i], ksgs[i], eps[i], T_gate, om_in + i, om_out + i, ld,
+                  kappa ? &kappa[i] : nullptr);
 }
 
 }  // extern "C"

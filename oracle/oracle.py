@@ -69,6 +69,8 @@ def lib():
             f.argtypes = [d, d]
         _lib.oracle_gelu.restype = d
         _lib.oracle_gelu.argtypes = [d]
+        _lib.oracle_extras.argtypes = [vp, ll, ll] + [P] * 12
+        _lib.oracle_pasr.argtypes = [vp, ll, ll, P, P, P, P, P, P, d, P, P, P]
         _lib.oracle_ann_features.argtypes = [vp, ll, ll, P, P, P, P]
         _lib.oracle_mlp_forward.argtypes = [vp, ll, P, P]
         _lib.oracle_ann_source.argtypes = [vp, vp, ll, ll, P, P, P, P, P]
@@ -151,6 +153,37 @@ class Mech:
         D = np.zeros((self.K, ld))
         lib().oracle_properties(self.h, n, ld, _p(T), _p(p), _p(Y), _p(cp), _p(h), _p(mu), _p(lam), _p(D))
         return dict(cp=cp, h=h, mu=mu, lam=lam, D=D)
+
+
+    # --- NEXT-4 (A22): rho, psi, alpha, rho D_k, h_k(T), s
+    def extras(self, T, p, Y, cp=None, lam=None, D=None):
+        T, Y, n, ld = self._fields(T, Y)
+        p = _f64(p)
+        cp = None if cp is None else _f64(cp)
+        lam = None if lam is None else _f64(lam)
+        D = None if D is None else _f64(D)
+        rho, psi, alpha, s = (np.empty(n) for _ in range(4))
+        rhoD, hk = np.zeros((self.K, ld)), np.zeros((self.K, ld))
+        lib().oracle_extras(self.h, n, ld, _p(T), _p(p), _p(Y), _p(cp), _p(lam), _p(D), _p(rho), _p(psi), _p(alpha),
+                            _p(rhoD), _p(hk), _p(s))
+        out = dict(rho=rho, psi=psi, hk=hk, s=s)
+        if cp is not None and lam is not None:
+            out["alpha"] = alpha
+        if D is not None:
+            out["rhoD"] = rhoD
+        return out
+
+    # --- NEXT-3 (A23): PaSR scaling + temperature gate
+    def pasr(self, T, p, Y, mu, ksgs, eps, T_gate, omega):
+        T, Y, n, ld = self._fields(T, Y)
+        p, mu, ksgs, eps = (_f64(x) for x in (p, mu, ksgs, eps))
+        om = _f64(omega)
+        assert om.shape == Y.shape
+        out = np.zeros_like(om)
+        kappa = np.empty(n)
+        lib().oracle_pasr(self.h, n, ld, _p(T), _p(p), _p(Y), _p(mu), _p(ksgs), _p(eps), float(T_gate), _p(om), _p(out),
+                          _p(kappa))
+        return out, kappa
 
 
 class Ann:
