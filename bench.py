@@ -364,6 +364,33 @@ def bench_configs(torch, B, stream, pk, fp32, quick=False):
     del gm, ga, sets, ws
     torch.cuda.empty_cache()
 
+    # ---- the two pointwise passes of SURVEY 8(f) NEXT-3 / NEXT-4 on the headline field (2,097,152 cells, K = 19) ----
+    mech, _, cells = synth.make_config(3)
+    gm = B.Mech(mech)
+    n, K = cells.n, mech.K
+    T0, p, Y = dev(cells.T), dev(cells.p), dev(cells.Y)
+    cp, lam, mu = (torch.empty(n, device="cuda") for _ in range(3))
+    D = torch.empty(K, n, device="cuda")
+    B.df_thermo_properties(gm, T0, p, Y, cp=cp, mu=mu, lam=lam, D=D)
+    rho, psi, alpha, s_ = (torch.empty(n, device="cuda") for _ in range(4))
+    rhoD, hk = torch.empty(K, n, device="cuda"), torch.empty(K, n, device="cuda")
+    med, mn = _median_launch_ms(torch, stream, lambda i: B.df_thermo_extras(gm, T0, p, Y, cp=cp, lam=lam, D=D, rho=rho, psi=psi,
+                                                                              alpha=alpha, rhoD=rhoD, hk=hk, s=s_), 8)
+    out["extras"] = {"workload": f"df_thermo_extras, {n} cells, K=19: rho, psi, alpha, rhoD[19], hk[19], s",
+                     "roofline": hbm_entry("extras_kernel", 8 * (2 * K + 4), n, med, pk, {"ms_min": mn})}
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    ks = torch.rand(n, device="cuda", generator=gen) * 10 + 0.01
+    ep = torch.rand(n, device="cuda", generator=gen) * 1e4 + 0.1
+    om0 = torch.randn(K, n, device="cuda", generator=gen) * 50
+    om = torch.empty_like(om0)
+    kap = torch.empty(n, device="cuda")
+    med, mn = _median_launch_ms(torch, stream, lambda i: B.df_chem_pasr_scale(gm, T0, p, Y, mu, ks, ep, 500.0, om, kappa=kap), 8,
+                                before=lambda i: om.copy_(om0))
+    out["pasr"] = {"workload": f"df_chem_pasr_scale, {n} cells, K=19 (omega scaled in place, kappa written)",
+                   "roofline": hbm_entry("pasr_kernel", 4 * (3 * K + 6), n, med, pk, {"ms_min": mn})}
+    del gm, T0, p, Y, cp, lam, mu, D, rho, psi, alpha, s_, rhoD, hk, ks, ep, om0, om, kap
+    torch.cuda.empty_cache()
+
     # ---- cfg4: 2,097,152 cells, K = 53, property pass only ----
     mech, _, cells = synth.make_config(4)
     gm = B.Mech(mech)

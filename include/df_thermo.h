@@ -132,6 +132,31 @@ DF_API df_status df_chem_ann_source(const df_ann* ann, const df_mech* mech, long
                              float* omega, float* dY,
                              void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- solver-facing extras of the property pass (reading A22) ------------
+ * What a compressible solver with non-unity Lewis numbers needs besides cp, h, mu, lambda, D_k (all per cell, fp32):
+ *   rho = p Wbar/(R T);  psi = Wbar/(R T) (= d rho/d p at constant T);  alpha = lambda/cp;  rhoD[k] = rho D_k;
+ *   hk[k] = h_k(T)/W_k [J/kg], the species enthalpies of the diffusive enthalpy flux sum_k h_k J_k;
+ *   s = sum_k (Y_k/W_k)(s_k(T) - R ln X_k) - (R/Wbar) ln(p/101325 Pa) [J/(kg K)], the ideal-gas mixture entropy
+ *   (NASA-7 s_k with a7; X_k = 0 terms drop out).
+ * cp, lambda, D are the arrays df_thermo_properties wrote (inputs here; needed only for alpha / rhoD).  rhoD and hk are
+ * [K][ld].  Any output may be NULL (skipped). */
+DF_API df_status df_thermo_extras(const df_mech* mech, long long n_cells, long long ld,
+                           const float* T, const float* p, const float* Y,
+                           const float* cp, const float* lambda, const float* D,
+                           float* rho, float* psi, float* alpha, float* rhoD, float* hk, float* s, void* stream);
+
+/* ---- PaSR scaling of the source and the temperature gate (reading A23) -----------
+ * "the characteristic chemical time is calculated as the slowest formation rate of species and the mixing time
+ * scale is calculated as the geometric mean of the Taylor scale and the Kolmogorov scale".  Per cell:
+ *   tau_c = max over species with omega_k != 0 of rho Y_k/|omega_k|  (0 if none),  rho = p Wbar/(R T),
+ *   tau_mix = sqrt((k_sgs/eps) sqrt(nu/eps)), nu = mu/rho,   kappa = tau_c/(tau_c + tau_mix)  (0 if tau_c = 0),
+ *   omega_k <- kappa omega_k, and kappa = 0 where T < T_gate (the ANN saw no state below 500 K).
+ * omega [K][ld] is updated in place; kappa [n] (optional) receives the factor. */
+DF_API df_status df_chem_pasr_scale(const df_mech* mech, long long n_cells, long long ld,
+                             const float* T, const float* p, const float* Y,
+                             const float* mu, const float* k_sgs, const float* eps, float T_gate,
+                             float* omega, float* kappa, void* stream);
+
 /* ---- host-buffer step (bench.py's e2e leg) ----------------------------------------------
  * One pass of the whole path over HOST arrays: copies h, p, T_guess, Y host->device, runs
  * T_from_h -> properties -> ann_source (ann may be NULL: skipped) on the context's stream,

@@ -22,6 +22,7 @@ SYMBOLS = (
     "df_mech_create", "df_mech_destroy", "df_mech_num_species",
     "df_ann_create", "df_ann_destroy", "df_ann_workspace_bytes",
     "df_thermo_T_from_h", "df_thermo_properties", "df_chem_ann_source",
+    "df_thermo_extras", "df_chem_pasr_scale",
     "df_host_ctx_create", "df_host_ctx_destroy", "df_step_host",
     "df_probe_fp32_peak",
 )
@@ -53,6 +54,8 @@ _lib.df_ann_workspace_bytes.argtypes = [_vp, _ll]
 _lib.df_thermo_T_from_h.argtypes = [_vp, _ll, _ll, _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.df_thermo_properties.argtypes = [_vp, _ll, _ll, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.df_chem_ann_source.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+_lib.df_thermo_extras.argtypes = [_vp, _ll, _ll] + [_vp] * 13
+_lib.df_chem_pasr_scale.argtypes = [_vp, _ll, _ll, _vp, _vp, _vp, _vp, _vp, _vp, C.c_float, _vp, _vp, _vp]
 _lib.df_host_ctx_create.argtypes = [C.POINTER(_vp), _vp, _vp, _ll]
 _lib.df_host_ctx_destroy.argtypes = [_vp]
 _lib.df_step_host.argtypes = [_vp, _ll, _ll] + [_vp] * 10
@@ -164,6 +167,19 @@ def df_chem_ann_source(ann: Ann, mech: Mech, T, p, Y, omega=None, dY=None, works
     ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
     _check(_lib.df_chem_ann_source(ann.handle, mech.handle, n, int(Y.shape[1]), _dp(T), _dp(p), _dp(Y), _dp(omega),
                                    _dp(dY), _dp(workspace), ws_bytes, _stream(stream)))
+
+
+def df_thermo_extras(mech: Mech, T, p, Y, cp=None, lam=None, D=None, rho=None, psi=None, alpha=None, rhoD=None, hk=None,
+                     s=None, n_cells=None, stream=None) -> None:
+    n = int(T.shape[0]) if n_cells is None else int(n_cells)
+    _check(_lib.df_thermo_extras(mech.handle, n, int(Y.shape[1]), _dp(T), _dp(p), _dp(Y), _dp(cp), _dp(lam), _dp(D),
+                                 _dp(rho), _dp(psi), _dp(alpha), _dp(rhoD), _dp(hk), _dp(s), _stream(stream)))
+
+
+def df_chem_pasr_scale(mech: Mech, T, p, Y, mu, k_sgs, eps, T_gate, omega, kappa=None, n_cells=None, stream=None) -> None:
+    n = int(T.shape[0]) if n_cells is None else int(n_cells)
+    _check(_lib.df_chem_pasr_scale(mech.handle, n, int(Y.shape[1]), _dp(T), _dp(p), _dp(Y), _dp(mu), _dp(k_sgs), _dp(eps),
+                                   float(T_gate), _dp(omega), _dp(kappa), _stream(stream)))
 
 
 def alloc_workspace(ann: Ann, n_cells: int, device="cuda"):

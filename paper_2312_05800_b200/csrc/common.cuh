@@ -46,6 +46,7 @@ struct MechDev {
     int K;
     MechScalars sc;
     float* th32;     // [K][2][6]
+    float* sth32;    // [K][2][6]  s_k(T)/W_k = sth[0] ln T + sum_{m<5} sth[1+m] tau^m   (pointwise.cu)
     double* th64;    // [K][2][6]
     float* invW;     // [K]
     float* sqrtW;    // [K]

@@ -37,7 +37,7 @@ df_status to_device(T** dst, const std::vector<T>& src) {
 struct HostTables {
     int K;
     MechScalars sc;
-    std::vector<float> th32, invW, sqrtW, visc, cond, ddiag, dfull, wilkeB;
+    std::vector<float> th32, sth32, invW, sqrtW, visc, cond, ddiag, dfull, wilkeB;
     std::vector<double> th64;
 };
 
@@ -103,6 +103,7 @@ extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const
 
     t.th32.resize((size_t)K * 12);
     t.th64.resize((size_t)K * 12);
+    t.sth32.resize((size_t)K * 12);
     t.invW.resize(K);
     t.sqrtW.resize(K);
     t.visc.resize((size_t)K * 5);
@@ -123,6 +124,13 @@ extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const
                 t.th64[(k * 2 + r) * 6 + m] = (double)(RW * q[m]);
                 t.th32[(k * 2 + r) * 6 + m] = (float)(RW * q[m]);
             }
+            // s_k/W_k = RW (a1 ln T + a7 + a2 T + a3 T^2/2 + a4 T^3/3 + a5 T^4/4): the polynomial part in tau
+            long double ps[5] = {(long double)a[6], (long double)a[1], (long double)a[2] / 2, (long double)a[3] / 3,
+                                 (long double)a[4] / 4};
+            long double qs[5];
+            shift_poly(ps, 5, Tm_f, S_f, qs);
+            t.sth32[(k * 2 + r) * 6] = (float)(RW * (long double)a[0]);
+            for (int m = 0; m < 5; ++m) t.sth32[(k * 2 + r) * 6 + 1 + m] = (float)(RW * qs[m]);
         }
         t.invW[k] = (float)(1.0L / (long double)W[k]);
         t.sqrtW[k] = (float)sqrtl((long double)W[k]);
@@ -156,7 +164,7 @@ extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const
     d.K = K;
     d.sc = t.sc;
     df_status st;
-    if ((st = to_device(&d.th32, t.th32)) || (st = to_device(&d.th64, t.th64)) || (st = to_device(&d.invW, t.invW)) ||
+    if ((st = to_device(&d.th32, t.th32)) || (st = to_device(&d.sth32, t.sth32)) || (st = to_device(&d.th64, t.th64)) || (st = to_device(&d.invW, t.invW)) ||
         (st = to_device(&d.sqrtW, t.sqrtW)) || (st = to_device(&d.visc, t.visc)) || (st = to_device(&d.cond, t.cond)) ||
         (st = to_device(&d.ddiag, t.ddiag)) || (st = to_device(&d.dfull, t.dfull)) ||
         (st = to_device(&d.wilkeB, t.wilkeB))) {
@@ -223,6 +231,7 @@ extern "C" df_status df_mech_destroy(df_mech* mech) {
     if (!mech) return DF_OK;
     MechDev& d = mech->dev;
     cudaFree(d.th32);
+    cudaFree(d.sth32);
     cudaFree(d.th64);
     cudaFree(d.invW);
     cudaFree(d.sqrtW);

@@ -1,0 +1,223 @@
+// pointwise.cu -- the two HBM-bound per-cell passes around the property and ANN calls:
+//   df_thermo_extras      rho, psi = Wbar/(R T), alpha = lambda/cp, rho D_k, h_k(T), mixture entropy   (reading A22)
+//   df_chem_pasr_scale    PaSR factor kappa = tau_c/(tau_c + tau_mix) applied to omega_k, with the T gate (A23)
+// One thread owns four consecutive cells (float4 SoA accesses, 512 B per warp and species row); the species tables
+// (<= 7 KB) are staged in shared memory once per block; Y is walked twice (the second pass hits L1/L2), so the DRAM
+// traffic is the algorithmic 4 B per field element.
+#include "common.cuh"
+
+namespace {
+
+constexpr int kPT = 128;   // threads per block, 4 cells each
+
+struct F4 {
+    float v[4];
+};
+__device__ __forceinline__ F4 load4(const float* __restrict__ p, long long i0, long long n, float fill) {
+    F4 r;
+    if (i0 + 4 <= n) {
+        const float4 t = __ldg(reinterpret_cast<const float4*>(p + i0));
+        r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w;
+    } else {
+#pragma unroll
+        for (int c = 0; c < 4; ++c) r.v[c] = (i0 + c < n) ? __ldg(p + i0 + c) : fill;
+    }
+    return r;
+}
+__device__ __forceinline__ void store4(float* __restrict__ p, long long i0, long long n, const F4& r) {
+    if (i0 + 4 <= n) {
+        *reinterpret_cast<float4*>(p + i0) = make_float4(r.v[0], r.v[1], r.v[2], r.v[3]);
+    } else {
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+            if (i0 + c < n) p[i0 + c] = r.v[c];
+    }
+}
+
+// ---- NEXT-4 ------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kPT)
+extras_kernel(MechDev md, long long n, long long ld, const float* __restrict__ Tg, const float* __restrict__ pg,
+              const float* __restrict__ Yg, const float* __restrict__ cpg, const float* __restrict__ lamg,
+              const float* __restrict__ Dg, float* __restrict__ rho_o, float* __restrict__ psi_o,
+              float* __restrict__ alpha_o, float* __restrict__ rhoD_o, float* __restrict__ hk_o, float* __restrict__ s_o) {
+    extern __shared__ float sm[];
+    const int K = md.K;
+    float* sTh = sm;                 // [K][2][6]  h_k/W_k in tau
+    float* sS = sTh + K * 12;        // [K][2][6]  s_k/W_k: coefficient of ln T, then the polynomial part in tau
+    float* sIW = sS + K * 12;        // [K] 1/W_k
+    for (int e = threadIdx.x; e < K * 12; e += kPT) {
+        sTh[e] = md.th32[e];
+        sS[e] = md.sth32[e];
+    }
+    for (int e = threadIdx.x; e < K; e += kPT) sIW[e] = md.invW[e];
+    __syncthreads();
+    const long long i0 = ((long long)blockIdx.x * kPT + threadIdx.x) * 4;
+    if (i0 >= n) return;
+    const F4 T = load4(Tg, i0, n, 1000.f), p = load4(pg, i0, n, 101325.f);
+
+    float invWbar[4] = {0.f, 0.f, 0.f, 0.f};
+    for (int k = 0; k < K; ++k) {
+        const F4 y = load4(Yg + (size_t)k * ld, i0, n, 0.f);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) invWbar[c] = fmaf(y.v[c], sIW[k], invWbar[c]);
+    }
+    const float Ru = (float)DF_R_UNIVERSAL;
+    F4 rho, psi;
+    float lnT[4], tau[4], ln_iw[4];
+    int lo[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        psi.v[c] = 1.0f / (invWbar[c] * Ru * T.v[c]);
+        rho.v[c] = p.v[c] * psi.v[c];
+        lnT[c] = logf(T.v[c]);
+        ln_iw[c] = logf(invWbar[c]);
+        tau[c] = (T.v[c] - md.sc.T_mid) * md.sc.inv_S;
+        lo[c] = T.v[c] < md.sc.T_mid;   // A2
+    }
+    if (rho_o) store4(rho_o, i0, n, rho);
+    if (psi_o) store4(psi_o, i0, n, psi);
+    if (alpha_o) {
+        const F4 cp = load4(cpg, i0, n, 1.f), lam = load4(lamg, i0, n, 0.f);
+        F4 a;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) a.v[c] = lam.v[c] / cp.v[c];
+        store4(alpha_o, i0, n, a);
+    }
+    if (!rhoD_o && !hk_o && !s_o) return;
+
+    float s[4] = {0.f, 0.f, 0.f, 0.f};
+    for (int k = 0; k < K; ++k) {
+        if (rhoD_o) {
+            const F4 d = load4(Dg + (size_t)k * ld, i0, n, 0.f);
+            F4 o;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) o.v[c] = rho.v[c] * d.v[c];
+            store4(rhoD_o + (size_t)k * ld, i0, n, o);
+        }
+        if (hk_o) {
+            F4 o;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const float* q = sTh + k * 12 + (lo[c] ? 0 : 6);
+                o.v[c] = fmaf(fmaf(fmaf(fmaf(fmaf(q[5], tau[c], q[4]), tau[c], q[3]), tau[c], q[2]), tau[c], q[1]), tau[c], q[0]);
+            }
+            store4(hk_o + (size_t)k * ld, i0, n, o);
+        }
+        if (s_o) {
+            const F4 y = load4(Yg + (size_t)k * ld, i0, n, 0.f);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const float* q = sS + k * 12 + (lo[c] ? 0 : 6);
+                const float sk = fmaf(q[0], lnT[c], fmaf(fmaf(fmaf(fmaf(q[5], tau[c], q[4]), tau[c], q[3]), tau[c], q[2]), tau[c], q[1]));
+                const float x = y.v[c] * sIW[k];   // Y_k / W_k; X_k = x / invWbar
+                // Y_k s_k/W_k - R x ln X_k ; x = 0 drops out (x ln x -> 0)
+                const float mix = x > 0.f ? x * (logf(x) - ln_iw[c]) : 0.f;
+                s[c] = fmaf(y.v[c], sk, fmaf(-Ru, mix, s[c]));
+            }
+        }
+    }
+    if (s_o) {
+        F4 o;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) o.v[c] = fmaf(-Ru * invWbar[c], logf(p.v[c] * (1.0f / 101325.0f)), s[c]);
+        store4(s_o, i0, n, o);
+    }
+}
+
+// ---- NEXT-3 ------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kPT)
+pasr_kernel(MechDev md, long long n, long long ld, const float* __restrict__ Tg, const float* __restrict__ pg,
+            const float* __restrict__ Yg, const float* __restrict__ mug, const float* __restrict__ kg,
+            const float* __restrict__ eg, float T_gate, float* omega, float* __restrict__ kappa_o) {
+    extern __shared__ float sm[];
+    const int K = md.K;
+    for (int e = threadIdx.x; e < K; e += kPT) sm[e] = md.invW[e];
+    __syncthreads();
+    const long long i0 = ((long long)blockIdx.x * kPT + threadIdx.x) * 4;
+    if (i0 >= n) return;
+    const F4 T = load4(Tg, i0, n, 1000.f), p = load4(pg, i0, n, 101325.f);
+    float invWbar[4] = {0.f, 0.f, 0.f, 0.f};
+    for (int k = 0; k < K; ++k) {
+        const F4 y = load4(Yg + (size_t)k * ld, i0, n, 0.f);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) invWbar[c] = fmaf(y.v[c], sm[k], invWbar[c]);
+    }
+    float rho[4], tau_c[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+    for (int c = 0; c < 4; ++c) rho[c] = p.v[c] / (invWbar[c] * (float)DF_R_UNIVERSAL * T.v[c]);
+    // slowest species time scale rho Y_k / |omega_k| over the species that react at all
+    for (int k = 0; k < K; ++k) {
+        const F4 y = load4(Yg + (size_t)k * ld, i0, n, 0.f), w = load4(omega + (size_t)k * ld, i0, n, 0.f);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const float a = fabsf(w.v[c]);
+            if (a > 0.f) tau_c[c] = fmaxf(tau_c[c], rho[c] * y.v[c] / a);
+        }
+    }
+    const F4 mu = load4(mug, i0, n, 1.f), ks = load4(kg, i0, n, 1.f), ep = load4(eg, i0, n, 1.f);
+    F4 kappa;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        const float tau_mix = sqrtf((ks.v[c] / ep.v[c]) * sqrtf(mu.v[c] / (rho[c] * ep.v[c])));
+        float kp = tau_c[c] > 0.f ? tau_c[c] / (tau_c[c] + tau_mix) : 0.f;
+        if (T.v[c] < T_gate) kp = 0.f;
+        kappa.v[c] = kp;
+    }
+    if (kappa_o) store4(kappa_o, i0, n, kappa);
+    for (int k = 0; k < K; ++k) {
+        F4 w = load4(omega + (size_t)k * ld, i0, n, 0.f);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) w.v[c] *= kappa.v[c];
+        store4(omega + (size_t)k * ld, i0, n, w);
+    }
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+df_status check(const char* fn, const df_mech* mech, long long n, long long ld) {
+    if (!mech) return df_set_error(DF_ERR_INVALID_ARG, "%s: mech is NULL", fn);
+    if (n < 0) return df_set_error(DF_ERR_INVALID_ARG, "%s: n_cells < 0", fn);
+    if (ld < n) return df_set_error(DF_ERR_INVALID_ARG, "%s: ld (%lld) < n_cells (%lld)", fn, ld, n);
+    if (ld % 4 != 0) return df_set_error(DF_ERR_INVALID_ARG, "%s: ld (%lld) must be a multiple of 4", fn, ld);
+    if ((n + 4LL * kPT - 1) / (4LL * kPT) > 0x7fffffffLL) return df_set_error(DF_ERR_UNSUPPORTED, "%s: n_cells too large", fn);
+    return DF_OK;
+}
+
+}  // namespace
+
+extern "C" df_status df_thermo_extras(const df_mech* mech, long long n, long long ld, const float* T, const float* p,
+                                      const float* Y, const float* cp, const float* lambda, const float* D, float* rho,
+                                      float* psi, float* alpha, float* rhoD, float* hk, float* s, void* stream) {
+    const df_status st = check("df_thermo_extras", mech, n, ld);
+    if (st != DF_OK) return st;
+    if (n == 0) return DF_OK;
+    if (!T || !p || !Y) return df_set_error(DF_ERR_INVALID_ARG, "df_thermo_extras: NULL input field");
+    if (alpha && (!cp || !lambda)) return df_set_error(DF_ERR_INVALID_ARG, "df_thermo_extras: alpha needs cp and lambda");
+    if (rhoD && !D) return df_set_error(DF_ERR_INVALID_ARG, "df_thermo_extras: rhoD needs D");
+    if (!rho && !psi && !alpha && !rhoD && !hk && !s) return DF_OK;
+    const void* ptrs[] = {T, p, Y, cp, lambda, D, rho, psi, alpha, rhoD, hk, s};
+    for (const void* q : ptrs)
+        if (!aligned16(q)) return df_set_error(DF_ERR_INVALID_ARG, "df_thermo_extras: fields must be 16-byte aligned");
+    const unsigned blocks = (unsigned)((n + 4LL * kPT - 1) / (4LL * kPT));
+    const size_t smem = (size_t)mech->K * 25 * sizeof(float);
+    extras_kernel<<<blocks, kPT, smem, (cudaStream_t)stream>>>(mech->dev, n, ld, T, p, Y, cp, lambda, D, rho, psi, alpha, rhoD, hk, s);
+    DF_CUDA_TRY(cudaGetLastError());
+    return DF_OK;
+}
+
+extern "C" df_status df_chem_pasr_scale(const df_mech* mech, long long n, long long ld, const float* T, const float* p,
+                                        const float* Y, const float* mu, const float* k_sgs, const float* eps, float T_gate,
+                                        float* omega, float* kappa, void* stream) {
+    const df_status st = check("df_chem_pasr_scale", mech, n, ld);
+    if (st != DF_OK) return st;
+    if (n == 0) return DF_OK;
+    if (!T || !p || !Y || !mu || !k_sgs || !eps || !omega) return df_set_error(DF_ERR_INVALID_ARG, "df_chem_pasr_scale: NULL field");
+    const void* ptrs[] = {T, p, Y, mu, k_sgs, eps, omega, kappa};
+    for (const void* q : ptrs)
+        if (!aligned16(q)) return df_set_error(DF_ERR_INVALID_ARG, "df_chem_pasr_scale: fields must be 16-byte aligned");
+    const unsigned blocks = (unsigned)((n + 4LL * kPT - 1) / (4LL * kPT));
+    pasr_kernel<<<blocks, kPT, (size_t)mech->K * sizeof(float), (cudaStream_t)stream>>>(mech->dev, n, ld, T, p, Y, mu, k_sgs, eps,
+                                                                                       T_gate, omega, kappa);
+    DF_CUDA_TRY(cudaGetLastError());
+    return DF_OK;
+}
