@@ -218,6 +218,41 @@ void cell_source(const Ann& a, const Mech& m, double T, double p, const double* 
     }
 }
 
+// ---- NEXT-1: one MLP per species --------------------------------------------------------------------
+// P:79 "individual training and prediction are carried out for each species mass fraction" ("multiple multilayer
+// perceptrons"): K independent networks (K+2) -> ... -> 1 share the input vector x = {T, p, F(Y)} (O9) and each
+// predicts the z-scored Box-Cox-space change of ITS species: Delta_k = s^u_k o^(k) + m^u_k (A9).  Everything after the
+// networks is O11/O12 exactly as in cell_source (inverse Box-Cox with base clamp A10, Y' = Y*/sum Y* A11, ideal-gas
+// rho A17).  nets[k] is an Ann with dims[0] = K + 2 and one output; its x_mean/x_std are the shared input statistics
+// (taken from nets[0]), its u_mean[0]/u_std[0] are species k's.
+void cell_source_mmlp(const Ann* const* nets, const Mech& m, double T, double p, const double* Y, long long ld,
+                      double* omega, double* dY, long long ldo) {
+    const int K = m.K;
+    const Ann& a0 = *nets[0];
+    std::vector<double> f(K + 2), Ys(K);
+    f[0] = (T - a0.x_mean[0]) / a0.x_std[0];
+    f[1] = (p - a0.x_mean[1]) / a0.x_std[1];
+    for (int k = 0; k < K; ++k) f[2 + k] = (boxcox(Y[k * ld], a0.lambda) - a0.x_mean[2 + k]) / a0.x_std[2 + k];
+    double S = 0.0;
+    for (int k = 0; k < K; ++k) {
+        double o;
+        mlp_forward(*nets[k], f.data(), &o);
+        const double delta = nets[k]->u_std[0] * o + nets[k]->u_mean[0];
+        double base = std::pow(Y[k * ld], a0.lambda) + a0.lambda * delta;
+        if (base < 0.0) base = 0.0;
+        Ys[k] = std::pow(base, 1.0 / a0.lambda);
+        S += Ys[k];
+    }
+    double inv_Wbar = 0.0;
+    for (int k = 0; k < K; ++k) inv_Wbar += Y[k * ld] / m.W[k];
+    const double rho = p / (inv_Wbar * R * T);
+    for (int k = 0; k < K; ++k) {
+        const double d = Ys[k] / S - Y[k * ld];
+        if (dY) dY[k * ldo] = d;
+        if (omega) omega[k * ldo] = rho * d / a0.dt;
+    }
+}
+
 // ---- NEXT-4: solver-facing extras of the property pass -------------------------------------------
 // P:34-36 "computation of thermal and transport properties" for a compressible solver with non-unity Lewis numbers
 // ("Hirschfelder and Curtiss mixture-averaged transport"): besides cp, h, mu, lambda, D_k the transport
@@ -417,6 +452,15 @@ void oracle_pasr(const void* mv, long long n, long long ld, const double* T, con
     for (long long i = 0; i < n; ++i)
         cell_pasr(m, T[i], p[i], Y + i, ld, mu[i], ksgs[i], eps[i], T_gate, om_in + i, om_out + i, ld,
                   kappa ? &kappa[i] : nullptr);
+}
+
+void oracle_ann_source_mmlp(const void* const* nets, const void* mv, long long n, long long ld, const double* T,
+                            const double* p, const double* Y, double* omega, double* dY) {
+    const Mech& m = *static_cast<const Mech*>(mv);
+    const Ann* const* a = reinterpret_cast<const Ann* const*>(nets);
+#pragma omp parallel for schedule(static)
+    for (long long i = 0; i < n; ++i)
+        cell_source_mmlp(a, m, T[i], p[i], Y + i, ld, omega ? omega + i : nullptr, dY ? dY + i : nullptr, ld);
 }
 
 }  // extern "C"

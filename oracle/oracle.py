@@ -74,6 +74,7 @@ def lib():
         _lib.oracle_ann_features.argtypes = [vp, ll, ll, P, P, P, P]
         _lib.oracle_mlp_forward.argtypes = [vp, ll, P, P]
         _lib.oracle_ann_source.argtypes = [vp, vp, ll, ll, P, P, P, P, P]
+        _lib.oracle_ann_source_mmlp.argtypes = [P, vp, ll, ll, P, P, P, P, P]
     return _lib
 
 
@@ -231,6 +232,26 @@ class Ann:
         om = np.zeros((self.K, ld))
         dY = np.zeros((self.K, ld))
         lib().oracle_ann_source(self.h, mech.h, n, ld, _p(T), _p(p), _p(Y), _p(om), _p(dY))
+        return om, dY
+
+
+class Mmlp:
+    """K one-output networks, one per species (NEXT-1): nets[k] has the attributes of synth.AnnModel with
+    dims[0] = K + 2, dims[-1] = 1, the shared input statistics in x_mean/x_std and species k's u_mean/u_std."""
+
+    def __init__(self, nets):
+        self.K = len(nets)
+        for a in nets:
+            assert int(a.dims[0]) == self.K + 2 and int(a.dims[-1]) == 1
+        self.nets = [Ann(a) for a in nets]
+        self._arr = (C.c_void_p * self.K)(*[a.h for a in self.nets])
+
+    def source(self, mech: Mech, T, p, Y):
+        T, Y, n, ld = Mech._fields(T, Y)
+        p = _f64(p)
+        om = np.zeros((self.K, ld))
+        dY = np.zeros((self.K, ld))
+        lib().oracle_ann_source_mmlp(self._arr, mech.h, n, ld, _p(T), _p(p), _p(Y), _p(om), _p(dY))
         return om, dY
 
 

@@ -219,6 +219,30 @@ def make_ann(K: int, hidden: List[int], precision: int, seed: int,
     return AnnModel(dims, Ws, bs, precision, x_mean, x_std, u_mean, u_std, boxcox_lambda, dt)
 
 
+def make_mmlp(K: int, hidden: List[int], precision: int, seed: int, boxcox_lambda: float = 0.1, dt: float = 1e-6) -> List[AnnModel]:
+    """One network per species ("individual training and prediction ... for each species mass fraction"):
+    K independent (K+2) -> hidden -> 1 networks, Xavier-uniform from one seeded generator (net after net), sharing
+    the input statistics; net k carries species k's output statistics as its u_mean[0], u_std[0]."""
+    proto = make_ann(K, hidden, precision, seed, boxcox_lambda, dt)      # shared x_mean/x_std, per-species u statistics
+    rng = _rng(seed, 5)
+    dims = [K + 2] + list(hidden) + [1]
+    nets = []
+    for k in range(K):
+        Ws, bs = [], []
+        for l in range(len(dims) - 1):
+            fan_in, fan_out = dims[l], dims[l + 1]
+            lim = np.sqrt(6.0 / (fan_in + fan_out))
+            Wl = rng.uniform(-lim, lim, (fan_out, fan_in)).astype(np.float32)
+            bl = rng.uniform(-1.0 / np.sqrt(fan_in), 1.0 / np.sqrt(fan_in), fan_out).astype(np.float32)
+            if precision == 1:
+                Wl = round_to_bf16(Wl)
+            Ws.append(np.ascontiguousarray(Wl))
+            bs.append(np.ascontiguousarray(bl))
+        nets.append(AnnModel(dims, Ws, bs, precision, proto.x_mean, proto.x_std, proto.u_mean[k:k + 1].copy(),
+                             proto.u_std[k:k + 1].copy(), boxcox_lambda, dt))
+    return nets
+
+
 # --------------------------------------------------------------------------------------
 # cell fields
 # --------------------------------------------------------------------------------------
