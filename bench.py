@@ -361,7 +361,25 @@ def bench_configs(torch, B, stream, pk, fp32, quick=False):
                                 "frac": ach / pk["bf16"], "peak_source": f"{pk['src']} bf16 burst (kernel timed alone)",
                                 "algorithmic": f"{FLOPS_PER_CELL_MLP} flop/cell x {n} cells/launch",
                                 "note": "2048 tiles over 148 CTAs = 13.8 waves: 1 - 13.84/14 = 1.1 % tail"}}
-    del gm, ga, sets, ws
+    # ---- NEXT-1: one MLP per species, 19 networks 21-1600-800-400-1 on the same field ----
+    nets = synth.make_mmlp(K, HIDDEN, 1, synth.config_seed(2))
+    gn = B.AnnMmlp(nets)
+    wsm = B.alloc_workspace_mmlp(gn, n, n)
+
+    def mmlp_launch(i):
+        T_, p_, Y_, o_ = sets[i % len(sets)]
+        B.df_chem_ann_source_mmlp(gn, gm, T_, p_, Y_, omega=o_, workspace=wsm)
+    med, mn = _median_launch_ms(torch, stream, mmlp_launch, 4, warm=1)
+    fl = K * 2 * (21 * 1600 + 1600 * 800 + 800 * 400 + 400 * 1)
+    ach = fl * n / (med * 1e-3) / 1e12
+    out["mmlp"] = {"workload": "NEXT-1 (P:79): 19 per-species MLPs 21-1600-800-400-1 on configs[1]'s 262144 cells "
+                               "(19 tensor-chain launches + 1 epilogue launch per call)",
+                   "ms": med, "ms_min": mn, "cells_per_s": n / (med * 1e-3),
+                   "roofline": {"kernel": "ann_bf16_kernel x19", "bound": "tensor", "achieved": ach, "peak": pk["bf16_sust"], "unit": "TFLOP/s",
+                                "frac": ach / pk["bf16_sust"], "frac_vs_burst": ach / pk["bf16"],
+                                "peak_source": f"{pk['src']} bf16 sustained (a 15 ms back-to-back tensor load)",
+                                "algorithmic": f"{fl} flop/cell x {n} cells/call"}}
+    del gm, ga, sets, ws, gn, wsm, nets
     torch.cuda.empty_cache()
 
     # ---- the two pointwise passes of SURVEY 8(f) NEXT-3 / NEXT-4 on the headline field (2,097,152 cells, K = 19) ----

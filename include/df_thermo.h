@@ -45,6 +45,7 @@ extern "C" {
 
 typedef struct df_mech df_mech; /* species tables, opaque */
 typedef struct df_ann df_ann;   /* MLP + normalisation tables, opaque */
+typedef struct df_ann_mmlp df_ann_mmlp; /* one MLP per species, opaque */
 typedef struct df_host_ctx df_host_ctx; /* device staging buffers for df_step_host, opaque */
 
 typedef enum {
@@ -131,6 +132,27 @@ DF_API df_status df_chem_ann_source(const df_ann* ann, const df_mech* mech, long
                              const float* T, const float* p, const float* Y,
                              float* omega, float* dY,
                              void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- one MLP per species ("individual training and prediction are carried out for each
+ * species mass fraction", "multiple multilayer perceptrons") --------------------------------------------------
+ * K independent networks with dims = {K+2, d1, d2, d3, 1} (n_layers = 4, the tensor path's shapes, see df_ann_create
+ * precision 1: bf16-valued weights).  W[k*4 + l] / b[k*4 + l] are layer l of species k's network.  All networks
+ * share the input vector x = {T, p, F(Y)} and its statistics x_mean/x_std [K+2]; network k's output o^(k) is the
+ * z-scored Box-Cox-space change of species k: Delta_k = u_std[k] o^(k) + u_mean[k]; everything after that is the
+ * epilogue of df_chem_ann_source.  The hot call runs the K tensor-core chains back to back on `stream`, then one
+ * pointwise kernel; workspace (1024-byte aligned) holds the K raw outputs per cell ([K][ld] fp32) and the chain's
+ * scratch: df_ann_mmlp_workspace_bytes(m, n_cells, ld) bytes on the current device. */
+DF_API df_status df_ann_mmlp_create(df_ann_mmlp** out, int K, int n_layers, const int* dims,
+                             const float* const* W, const float* const* b,
+                             const double* x_mean, const double* x_std,
+                             const double* u_mean, const double* u_std,
+                             double boxcox_lambda, double dt);
+DF_API df_status df_ann_mmlp_destroy(df_ann_mmlp* m);
+DF_API size_t df_ann_mmlp_workspace_bytes(const df_ann_mmlp* m, long long n_cells, long long ld);
+DF_API df_status df_chem_ann_source_mmlp(const df_ann_mmlp* m, const df_mech* mech, long long n_cells, long long ld,
+                                  const float* T, const float* p, const float* Y,
+                                  float* omega, float* dY,
+                                  void* workspace, size_t workspace_bytes, void* stream);
 
 /* ---- solver-facing extras of the property pass (reading A22) ------------
  * What a compressible solver with non-unity Lewis numbers needs besides cp, h, mu, lambda, D_k (all per cell, fp32):

@@ -23,6 +23,7 @@ SYMBOLS = (
     "df_ann_create", "df_ann_destroy", "df_ann_workspace_bytes",
     "df_thermo_T_from_h", "df_thermo_properties", "df_chem_ann_source",
     "df_thermo_extras", "df_chem_pasr_scale",
+    "df_ann_mmlp_create", "df_ann_mmlp_destroy", "df_ann_mmlp_workspace_bytes", "df_chem_ann_source_mmlp",
     "df_host_ctx_create", "df_host_ctx_destroy", "df_step_host",
     "df_probe_fp32_peak",
 )
@@ -56,6 +57,11 @@ _lib.df_thermo_properties.argtypes = [_vp, _ll, _ll, _vp, _vp, _vp, _vp, _vp, _v
 _lib.df_chem_ann_source.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 _lib.df_thermo_extras.argtypes = [_vp, _ll, _ll] + [_vp] * 13
 _lib.df_chem_pasr_scale.argtypes = [_vp, _ll, _ll, _vp, _vp, _vp, _vp, _vp, _vp, C.c_float, _vp, _vp, _vp]
+_lib.df_ann_mmlp_create.argtypes = [C.POINTER(_vp), _i, _i, _vp, C.POINTER(_vp), C.POINTER(_vp), _vp, _vp, _vp, _vp, _d, _d]
+_lib.df_ann_mmlp_destroy.argtypes = [_vp]
+_lib.df_ann_mmlp_workspace_bytes.restype = _sz
+_lib.df_ann_mmlp_workspace_bytes.argtypes = [_vp, _ll, _ll]
+_lib.df_chem_ann_source_mmlp.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 _lib.df_host_ctx_create.argtypes = [C.POINTER(_vp), _vp, _vp, _ll]
 _lib.df_host_ctx_destroy.argtypes = [_vp]
 _lib.df_step_host.argtypes = [_vp, _ll, _ll] + [_vp] * 10
@@ -145,6 +151,55 @@ class Ann:
             self.handle = None
 
     __del__ = close
+
+
+class AnnMmlp:
+    """df_ann_mmlp handle from a list of K one-output networks (attributes of synth.AnnModel; see synth.make_mmlp)."""
+
+    def __init__(self, nets):
+        self.K = len(nets)
+        dims = np.asarray([int(x) for x in nets[0].dims], dtype=np.int32)
+        nl = len(dims) - 1
+        Ws = [np.ascontiguousarray(w, dtype=np.float32) for a in nets for w in a.W]
+        bs = [np.ascontiguousarray(x, dtype=np.float32) for a in nets for x in a.b]
+        for a in nets:
+            if [int(x) for x in a.dims] != list(dims):
+                raise ValueError("all networks must have the same dims")
+        Wp = (_vp * len(Ws))(*[w.ctypes.data for w in Ws])
+        bp = (_vp * len(bs))(*[x.ctypes.data for x in bs])
+        xm, xs = _f64(nets[0].x_mean), _f64(nets[0].x_std)
+        um = _f64([float(np.asarray(a.u_mean).ravel()[0]) for a in nets])
+        us = _f64([float(np.asarray(a.u_std).ravel()[0]) for a in nets])
+        h = _vp()
+        _check(_lib.df_ann_mmlp_create(C.byref(h), self.K, nl, _np(dims), Wp, bp, _np(xm), _np(xs), _np(um), _np(us),
+                                       float(nets[0].boxcox_lambda), float(nets[0].dt)))
+        self.handle = h
+
+    def workspace_bytes(self, n_cells: int, ld: int) -> int:
+        return int(_lib.df_ann_mmlp_workspace_bytes(self.handle, int(n_cells), int(ld)))
+
+    def close(self):
+        if getattr(self, "handle", None) and _lib is not None:
+            _lib.df_ann_mmlp_destroy(self.handle)
+            self.handle = None
+
+    __del__ = close
+
+
+def df_chem_ann_source_mmlp(m: AnnMmlp, mech: Mech, T, p, Y, omega=None, dY=None, workspace=None, n_cells=None,
+                            stream=None) -> None:
+    n = int(T.shape[0]) if n_cells is None else int(n_cells)
+    ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    _check(_lib.df_chem_ann_source_mmlp(m.handle, mech.handle, n, int(Y.shape[1]), _dp(T), _dp(p), _dp(Y), _dp(omega),
+                                        _dp(dY), _dp(workspace), ws_bytes, _stream(stream)))
+
+
+def alloc_workspace_mmlp(m: AnnMmlp, n_cells: int, ld: int, device="cuda"):
+    import torch
+    nbytes = m.workspace_bytes(n_cells, ld)
+    ws = torch.empty(nbytes + 1024, dtype=torch.uint8, device=device)
+    off = (-ws.data_ptr()) % 1024
+    return ws[off:off + nbytes]
 
 
 def df_thermo_T_from_h(mech: Mech, h, Y, T, cp=None, n_unconverged=None, n_cells=None, stream=None) -> None:

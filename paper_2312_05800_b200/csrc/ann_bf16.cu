@@ -248,6 +248,8 @@ struct KArgs {
     long long n, ld;
     const float *T, *p, *Y;
     float *omega, *dY;
+    float* raw;        // per-species-network mode (ann_mmlp.cu): the final epilogue only stores o[raw_row] + b4 to raw[raw_row][ld]
+    int raw_row;
     uint8_t* scratch;  // gridDim.x * NKC * 16384 bytes
 };
 
@@ -687,6 +689,14 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(B_SMALL_EMPTY + sb));
+            if (a.raw) {   // kernel-uniform: this launch is one of K one-output networks; the shared epilogue runs afterwards
+                float o = 0.f;
+#pragma unroll
+                for (int k = 0; k < 32; ++k)
+                    if (k == a.raw_row) o = __uint_as_float(r[k]) + a.b4[k];
+                if (valid) a.raw[(size_t)a.raw_row * a.ld + cell] = o;
+                continue;
+            }
             // first pass: dY*_k (kept in r[k]), sum Y, sum dY*, 1 / Wbar; branch-free so the MUFU chains interleave
             float sumY = 0.f, sumd = 0.f, inv_Wbar = 0.f;
 #pragma unroll
@@ -907,7 +917,7 @@ size_t ann_bf16_workspace(const df_ann* ann, long long n) {
 
 df_status launch_ann_bf16(const df_ann* ann, const df_mech* mech, long long n, long long ld, const float* T,
                           const float* p, const float* Y, float* omega, float* dY, void* ws, size_t ws_bytes,
-                          cudaStream_t s) {
+                          cudaStream_t s, float* raw, int raw_row) {
     const Bf16Plan* P = ann->bf16;
     const long long grid = bf16_grid(n);
     if (ws_bytes < (size_t)grid * P->g.NKC * kChunkBytes)
@@ -924,6 +934,7 @@ df_status launch_ann_bf16(const df_ann* ann, const df_mech* mech, long long n, l
     a.ld = ld;
     a.T = T; a.p = p; a.Y = Y;
     a.omega = omega; a.dY = dY;
+    a.raw = raw; a.raw_row = raw_row;
     a.scratch = static_cast<uint8_t*>(ws);
     ann_bf16_kernel<<<(unsigned)grid, kThreads, P->g.smem_bytes, s>>>(a, ann->norm);
     DF_CUDA_TRY(cudaGetLastError());

@@ -131,4 +131,5 @@ df_status ann_bf16_create(df_ann*, const float* const* W, const float* const* b)
 void ann_bf16_destroy(df_ann*);
 size_t ann_bf16_workspace(const df_ann*, long long n);
 df_status launch_ann_bf16(const df_ann*, const df_mech*, long long n, long long ld, const float* T, const float* p,
-                          const float* Y, float* omega, float* dY, void* ws, size_t ws_bytes, cudaStream_t s);
+                          const float* Y, float* omega, float* dY, void* ws, size_t ws_bytes, cudaStream_t s,
+                          float* raw = nullptr, int raw_row = 0);

@@ -36,6 +36,54 @@ def _rounder(fmt):
     raise ValueError(fmt)
 
 
+def ideal_chain_source_mmlp(mech, nets, T, p, Y, fmt="fp16"):
+    """The same floor for K one-output networks (NEXT-1): net k supplies o_k; shared features and epilogue."""
+    from types import SimpleNamespace
+    K = len(nets)
+    outs = []
+    for a in nets:
+        one = SimpleNamespace(W=a.W, b=a.b, x_mean=a.x_mean, x_std=a.x_std, u_mean=np.zeros(1), u_std=np.ones(1),
+                              boxcox_lambda=a.boxcox_lambda, dt=a.dt)
+        outs.append(_chain_outputs(one, T, p, Y, fmt, K)[:, 0])
+    o = np.stack(outs, axis=1)
+    u_mean = np.array([float(np.asarray(a.u_mean).ravel()[0]) for a in nets])
+    u_std = np.array([float(np.asarray(a.u_std).ravel()[0]) for a in nets])
+    return _epilogue(mech, nets[0].boxcox_lambda, nets[0].dt, u_mean, u_std, o, T, p, Y)
+
+
+def _chain_outputs(ann, T, p, Y, fmt, K):
+    rnd = _rounder(fmt)
+    acc = (lambda z: z) if fmt is None else (lambda z: z.astype(np.float32).astype(np.float64))
+    lam = float(ann.boxcox_lambda)
+    Y = np.asarray(Y, np.float64)
+    T = np.asarray(T, np.float64)
+    p = np.asarray(p, np.float64)
+    n = T.shape[0]
+    Yt = Y[:K, :n].T
+    x = np.empty((n, K + 2))
+    x[:, 0] = (T - ann.x_mean[0]) / ann.x_std[0]
+    x[:, 1] = (p - ann.x_mean[1]) / ann.x_std[1]
+    x[:, 2:] = ((Yt ** lam - 1.0) / lam - np.asarray(ann.x_mean)[2:]) / np.asarray(ann.x_std)[2:]
+    a = rnd(x)
+    for l in range(len(ann.W) - 1):
+        z = acc(a @ np.asarray(ann.W[l], np.float64).T + np.asarray(ann.b[l], np.float64))
+        a = rnd(0.5 * z * (1.0 + erf(z / np.sqrt(2.0))))
+    return a @ np.asarray(ann.W[-1], np.float64).T + np.asarray(ann.b[-1], np.float64)
+
+
+def _epilogue(mech, lam, dt, u_mean, u_std, o, T, p, Y):
+    lam = float(lam)
+    T = np.asarray(T, np.float64)
+    p = np.asarray(p, np.float64)
+    n = T.shape[0]
+    Yt = np.asarray(Y, np.float64)[:, :n].T
+    delta = u_std * o + u_mean
+    Ys = np.maximum(Yt ** lam + lam * delta, 0.0) ** (1.0 / lam)
+    dY = Ys / Ys.sum(axis=1, keepdims=True) - Yt
+    rho = p / ((Yt / np.asarray(mech.W)).sum(axis=1) * R * T)
+    return (rho[:, None] * dY / float(dt)).T.copy(), dY.T.copy()
+
+
 def ideal_chain_source(mech, ann, T, p, Y, fmt="fp16"):
     """(omega[K, n], dY[K, n]) of O9-O12 with 16-bit rounding of features/activations only (fmt: fp16|bf16|None)."""
     rnd = _rounder(fmt)

@@ -53,3 +53,18 @@ def test_bf16_chain_is_an_order_of_magnitude_coarser(case):
     nb = max(t["normwise"] for t in helpers.mixed_err_table(omb, sub(om_r)))
     assert 4.0 <= nb / n16 <= 16.0, (nb, n16)      # 3 more significand bits = 8 x, up to sampling noise
     assert nb > 2e-2                               # an ideal bf16-activation chain misses even the normwise form
+
+
+def test_unrounded_mmlp_chain_reproduces_the_oracle():
+    """The per-species-network variant of the floor (NEXT-1) is pinned the same way."""
+    from oracle import oracle
+    from paper_2312_05800_b200 import synth
+    K, n = 6, 64
+    mech = synth.make_mechanism(K, 31)
+    nets = synth.make_mmlp(K, [16, 12, 8], 1, 31)
+    cells = synth.cells_stratified(K, n, 31)
+    om_r, dY_r = oracle.Mmlp(nets).source(oracle.Mech(mech), cells.T, cells.p, cells.Y)
+    om, dY = ideal16.ideal_chain_source_mmlp(mech, nets, cells.T, cells.p, cells.Y, fmt=None)
+    for got, ref in ((om, om_r), (dY, dY_r)):
+        mixed, norm = helpers.mixed_err(got, ref)
+        assert mixed <= 1e-5 and norm <= 1e-6, (mixed, norm)
