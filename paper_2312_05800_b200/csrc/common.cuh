@@ -82,6 +82,7 @@ struct df_mech {
     int K;
     MechDev dev;
     std::vector<double> W_host;
+    std::vector<double> th64_host;  // [K][2][6] host copy of dev.th64 (fixed-K Newton tables are built from it per launch)
     PropTables<9>* t9 = nullptr;    // host copies of the fixed-K tables (only the matching one is set)
     PropTables<19>* t19 = nullptr;
 };

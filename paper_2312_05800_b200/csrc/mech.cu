@@ -159,6 +159,7 @@ extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const
     if (!mech) return df_set_error(DF_ERR_ALLOC, "df_mech_create: out of host memory");
     mech->K = K;
     mech->W_host.assign(W, W + K);
+    mech->th64_host = t.th64;
     MechDev& d = mech->dev;
     memset(&d, 0, sizeof(d));
     d.K = K;
