@@ -32,34 +32,42 @@ __device__ __forceinline__ int newton_pair(const MechScalars& sc, double (&A)[6]
     const float a1 = (float)A[1], a2 = 2.f * (float)A[2], a3 = 3.f * (float)A[3], a4 = 4.f * (float)A[4], a5 = 5.f * (float)A[5];
     const float b1 = (float)Bc[1], b2 = 2.f * (float)Bc[2], b3 = 3.f * (float)Bc[3], b4 = 4.f * (float)Bc[4], b5 = 5.f * (float)Bc[5];
     // A4: invalid guess -> T_mid; the start is moved onto the root's side of T_mid, the iterates stay there
+    // (a mechanism whose two ranges do not quite meet at T_mid may have its root a hair across it, hence the 1 K margin)
+    constexpr float kMargin = 1e-3f;
+    const float la = hi_a ? -kMargin : sc.tau_min, ua = hi_a ? sc.tau_max : kMargin;
+    const float lb = hi_b ? -kMargin : sc.tau_min, ub = hi_b ? sc.tau_max : kMargin;
     const float ga = (tg.x > 0.f && tg.x < 3.0e38f) ? (tg.x - sc.T_mid) * sc.inv_S : 0.f;
     const float gb = (tg.y > 0.f && tg.y < 3.0e38f) ? (tg.y - sc.T_mid) * sc.inv_S : 0.f;
-    // (a mechanism whose two ranges do not quite meet at T_mid may have its root a hair across it, hence the 1 K margin)
-    constexpr double kMargin = 1e-3;
-    const double la = hi_a ? -kMargin : (double)sc.tau_min, ua = hi_a ? (double)sc.tau_max : kMargin;
-    const double lb = hi_b ? -kMargin : (double)sc.tau_min, ub = hi_b ? (double)sc.tau_max : kMargin;
-    double ta = fmin(fmax((double)ga, la), ua), tb = fmin(fmax((double)gb, lb), ub);
+    double ta = (double)fminf(fmaxf(ga, la), ua), tb = (double)fminf(fmaxf(gb, lb), ub);
     const double ha = (double)hin.x, hb = (double)hin.y;
-    double da = 0.0, db = 0.0;
+    // The residual is formed in fp64 (it is the difference of two numbers ~1e7 that must be good to 0.1); the step
+    // itself -- residual x 1/slope -- needs no more than fp32: its rounding is 1e-7 of the step, a quasi-Newton
+    // perturbation.  The loop leaves after a step below 10 mK: the error left is (step)^2 cp'/(2 cp) < 1e-7 K.
+    float sa_step = 0.f, sb_step = 0.f;
     for (int it = 0; it < kMaxIter; ++it) {
         const double va = fma(fma(fma(fma(fma(A[5], ta, A[4]), ta, A[3]), ta, A[2]), ta, A[1]), ta, A[0]);
         const double vb = fma(fma(fma(fma(fma(Bc[5], tb, Bc[4]), tb, Bc[3]), tb, Bc[2]), tb, Bc[1]), tb, Bc[0]);
         const float fa = (float)ta, fb = (float)tb;
         const float sa = fmaf(fmaf(fmaf(fmaf(a5, fa, a4), fa, a3), fa, a2), fa, a1);
         const float sb = fmaf(fmaf(fmaf(fmaf(b5, fb, b4), fb, b3), fb, b2), fb, b1);
-        da = (ha - va) * (double)__frcp_rn(sa);
-        db = (hb - vb) * (double)__frcp_rn(sb);
-        ta = fmin(fmax(ta + da, la), ua);
-        tb = fmin(fmax(tb + db, lb), ub);
-        if (!(fmax(fabs(da), fabs(db)) >= 1e-6)) break;  // 1 mK step: the error left is ~1e-9 K (also leaves on NaN)
+        sa_step = (float)(ha - va) * rcp_approx(sa);
+        sb_step = (float)(hb - vb) * rcp_approx(sb);
+        ta += (double)sa_step;
+        tb += (double)sb_step;
+        const float na = fa + sa_step, nb = fb + sb_step;   // where the iterate went, to fp32: enough for the (rare) clamp
+        if (na < la) ta = (double)la;
+        if (na > ua) ta = (double)ua;
+        if (nb < lb) tb = (double)lb;
+        if (nb > ub) tb = (double)ub;
+        if (!(fmaxf(fabsf(sa_step), fabsf(sb_step)) >= 1e-5f)) break;   // also leaves on NaN
     }
     const float fa = (float)ta, fb = (float)tb;
     Tout = make_float2((float)fma(ta, (double)sc.S, (double)sc.T_mid), (float)fma(tb, (double)sc.S, (double)sc.T_mid));
     cpv = make_float2(fmaf(fmaf(fmaf(fmaf(a5, fa, a4), fa, a3), fa, a2), fa, a1) * sc.inv_S,   // cp at the root
-                                   fmaf(fmaf(fmaf(fmaf(b5, fb, b4), fb, b3), fb, b2), fb, b1) * sc.inv_S);
+                      fmaf(fmaf(fmaf(fmaf(b5, fb, b4), fb, b3), fb, b2), fb, b1) * sc.inv_S);
     int bad = 0;
-    if (!(fabs(da) * (double)sc.S <= 1e-2)) ++bad;
-    if (two && !(fabs(db) * (double)sc.S <= 1e-2)) ++bad;
+    if (!(fabsf(sa_step) * sc.S <= 1e-2f)) ++bad;
+    if (two && !(fabsf(sb_step) * sc.S <= 1e-2f)) ++bad;
     return bad;
 }
 
@@ -84,7 +92,7 @@ struct TfhTables {
 };
 
 template <int K>
-__global__ void __launch_bounds__(kThreads, 4)
+__global__ void __launch_bounds__(kThreads, 6)
 t_from_h_fixed_kernel(const __grid_constant__ TfhTables<K> tab, long long n, long long ld, const float* __restrict__ h,
                       const float* __restrict__ Y, float* __restrict__ T, float* __restrict__ cp_out, int* __restrict__ n_unconv) {
     const long long i = ((long long)blockIdx.x * kThreads + threadIdx.x) * 2;
