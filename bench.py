@@ -334,9 +334,21 @@ def bench_configs(torch, B, stream, pk, fp32, quick=False):
     t1, _ = _median_launch_ms(torch, stream, lambda i: B.df_thermo_T_from_h(gm, h, Y, T), 20, before=lambda i: T.copy_(Tg))
     t2, _ = _median_launch_ms(torch, stream, lambda i: B.df_thermo_properties(gm, T, p, Y, cp=cp, mu=mu, lam=lam, D=D), 20)
     t3, _ = _median_launch_ms(torch, stream, lambda i: B.df_chem_ann_source(ga, gm, T, p, Y, omega=om), 20)
+    # the same step as ONE CUDA-graph launch (df_step_plan / df_thermochem_step, NEXT-2), and as three calls back to back
+    plan = B.StepPlan(gm, ga, h, p, Y, T, T_guess=Tg, cp=cp, mu=mu, lam=lam, D=D, omega=om)
+    tg_, _ = _median_launch_ms(torch, stream, lambda i: plan.launch(), 20)
+
+    def three(i):
+        T.copy_(Tg)
+        B.df_thermo_T_from_h(gm, h, Y, T)
+        B.df_thermo_properties(gm, T, p, Y, cp=cp, mu=mu, lam=lam, D=D)
+        B.df_chem_ann_source(ga, gm, T, p, Y, omega=om)
+    t3c, _ = _median_launch_ms(torch, stream, three, 20)
+    plan.close()
     out["cfg1"] = {"workload": "configs[0]: 4096 cells, K=9, T_from_h + properties + fp32 MLP 11-64-64-9",
                    "us_per_call": {"T_from_h": 1e3 * t1, "properties": 1e3 * t2, "ann_fp32": 1e3 * t3},
-                   "cells_per_s": n / ((t1 + t2 + t3) * 1e-3), "note": "launch-latency bound (problem < 1 MB): no roofline fraction"}
+                   "us_per_step": {"three_calls": 1e3 * t3c, "one_graph_launch": 1e3 * tg_},
+                   "cells_per_s": n / (tg_ * 1e-3), "note": "launch-latency bound (problem < 1 MB): no roofline fraction"}
     del gm, ga
 
     # ---- cfg2: 262,144 cells, K = 19, the tensor-path MLP alone; 6 rotating buffer sets (the 42 MB of one set would

@@ -46,6 +46,7 @@ extern "C" {
 typedef struct df_mech df_mech; /* species tables, opaque */
 typedef struct df_ann df_ann;   /* MLP + normalisation tables, opaque */
 typedef struct df_ann_mmlp df_ann_mmlp; /* one MLP per species, opaque */
+typedef struct df_step_plan df_step_plan; /* one time step captured as a CUDA graph, opaque */
 typedef struct df_host_ctx df_host_ctx; /* device staging buffers for df_step_host, opaque */
 
 typedef enum {
@@ -178,6 +179,20 @@ DF_API df_status df_chem_pasr_scale(const df_mech* mech, long long n_cells, long
                              const float* T, const float* p, const float* Y,
                              const float* mu, const float* k_sgs, const float* eps, float T_gate,
                              float* omega, float* kappa, void* stream);
+
+/* ---- single-launch step ("the entire computational process is executed on GPU") -----------
+ * A solver calls the update every time step on the same DEVICE arrays.  df_step_plan_create captures the whole step on
+ * those arrays -- T <- T_guess (skipped when T_guess is NULL or equal to T: T then holds the guess), df_thermo_T_from_h,
+ * df_thermo_properties (outputs that are NULL are skipped; the call is skipped when all are), df_chem_ann_source (when
+ * omega is not NULL; workspace as for that call) -- as one CUDA graph; df_thermochem_step replays it on `stream` with a
+ * single launch.  The arrays (and the handles) must stay valid and unmoved for the life of the plan; results are those
+ * of the three calls made one after the other. */
+DF_API df_status df_step_plan_create(df_step_plan** out, const df_mech* mech, const df_ann* ann, long long n_cells, long long ld,
+                              const float* h, const float* p, const float* T_guess, const float* Y,
+                              float* T, float* cp, float* mu, float* lambda, float* D, float* omega,
+                              void* workspace, size_t workspace_bytes);
+DF_API df_status df_thermochem_step(df_step_plan* plan, void* stream);
+DF_API df_status df_step_plan_destroy(df_step_plan* plan);
 
 /* ---- host-buffer step (bench.py's e2e leg) ----------------------------------------------
  * One pass of the whole path over HOST arrays: copies h, p, T_guess, Y host->device, runs

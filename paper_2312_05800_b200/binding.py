@@ -24,6 +24,7 @@ SYMBOLS = (
     "df_thermo_T_from_h", "df_thermo_properties", "df_chem_ann_source",
     "df_thermo_extras", "df_chem_pasr_scale",
     "df_ann_mmlp_create", "df_ann_mmlp_destroy", "df_ann_mmlp_workspace_bytes", "df_chem_ann_source_mmlp",
+    "df_step_plan_create", "df_thermochem_step", "df_step_plan_destroy",
     "df_host_ctx_create", "df_host_ctx_destroy", "df_step_host",
     "df_probe_fp32_peak",
 )
@@ -62,6 +63,9 @@ _lib.df_ann_mmlp_destroy.argtypes = [_vp]
 _lib.df_ann_mmlp_workspace_bytes.restype = _sz
 _lib.df_ann_mmlp_workspace_bytes.argtypes = [_vp, _ll, _ll]
 _lib.df_chem_ann_source_mmlp.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+_lib.df_step_plan_create.argtypes = [C.POINTER(_vp), _vp, _vp, _ll, _ll] + [_vp] * 11 + [_sz]
+_lib.df_thermochem_step.argtypes = [_vp, _vp]
+_lib.df_step_plan_destroy.argtypes = [_vp]
 _lib.df_host_ctx_create.argtypes = [C.POINTER(_vp), _vp, _vp, _ll]
 _lib.df_host_ctx_destroy.argtypes = [_vp]
 _lib.df_step_host.argtypes = [_vp, _ll, _ll] + [_vp] * 10
@@ -246,6 +250,31 @@ def alloc_workspace(ann: Ann, n_cells: int, device="cuda"):
     ws = torch.empty(nbytes + 1024, dtype=torch.uint8, device=device)
     off = (-ws.data_ptr()) % 1024
     return ws[off:off + nbytes]
+
+
+class StepPlan:
+    """df_step_plan: the whole step on fixed device arrays as one CUDA graph; launch() replays it with one launch."""
+
+    def __init__(self, mech: Mech, ann: Optional[Ann], h, p, Y, T, T_guess=None, cp=None, mu=None, lam=None, D=None,
+                 omega=None, workspace=None, n_cells=None):
+        n = int(T.shape[0]) if n_cells is None else int(n_cells)
+        ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+        hdl = _vp()
+        _check(_lib.df_step_plan_create(C.byref(hdl), mech.handle, ann.handle if ann is not None else None, n, int(Y.shape[1]),
+                                        _dp(h), _dp(p), _dp(T_guess), _dp(Y), _dp(T), _dp(cp), _dp(mu), _dp(lam), _dp(D),
+                                        _dp(omega), _dp(workspace), ws_bytes))
+        self.handle = hdl
+        self._keep = (mech, ann, h, p, Y, T, T_guess, cp, mu, lam, D, omega, workspace)
+
+    def launch(self, stream=None) -> None:
+        _check(_lib.df_thermochem_step(self.handle, _stream(stream)))
+
+    def close(self):
+        if getattr(self, "handle", None) and _lib is not None:
+            _lib.df_step_plan_destroy(self.handle)
+            self.handle = None
+
+    __del__ = close
 
 
 class HostCtx:

@@ -283,3 +283,74 @@ extern "C" df_status df_step_host(df_host_ctx* c, long long n, long long ld, con
     DF_CUDA_TRY(cudaStreamSynchronize(c->stream));
     return DF_OK;
 }
+
+// ---- single-launch step ---------------------------------------------------------------------------
+// P:34 "to avoid the CPU-GPU memory copy overhead, the entire computational process is executed on GPU": a solver calls
+// the update every time step on the same field arrays, so the whole step -- guess copy, T_from_h, properties, ANN
+// source -- is captured once as a CUDA graph and replayed with ONE launch per time step.
+struct df_step_plan {
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    int n_kernels = 0;
+};
+
+extern "C" df_status df_step_plan_destroy(df_step_plan* p) {
+    if (!p) return DF_OK;
+    if (p->exec) cudaGraphExecDestroy(p->exec);
+    if (p->graph) cudaGraphDestroy(p->graph);
+    delete p;
+    return DF_OK;
+}
+
+extern "C" df_status df_step_plan_create(df_step_plan** out, const df_mech* mech, const df_ann* ann, long long n, long long ld,
+                                         const float* h, const float* p, const float* T_guess, const float* Y, float* T,
+                                         float* cp, float* mu, float* lambda, float* D, float* omega, void* workspace,
+                                         size_t workspace_bytes) {
+    if (!out) return df_set_error(DF_ERR_INVALID_ARG, "df_step_plan_create: out is NULL");
+    *out = nullptr;
+    if (!mech || n < 1 || !h || !Y || !T) return df_set_error(DF_ERR_INVALID_ARG, "df_step_plan_create: bad argument");
+    if (omega && !ann) return df_set_error(DF_ERR_INVALID_ARG, "df_step_plan_create: omega requested but ann is NULL");
+    df_step_plan* pl = new (std::nothrow) df_step_plan;
+    if (!pl) return df_set_error(DF_ERR_ALLOC, "df_step_plan_create: out of host memory");
+    cudaStream_t cs = nullptr;
+    if (cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking) != cudaSuccess) {
+        delete pl;
+        return df_set_error(DF_ERR_CUDA, "df_step_plan_create: cudaStreamCreate failed");
+    }
+    df_status st = DF_OK;
+    cudaError_t ce = cudaStreamBeginCapture(cs, cudaStreamCaptureModeRelaxed);
+    if (ce != cudaSuccess) st = df_set_error(DF_ERR_CUDA, "df_step_plan_create: cudaStreamBeginCapture: %s", cudaGetErrorString(ce));
+    if (st == DF_OK) {
+        if (T_guess && T_guess != T && cudaMemcpyAsync(T, T_guess, (size_t)n * sizeof(float), cudaMemcpyDeviceToDevice, cs) != cudaSuccess)
+            st = df_set_error(DF_ERR_CUDA, "df_step_plan_create: guess copy failed");
+        if (st == DF_OK) st = df_thermo_T_from_h(mech, n, ld, h, Y, T, nullptr, nullptr, cs);
+        if (st == DF_OK) ++pl->n_kernels;
+        if (st == DF_OK && (cp || mu || lambda || D)) {
+            st = df_thermo_properties(mech, n, ld, T, p, Y, cp, nullptr, mu, lambda, D, cs);
+            if (st == DF_OK) ++pl->n_kernels;
+        }
+        if (st == DF_OK && omega) {
+            st = df_chem_ann_source(ann, mech, n, ld, T, p, Y, omega, nullptr, workspace, workspace_bytes, cs);
+            if (st == DF_OK) ++pl->n_kernels;
+        }
+        ce = cudaStreamEndCapture(cs, &pl->graph);   // always ends the capture, also after an error above
+        if (st == DF_OK && ce != cudaSuccess) st = df_set_error(DF_ERR_CUDA, "df_step_plan_create: cudaStreamEndCapture: %s", cudaGetErrorString(ce));
+    }
+    if (st == DF_OK) {
+        ce = cudaGraphInstantiate(&pl->exec, pl->graph, 0);
+        if (ce != cudaSuccess) st = df_set_error(DF_ERR_CUDA, "df_step_plan_create: cudaGraphInstantiate: %s", cudaGetErrorString(ce));
+    }
+    cudaStreamDestroy(cs);
+    if (st != DF_OK) {
+        df_step_plan_destroy(pl);
+        return st;
+    }
+    *out = pl;
+    return DF_OK;
+}
+
+extern "C" df_status df_thermochem_step(df_step_plan* plan, void* stream) {
+    if (!plan || !plan->exec) return df_set_error(DF_ERR_INVALID_ARG, "df_thermochem_step: plan is NULL");
+    DF_CUDA_TRY(cudaGraphLaunch(plan->exec, (cudaStream_t)stream));
+    return DF_OK;
+}

@@ -397,3 +397,44 @@ def test_ann_tensor_path_reuses_scratch_across_launches(B):
         torch.cuda.synchronize()
         nw = ((out - ref).double().norm(dim=1) / ref.double().norm(dim=1)).max().item()
         assert nw <= 1e-3, nw
+
+
+# --------------------------------------------------------------------------------------------
+# df_step_plan / df_thermochem_step: the step as one CUDA graph launch (NEXT-2)
+# --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,n,ld", [(1, 4097, 4100), (3, 20001, 20004)])
+def test_step_plan_matches_the_three_calls(B, cfg, n, ld):
+    """Replaying the captured step (twice: the graph must be re-launchable) gives what the three calls give on the same
+    arrays: bit for bit for T, cp, mu, lambda, D and the fp32-path omega; within the run-to-run bound on the 16-bit path."""
+    mech, ann, cells, om = make_case(cfg, n, ld)
+    K = mech.K
+    h32 = h_from_T(om, cells)
+    gm, ga = B.Mech(mech), B.Ann(ann)
+    dh, dp, dY, dTg = dev(h32), dev(cells.p), dev(cells.Y), dev(cells.T_guess)
+    ws = B.alloc_workspace(ga, n)
+    # the three calls
+    T = dTg.clone()
+    B.df_thermo_T_from_h(gm, dh, dY, T)
+    cp, mu, lam = (torch.empty(n, device="cuda") for _ in range(3))
+    D, omg = torch.zeros(K, ld, device="cuda"), torch.zeros(K, ld, device="cuda")
+    B.df_thermo_properties(gm, T, dp, dY, cp=cp, mu=mu, lam=lam, D=D)
+    B.df_chem_ann_source(ga, gm, T, dp, dY, omega=omg, workspace=ws)
+    torch.cuda.synchronize()
+    # the plan
+    T2 = torch.full((n,), -1.0, device="cuda")
+    cp2, mu2, lam2 = (torch.empty(n, device="cuda") for _ in range(3))
+    D2, om2 = torch.zeros(K, ld, device="cuda"), torch.zeros(K, ld, device="cuda")
+    plan = B.StepPlan(gm, ga, dh, dp, dY, T2, T_guess=dTg, cp=cp2, mu=mu2, lam=lam2, D=D2, omega=om2, workspace=ws)
+    for _ in range(2):
+        plan.launch()
+    torch.cuda.synchronize()
+    for a, b in ((T, T2), (cp, cp2), (mu, mu2), (lam, lam2), (D, D2)):
+        assert torch.equal(a, b)
+    if ann.precision == 0:
+        assert torch.equal(omg, om2)
+    else:
+        nw = ((omg - om2).double().norm(dim=1) / omg.double().norm(dim=1)).max().item()
+        assert nw <= 1e-3, nw
+    T_ref = om.T_from_h(h32, cells.Y[:, :n], cells.T_guess)
+    assert np.abs(T2.cpu().numpy() - T_ref).max() <= 1e-3
+    plan.close()
