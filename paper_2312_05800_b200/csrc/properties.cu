@@ -37,11 +37,10 @@ __device__ __forceinline__ f2 poly4_2(const float* c, f2 u) {
     return fma2(fma2(fma2(fma2(u, c[4], c[3]), u, bc(c[2])), u, bc(c[1])), u, bc(c[0]));
 }
 
-#ifndef DF_PROPS_MINBLOCKS
-#define DF_PROPS_MINBLOCKS 4
-#endif
+// 4 blocks of 128 threads per SM (128 registers): measured best -- 5 blocks (96 registers) spill 600 B per thread and run
+// 19 % slower, 3 blocks (168 registers) 23 % slower
 template <int K, bool TRANSPORT>
-__global__ void __launch_bounds__(kThreads, DF_PROPS_MINBLOCKS)
+__global__ void __launch_bounds__(kThreads, 4)
 props_fixed_kernel(const __grid_constant__ PropTables<K> tab, long long n, long long ld,
                    const float* __restrict__ Tg, const float* __restrict__ pg, const float* __restrict__ Yg,
                    float* __restrict__ cp_o, float* __restrict__ h_o, float* __restrict__ mu_o,
@@ -113,25 +112,6 @@ props_fixed_kernel(const __grid_constant__ PropTables<K> tab, long long n, long 
 
     // ---- Wilke viscosity ----------------------------------------------------------------------
     if (mu_o) {
-#ifdef DF_WILKE_3VEC
-        f2 g[K], b2[K], c[K];
-#pragma unroll
-        for (int k = 0; k < K; ++k) {
-            g[k] = poly4_2(tab.visc[k], u);
-            const f2 rg = rcp2(g[k]);
-            const f2 xr = mul2(X[k], rg);
-            b2[k] = add2(xr, xr);
-            c[k] = mul2(xr, rg);
-        }
-        f2 acc = bc(0.f);
-#pragma unroll
-        for (int k = 0; k < K; ++k) {
-            f2 den = bc(0.f);
-#pragma unroll
-            for (int j = 0; j < K; ++j) den = fma2(tab.B[k][j], fma2(g[k], fma2(g[k], c[j], b2[j]), X[j]), den);
-            acc = fma2(mul2(mul2(X[k], tab.sqrtW[k]), mul2(g[k], g[k])), rcp2(den), acc);
-        }
-#else
         // Phi_kj = B_kj (1 + g_k/g_j)^2 with only two per-species vectors live (X_j and r_j = 1/g_j): 4 packed
         // instructions per (k,j) instead of the 3 of the three-vector form, but 76 registers less, which buys the
         // occupancy this latency-sensitive kernel needs
@@ -150,7 +130,6 @@ props_fixed_kernel(const __grid_constant__ PropTables<K> tab, long long n, long 
             }
             acc = fma2(mul2(mul2(X[k], tab.sqrtW[k]), mul2(gk, gk)), rcp2(den), acc);
         }
-#endif
         st2(mu_o, mul2(sqrtT, acc));
     }
 
