@@ -129,18 +129,22 @@ def ncu_traffic(kernel_substr: str, grid_x=None):
         return None
     with open(NCU_RAW, newline="") as f:
         rows = [r for r in csv.reader(f) if r]
-    hdr = next((i for i, r in enumerate(rows) if "Kernel Name" in r), None)
-    if hdr is None or hdr + 1 >= len(rows):
-        return None
-    names, units = rows[hdr], rows[hdr + 1]
-    try:
-        ck, cg = names.index("Kernel Name"), names.index("Grid Size")
-        cr, cw = names.index("dram__bytes_read.sum"), names.index("dram__bytes_write.sum")
-    except ValueError:
-        return None
-    best = None
-    for r in rows[hdr + 2:]:
-        if len(r) <= max(ck, cg, cr, cw) or kernel_substr not in r[ck]:
+    best, cols, units, skip = None, None, None, False
+    for r in rows:          # the file is several exports one after the other: every header row resets the columns
+        if "Kernel Name" in r:
+            try:
+                cols = (r.index("Kernel Name"), r.index("Grid Size"), r.index("dram__bytes_read.sum"), r.index("dram__bytes_write.sum"))
+            except ValueError:
+                cols = None
+            skip = True     # the row after a header holds the units
+            continue
+        if skip:
+            units, skip = r, False
+            continue
+        if cols is None or units is None:
+            continue
+        ck, cg, cr, cw = cols
+        if len(r) <= max(cols) or kernel_substr not in r[ck]:
             continue
         try:
             gx = int(r[cg].strip("() ").split(",")[0])
@@ -239,13 +243,13 @@ def aggregate_value(world: int, cells_per_gpu: int, ms_per_step: float) -> float
 
 def cpu_baseline(ns: int):
     """cpu_baseline leg: the fp64 oracle on a bounded sample of the workload, all host cores, plus the same on one
-    thread over a sixteenth of the sample (rank 0, N = 1 only)."""
+    thread over 1/64 of the sample (rank 0, N = 1 only)."""
     oracle, om, oa, cells, h32 = _oracle_setup(ns)
     cores = oracle.get_threads()
     t0 = time.perf_counter()
     _oracle_step(om, oa, cells, h32)
     dt = time.perf_counter() - t0
-    n1 = max(1024, ns // 16)
+    n1 = max(1024, ns // 64)
     from paper_2312_05800_b200 import synth
     sub = synth.Cells(n1, cells.T[:n1], cells.p[:n1], np.ascontiguousarray(cells.Y[:, :n1]), cells.T_guess[:n1])
     oracle.set_threads(1)
@@ -433,7 +437,7 @@ def bench_configs(torch, B, stream, pk, fp32, quick=False):
     out["cfg4"] = {"workload": "configs[3]: 2097152 cells, K=53, properties (cp, h, mu, lambda, D[53])", "ms": med, "ms_min": mn,
                    "cells_per_s": n / (med * 1e-3),
                    "roofline": alu_entry("props_kernel (K=53)", props_flops(K), n, med, fp32,
-                                         {"hbm_bytes_per_cell": 4 * (2 * K + 6), "traffic": ncu_traffic("props_tiled")})}
+                                         {"hbm_bytes_per_cell": 4 * (2 * K + 6), "traffic": ncu_traffic("props_group_kernel")})}
     del gm, T0, p, Y, cp, hh, mu, lam, D
     torch.cuda.empty_cache()
 

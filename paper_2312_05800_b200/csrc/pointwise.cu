@@ -111,7 +111,7 @@ extras_kernel(MechDev md, long long n, long long ld, const float* __restrict__ T
                 const float sk = fmaf(q[0], lnT[c], fmaf(fmaf(fmaf(fmaf(q[5], tau[c], q[4]), tau[c], q[3]), tau[c], q[2]), tau[c], q[1]));
                 const float x = y.v[c] * sIW[k];   // Y_k / W_k; X_k = x / invWbar
                 // Y_k s_k/W_k - R x ln X_k ; x = 0 drops out (x ln x -> 0)
-                const float mix = x > 0.f ? x * (logf(x) - ln_iw[c]) : 0.f;
+                const float mix = x > 0.f ? x * (__logf(x) - ln_iw[c]) : 0.f;   // MUFU lg2: |err| < 1e-6 on a term that is ~1 % of s
                 s[c] = fmaf(y.v[c], sk, fmaf(-Ru, mix, s[c]));
             }
         }
@@ -151,15 +151,16 @@ pasr_kernel(MechDev md, long long n, long long ld, const float* __restrict__ Tg,
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
             const float a = fabsf(w.v[c]);
-            if (a > 0.f) tau_c[c] = fmaxf(tau_c[c], rho[c] * y.v[c] / a);
+            if (a > 0.f) tau_c[c] = fmaxf(tau_c[c], rho[c] * y.v[c] * rcp_approx(a));   // MUFU reciprocal: 1e-7 against a 1e-5 tolerance
         }
     }
     const F4 mu = load4(mug, i0, n, 1.f), ks = load4(kg, i0, n, 1.f), ep = load4(eg, i0, n, 1.f);
     F4 kappa;
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
-        const float tau_mix = sqrtf((ks.v[c] / ep.v[c]) * sqrtf(mu.v[c] / (rho[c] * ep.v[c])));
-        float kp = tau_c[c] > 0.f ? tau_c[c] / (tau_c[c] + tau_mix) : 0.f;
+        const float re = rcp_approx(ep.v[c]);
+        const float tau_mix = sqrtf(ks.v[c] * re * sqrtf(mu.v[c] * re * rcp_approx(rho[c])));
+        float kp = tau_c[c] > 0.f ? tau_c[c] * rcp_approx(tau_c[c] + tau_mix) : 0.f;
         if (T.v[c] < T_gate) kp = 0.f;
         kappa.v[c] = kp;
     }
