@@ -2,8 +2,9 @@
 //   df_thermo_extras      rho, psi = Wbar/(R T), alpha = lambda/cp, rho D_k, h_k(T), mixture entropy   (reading A22)
 //   df_chem_pasr_scale    PaSR factor kappa = tau_c/(tau_c + tau_mix) applied to omega_k, with the T gate (A23)
 // One thread owns four consecutive cells (float4 SoA accesses, 512 B per warp and species row); the species tables
-// (<= 7 KB) are staged in shared memory once per block; Y is walked twice (the second pass hits L1/L2), so the DRAM
-// traffic is the algorithmic 4 B per field element.
+// (<= 7 KB) are staged in shared memory once per block; every input row is read once (single pass: rho factors out of
+// the PaSR time scale, the entropy of mixing is split as sum x ln x - (1/Wbar) ln(1/Wbar)), so the DRAM traffic is the
+// algorithmic 4 B per field element.
 #include "common.cuh"
 
 namespace {
@@ -55,24 +56,38 @@ extras_kernel(MechDev md, long long n, long long ld, const float* __restrict__ T
     if (i0 >= n) return;
     const F4 T = load4(Tg, i0, n, 1000.f), p = load4(pg, i0, n, 101325.f);
 
-    float invWbar[4] = {0.f, 0.f, 0.f, 0.f};
+    // ONE pass over Y: 1/Wbar and, when the entropy is wanted, sum_k Y_k s_k(T) and sum_k x_k ln x_k (x_k = Y_k/W_k):
+    //   s = sum_k Y_k s_k/W_k - R sum_k x_k ln(x_k Wbar) - (R/Wbar) ln(p/p0)
+    //     = sum_k Y_k s_k/W_k - R [sum_k x_k ln x_k - (1/Wbar) ln(1/Wbar)] - (R/Wbar) ln(p/p0)
+    float lnT[4], tau[4];
+    int lo[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        lnT[c] = logf(T.v[c]);
+        tau[c] = (T.v[c] - md.sc.T_mid) * md.sc.inv_S;
+        lo[c] = T.v[c] < md.sc.T_mid;   // A2
+    }
+    float invWbar[4] = {0.f, 0.f, 0.f, 0.f}, sy[4] = {0.f, 0.f, 0.f, 0.f}, sxlx[4] = {0.f, 0.f, 0.f, 0.f};
     for (int k = 0; k < K; ++k) {
         const F4 y = load4(Yg + (size_t)k * ld, i0, n, 0.f);
 #pragma unroll
-        for (int c = 0; c < 4; ++c) invWbar[c] = fmaf(y.v[c], sIW[k], invWbar[c]);
+        for (int c = 0; c < 4; ++c) {
+            const float x = y.v[c] * sIW[k];
+            invWbar[c] += x;
+            if (s_o) {
+                const float* q = sS + k * 12 + (lo[c] ? 0 : 6);
+                const float sk = fmaf(q[0], lnT[c], fmaf(fmaf(fmaf(fmaf(q[5], tau[c], q[4]), tau[c], q[3]), tau[c], q[2]), tau[c], q[1]));
+                sy[c] = fmaf(y.v[c], sk, sy[c]);
+                sxlx[c] += x > 0.f ? x * __logf(x) : 0.f;   // x ln x -> 0; MUFU lg2: |err| < 1e-6 on a term that is ~1 % of s
+            }
+        }
     }
     const float Ru = (float)DF_R_UNIVERSAL;
     F4 rho, psi;
-    float lnT[4], tau[4], ln_iw[4];
-    int lo[4];
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
         psi.v[c] = 1.0f / (invWbar[c] * Ru * T.v[c]);
         rho.v[c] = p.v[c] * psi.v[c];
-        lnT[c] = logf(T.v[c]);
-        ln_iw[c] = logf(invWbar[c]);
-        tau[c] = (T.v[c] - md.sc.T_mid) * md.sc.inv_S;
-        lo[c] = T.v[c] < md.sc.T_mid;   // A2
     }
     if (rho_o) store4(rho_o, i0, n, rho);
     if (psi_o) store4(psi_o, i0, n, psi);
@@ -83,9 +98,14 @@ extras_kernel(MechDev md, long long n, long long ld, const float* __restrict__ T
         for (int c = 0; c < 4; ++c) a.v[c] = lam.v[c] / cp.v[c];
         store4(alpha_o, i0, n, a);
     }
-    if (!rhoD_o && !hk_o && !s_o) return;
-
-    float s[4] = {0.f, 0.f, 0.f, 0.f};
+    if (s_o) {
+        F4 o;
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+            o.v[c] = sy[c] - Ru * (sxlx[c] - invWbar[c] * logf(invWbar[c])) - Ru * invWbar[c] * logf(p.v[c] * (1.0f / 101325.0f));
+        store4(s_o, i0, n, o);
+    }
+    if (!rhoD_o && !hk_o) return;
     for (int k = 0; k < K; ++k) {
         if (rhoD_o) {
             const F4 d = load4(Dg + (size_t)k * ld, i0, n, 0.f);
@@ -103,28 +123,13 @@ extras_kernel(MechDev md, long long n, long long ld, const float* __restrict__ T
             }
             store4(hk_o + (size_t)k * ld, i0, n, o);
         }
-        if (s_o) {
-            const F4 y = load4(Yg + (size_t)k * ld, i0, n, 0.f);
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                const float* q = sS + k * 12 + (lo[c] ? 0 : 6);
-                const float sk = fmaf(q[0], lnT[c], fmaf(fmaf(fmaf(fmaf(q[5], tau[c], q[4]), tau[c], q[3]), tau[c], q[2]), tau[c], q[1]));
-                const float x = y.v[c] * sIW[k];   // Y_k / W_k; X_k = x / invWbar
-                // Y_k s_k/W_k - R x ln X_k ; x = 0 drops out (x ln x -> 0)
-                const float mix = x > 0.f ? x * (__logf(x) - ln_iw[c]) : 0.f;   // MUFU lg2: |err| < 1e-6 on a term that is ~1 % of s
-                s[c] = fmaf(y.v[c], sk, fmaf(-Ru, mix, s[c]));
-            }
-        }
-    }
-    if (s_o) {
-        F4 o;
-#pragma unroll
-        for (int c = 0; c < 4; ++c) o.v[c] = fmaf(-Ru * invWbar[c], logf(p.v[c] * (1.0f / 101325.0f)), s[c]);
-        store4(s_o, i0, n, o);
     }
 }
 
 // ---- NEXT-3 ------------------------------------------------------------------------------------------------------
+// One pass over Y and omega: rho factors out of the slowest time scale, tau_c = rho max_k Y_k/|omega_k|; the omega rows
+// are read again for the scaling (a variant that kept them in registers for K <= 24 needed 140 registers and ran 45 %
+// slower: the occupancy is worth more than the 4 K bytes per cell, which come from L2 mostly).
 __global__ void __launch_bounds__(kPT)
 pasr_kernel(MechDev md, long long n, long long ld, const float* __restrict__ Tg, const float* __restrict__ pg,
             const float* __restrict__ Yg, const float* __restrict__ mug, const float* __restrict__ kg,
@@ -136,31 +141,25 @@ pasr_kernel(MechDev md, long long n, long long ld, const float* __restrict__ Tg,
     const long long i0 = ((long long)blockIdx.x * kPT + threadIdx.x) * 4;
     if (i0 >= n) return;
     const F4 T = load4(Tg, i0, n, 1000.f), p = load4(pg, i0, n, 101325.f);
-    float invWbar[4] = {0.f, 0.f, 0.f, 0.f};
-    for (int k = 0; k < K; ++k) {
-        const F4 y = load4(Yg + (size_t)k * ld, i0, n, 0.f);
-#pragma unroll
-        for (int c = 0; c < 4; ++c) invWbar[c] = fmaf(y.v[c], sm[k], invWbar[c]);
-    }
-    float rho[4], tau_c[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-    for (int c = 0; c < 4; ++c) rho[c] = p.v[c] / (invWbar[c] * (float)DF_R_UNIVERSAL * T.v[c]);
-    // slowest species time scale rho Y_k / |omega_k| over the species that react at all
+    float invWbar[4] = {0.f, 0.f, 0.f, 0.f}, m[4] = {0.f, 0.f, 0.f, 0.f};
     for (int k = 0; k < K; ++k) {
         const F4 y = load4(Yg + (size_t)k * ld, i0, n, 0.f), w = load4(omega + (size_t)k * ld, i0, n, 0.f);
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
+            invWbar[c] = fmaf(y.v[c], sm[k], invWbar[c]);
             const float a = fabsf(w.v[c]);
-            if (a > 0.f) tau_c[c] = fmaxf(tau_c[c], rho[c] * y.v[c] * rcp_approx(a));   // MUFU reciprocal: 1e-7 against a 1e-5 tolerance
+            if (a > 0.f) m[c] = fmaxf(m[c], y.v[c] * rcp_approx(a));   // species that do not react do not count
         }
     }
     const F4 mu = load4(mug, i0, n, 1.f), ks = load4(kg, i0, n, 1.f), ep = load4(eg, i0, n, 1.f);
     F4 kappa;
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
+        const float rho = p.v[c] * rcp_approx(invWbar[c] * (float)DF_R_UNIVERSAL * T.v[c]);
+        const float tau_c = rho * m[c];
         const float re = rcp_approx(ep.v[c]);
-        const float tau_mix = sqrtf(ks.v[c] * re * sqrtf(mu.v[c] * re * rcp_approx(rho[c])));
-        float kp = tau_c[c] > 0.f ? tau_c[c] * rcp_approx(tau_c[c] + tau_mix) : 0.f;
+        const float tau_mix = sqrtf(ks.v[c] * re * sqrtf(mu.v[c] * re * rcp_approx(rho)));
+        float kp = tau_c > 0.f ? tau_c * rcp_approx(tau_c + tau_mix) : 0.f;
         if (T.v[c] < T_gate) kp = 0.f;
         kappa.v[c] = kp;
     }
