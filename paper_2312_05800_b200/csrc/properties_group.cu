@@ -166,13 +166,14 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
         const bool valid = i_raw < n;
         const long long i = valid ? i_raw : 0;
         const bool two = valid && (i + 1 < n);
+        const bool full = (grp + 1) * kGroupCells <= n;   // block-uniform: all but the last group take the plain float2 path
         auto ld2 = [&](const float* p) -> f2 {
-            if (two) return __ldg(reinterpret_cast<const float2*>(p + i));
+            if (full || two) return __ldg(reinterpret_cast<const float2*>(p + i));
             const float v = __ldg(p + i);
             return make_float2(v, v);
         };
         auto st2 = [&](float* p, f2 v) {
-            if (two) *reinterpret_cast<float2*>(p + i) = v;
+            if (full || two) *reinterpret_cast<float2*>(p + i) = v;
             else if (valid) p[i] = v.x;
         };
         const f2 T = T_next, p_cell = p_next;
@@ -189,11 +190,12 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
 
         // ---- phase 1: x_k = Y_k / W_k and the thermo sums of this warp's species --------------------------------
         {
-            f2 C[5];
+            // both ranges are accumulated and the range is picked after the exchange: ten FFMA2 per species instead of
+            // five FFMA2 + ten selects (the exchange grows by five slots, which costs nothing)
+            f2 Cl[5], Ch[5];
 #pragma unroll
-            for (int m = 0; m < 5; ++m) C[m] = bc(0.f);
-            double H0a = 0.0, H0b = 0.0;
-            f2 Yhi = bc(0.f), Ylo = bc(0.f);   // sum_j Y_j of this warp's species as an unevaluated float-float sum
+            for (int m = 0; m < 5; ++m) Cl[m] = Ch[m] = bc(0.f);
+            double H0la = 0.0, H0ha = 0.0, H0lb = 0.0, H0hb = 0.0, Yta = 0.0, Ytb = 0.0;
             f2 sumx = bc(0.f);
 #pragma unroll
             for (int a = 0; a < KW; ++a) {
@@ -202,33 +204,39 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
                 const f2 x = mul2(y, sSmall[k * kSmallStride]);
                 sX[k * 32 + lane] = x;
                 sumx = add2(sumx, x);
-                if (D_o) two_sum_acc(Yhi, Ylo, y);
-                if (want_thermo) {
-                    const float4 a = *reinterpret_cast<const float4*>(sTh + k * 12), b = *reinterpret_cast<const float4*>(sTh + k * 12 + 4),
-                                 c = *reinterpret_cast<const float4*>(sTh + k * 12 + 8);   // lo c0..c5 | hi c0..c5
-                    C[0] = fma2(y, make_float2(lo0 ? a.y : b.w, lo1 ? a.y : b.w), C[0]);
-                    C[1] = fma2(y, make_float2(lo0 ? a.z : c.x, lo1 ? a.z : c.x), C[1]);
-                    C[2] = fma2(y, make_float2(lo0 ? a.w : c.y, lo1 ? a.w : c.y), C[2]);
-                    C[3] = fma2(y, make_float2(lo0 ? b.x : c.z, lo1 ? b.x : c.z), C[3]);
-                    C[4] = fma2(y, make_float2(lo0 ? b.y : c.w, lo1 ? b.y : c.w), C[4]);
-                    if (h_o) {   // formation-enthalpy term in fp64 (|h| ~ 1e7 J/kg against a 1e-5 tolerance)
-                        const double hl = sH0[2 * k], hh = sH0[2 * k + 1];
-                        H0a = fma((double)y.x, lo0 ? hl : hh, H0a);
-                        H0b = fma((double)y.y, lo1 ? hl : hh, H0b);
+                if ((want_thermo && h_o) || D_o) {
+                    const double ya = (double)y.x, yb = (double)y.y;
+                    if (D_o) {   // sum_j Y_j in fp64 (exact on the fp32 inputs to 1e-16): N_k = sum - Y_k without the fp32 rounding of the sum
+                        Yta += ya;
+                        Ytb += yb;
                     }
+                    if (want_thermo && h_o) {   // formation-enthalpy term in fp64 (|h| ~ 1e7 J/kg against a 1e-5 tolerance)
+                        const double hl = sH0[2 * k], hh = sH0[2 * k + 1];
+                        H0la = fma(ya, hl, H0la); H0ha = fma(ya, hh, H0ha);
+                        H0lb = fma(yb, hl, H0lb); H0hb = fma(yb, hh, H0hb);
+                    }
+                }
+                if (want_thermo) {
+                    const float4 a4 = *reinterpret_cast<const float4*>(sTh + k * 12), b4 = *reinterpret_cast<const float4*>(sTh + k * 12 + 4),
+                                 c4 = *reinterpret_cast<const float4*>(sTh + k * 12 + 8);   // lo c0..c5 | hi c0..c5
+                    Cl[0] = fma2(y, a4.y, Cl[0]); Cl[1] = fma2(y, a4.z, Cl[1]); Cl[2] = fma2(y, a4.w, Cl[2]);
+                    Cl[3] = fma2(y, b4.x, Cl[3]); Cl[4] = fma2(y, b4.y, Cl[4]);
+                    Ch[0] = fma2(y, b4.w, Ch[0]); Ch[1] = fma2(y, c4.x, Ch[1]); Ch[2] = fma2(y, c4.y, Ch[2]);
+                    Ch[3] = fma2(y, c4.z, Ch[3]); Ch[4] = fma2(y, c4.w, Ch[4]);
                 }
             }
             f2* my = sScr + (w * kScrSlots) * 32 + lane;
             my[0] = sumx;
-            if (D_o) {
-                my[11 * 32] = Yhi;
-                my[12 * 32] = Ylo;
+            if (D_o) {   // the warp's share of sum Y as a float-float pair
+                const f2 hi = make_float2((float)Yta, (float)Ytb);
+                my[11 * 32] = hi;
+                my[12 * 32] = make_float2((float)(Yta - (double)hi.x), (float)(Ytb - (double)hi.y));
             }
             if (want_thermo) {
 #pragma unroll
-                for (int m = 0; m < 5; ++m) my[(1 + m) * 32] = C[m];
-                reinterpret_cast<double*>(my)[6 * 32] = H0a;
-                reinterpret_cast<double*>(my)[7 * 32] = H0b;
+                for (int m = 0; m < 5; ++m) my[(1 + m) * 32] = make_float2(lo0 ? Cl[m].x : Ch[m].x, lo1 ? Cl[m].y : Ch[m].y);
+                reinterpret_cast<double*>(my)[6 * 32] = lo0 ? H0la : H0ha;
+                reinterpret_cast<double*>(my)[7 * 32] = lo1 ? H0lb : H0hb;
             }
         }
         __syncthreads();
