@@ -39,15 +39,17 @@ __device__ __forceinline__ f2 poly4_2(const float* c, f2 u) {
 
 // 4 blocks of 128 threads per SM (128 registers): measured best -- 5 blocks (96 registers) spill 600 B per thread and run
 // 19 % slower, 3 blocks (168 registers) 23 % slower
-template <int K, bool TRANSPORT>
+// FULL: every thread of the launch has both of its cells inside the field (the host launches the ragged last block
+// separately), so loads and stores are plain float2 accesses without the two-path predicates.
+template <int K, bool TRANSPORT, bool FULL>
 __global__ void __launch_bounds__(kThreads, 4)
-props_fixed_kernel(const __grid_constant__ PropTables<K> tab, long long n, long long ld,
+props_fixed_kernel(const __grid_constant__ PropTables<K> tab, long long i_first, long long n, long long ld,
                    const float* __restrict__ Tg, const float* __restrict__ pg, const float* __restrict__ Yg,
                    float* __restrict__ cp_o, float* __restrict__ h_o, float* __restrict__ mu_o,
                    float* __restrict__ lam_o, float* __restrict__ D_o) {
-    const long long i = ((long long)blockIdx.x * kThreads + threadIdx.x) * 2;
-    if (i >= n) return;
-    const bool two = (i + 1 < n);   // ld % 4 == 0 and 16-byte aligned bases make the float2 accesses legal
+    const long long i = i_first + ((long long)blockIdx.x * kThreads + threadIdx.x) * 2;
+    if (!FULL && i >= n) return;
+    const bool two = FULL || (i + 1 < n);   // ld % 4 == 0 and 16-byte aligned bases make the float2 accesses legal
     auto ld2 = [&](const float* p) -> f2 {
         if (two) return __ldg(reinterpret_cast<const float2*>(p + i));
         const float v = __ldg(p + i);
@@ -148,7 +150,7 @@ props_fixed_kernel(const __grid_constant__ PropTables<K> tab, long long n, long 
     // ---- mixture-averaged diffusivities (A7) ---------------------------------------------
     if (D_o) {
         const f2 p = ld2(pg);
-        const f2 scale = make_float2(T.x * sqrtT.x / p.x, T.y * sqrtT.y / p.y);
+        const f2 scale = mul2(mul2(T, sqrtT), rcp2(p));
         f2 S[K];
 #pragma unroll
         for (int k = 0; k < K; ++k) S[k] = bc(0.f);
@@ -177,7 +179,9 @@ props_fixed_kernel(const __grid_constant__ PropTables<K> tab, long long n, long 
             const f2 Nk = add2(pre, suf[k + 1]);
             pre = add2(pre, Y[k]);
             const f2 dk = poly4_2(tab.ddiag[k], u);
-            const f2 Dk = make_float2(S[k].x > 0.f ? Nk.x / S[k].x : dk.x, S[k].y > 0.f ? Nk.y / S[k].y : dk.y);
+            // MUFU reciprocal (1e-7) instead of the IEEE division: the 2 x 19 divisions were 17 % of the kernel's PC samples
+            const f2 q = mul2(Nk, rcp2(S[k]));
+            const f2 Dk = make_float2(S[k].x > 0.f ? q.x : dk.x, S[k].y > 0.f ? q.y : dk.y);
             st2(D_o + (size_t)k * ld, mul2(Dk, scale));
         }
     }
@@ -186,11 +190,17 @@ props_fixed_kernel(const __grid_constant__ PropTables<K> tab, long long n, long 
 template <int K>
 df_status launch_fixed(const PropTables<K>* tab, long long n, long long ld, const float* T, const float* p,
                        const float* Y, float* cp, float* h, float* mu, float* lam, float* D, cudaStream_t s) {
-    const unsigned blocks = (unsigned)((n + 2 * kThreads - 1) / (2 * kThreads));
-    if (mu || lam || D)
-        props_fixed_kernel<K, true><<<blocks, kThreads, 0, s>>>(*tab, n, ld, T, p, Y, cp, h, mu, lam, D);
-    else
-        props_fixed_kernel<K, false><<<blocks, kThreads, 0, s>>>(*tab, n, ld, T, p, Y, cp, h, mu, lam, D);
+    constexpr long long per_block = 2 * kThreads;
+    const long long full_blocks = n / per_block, tail_first = full_blocks * per_block;
+    const bool transport = mu || lam || D;
+    if (full_blocks > 0) {
+        if (transport) props_fixed_kernel<K, true, true><<<(unsigned)full_blocks, kThreads, 0, s>>>(*tab, 0, n, ld, T, p, Y, cp, h, mu, lam, D);
+        else props_fixed_kernel<K, false, true><<<(unsigned)full_blocks, kThreads, 0, s>>>(*tab, 0, n, ld, T, p, Y, cp, h, mu, lam, D);
+    }
+    if (tail_first < n) {   // the ragged last block
+        if (transport) props_fixed_kernel<K, true, false><<<1, kThreads, 0, s>>>(*tab, tail_first, n, ld, T, p, Y, cp, h, mu, lam, D);
+        else props_fixed_kernel<K, false, false><<<1, kThreads, 0, s>>>(*tab, tail_first, n, ld, T, p, Y, cp, h, mu, lam, D);
+    }
     DF_CUDA_TRY(cudaGetLastError());
     return DF_OK;
 }
