@@ -91,13 +91,15 @@ struct TfhTables {
     MechScalars sc;
 };
 
-template <int K>
+// FULL: every thread has both of its cells inside the field (the ragged last block is launched separately): plain
+// float2 accesses without the two-path predicates -- the kernel is issue-bound, every instruction counts.
+template <int K, bool FULL>
 __global__ void __launch_bounds__(kThreads, 6)
-t_from_h_fixed_kernel(const __grid_constant__ TfhTables<K> tab, long long n, long long ld, const float* __restrict__ h,
+t_from_h_fixed_kernel(const __grid_constant__ TfhTables<K> tab, long long i_first, long long n, long long ld, const float* __restrict__ h,
                       const float* __restrict__ Y, float* __restrict__ T, float* __restrict__ cp_out, int* __restrict__ n_unconv) {
-    const long long i = ((long long)blockIdx.x * kThreads + threadIdx.x) * 2;
-    if (i >= n) return;
-    const bool two = i + 1 < n;   // ld % 4 == 0 and 16-byte aligned bases make the float2 accesses legal
+    const long long i = i_first + ((long long)blockIdx.x * kThreads + threadIdx.x) * 2;
+    if (!FULL && i >= n) return;
+    const bool two = FULL || i + 1 < n;   // ld % 4 == 0 and 16-byte aligned bases make the float2 accesses legal
     auto ld2 = [&](const float* p) -> float2 {
         if (two) return __ldg(reinterpret_cast<const float2*>(p + i));
         const float v = __ldg(p + i);
@@ -144,8 +146,8 @@ t_from_h_fixed_kernel(const __grid_constant__ TfhTables<K> tab, long long n, lon
 template <int K>
 df_status launch_fixed(const df_mech* mech, long long n, long long ld, const float* h, const float* Y, float* T, float* cp,
                        int* n_unconv, cudaStream_t s) {
-    const long long blocks = (n + 2 * kThreads - 1) / (2 * kThreads);
-    if (blocks > 0x7fffffffLL) return df_set_error(DF_ERR_UNSUPPORTED, "df_thermo_T_from_h: n_cells too large");
+    const long long full_blocks = n / (2 * kThreads), tail_first = full_blocks * 2 * kThreads;
+    if (full_blocks > 0x7fffffffLL) return df_set_error(DF_ERR_UNSUPPORTED, "df_thermo_T_from_h: n_cells too large");
     TfhTables<K> tab;
     for (int k = 0; k < K; ++k)
         for (int m = 0; m < 6; ++m) {
@@ -153,7 +155,8 @@ df_status launch_fixed(const df_mech* mech, long long n, long long ld, const flo
             tab.dlo[k][m] = (float)(mech->th64_host[(k * 2) * 6 + m] - mech->th64_host[(k * 2 + 1) * 6 + m]);
         }
     tab.sc = mech->dev.sc;
-    t_from_h_fixed_kernel<K><<<(unsigned)blocks, kThreads, 0, s>>>(tab, n, ld, h, Y, T, cp, n_unconv);
+    if (full_blocks > 0) t_from_h_fixed_kernel<K, true><<<(unsigned)full_blocks, kThreads, 0, s>>>(tab, 0, n, ld, h, Y, T, cp, n_unconv);
+    if (tail_first < n) t_from_h_fixed_kernel<K, false><<<1, kThreads, 0, s>>>(tab, tail_first, n, ld, h, Y, T, cp, n_unconv);
     DF_CUDA_TRY(cudaGetLastError());
     return DF_OK;
 }
