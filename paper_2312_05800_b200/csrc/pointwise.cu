@@ -14,9 +14,12 @@ constexpr int kPT = 128;   // threads per block, 4 cells each
 struct F4 {
     float v[4];
 };
+// FULL (template parameter of the kernels): all four cells of every thread are inside the field -- the ragged last
+// block is launched separately -- so the accesses are plain float4 without the two-path branch.
+template <bool FULL>
 __device__ __forceinline__ F4 load4(const float* __restrict__ p, long long i0, long long n, float fill) {
     F4 r;
-    if (i0 + 4 <= n) {
+    if (FULL || i0 + 4 <= n) {
         const float4 t = __ldg(reinterpret_cast<const float4*>(p + i0));
         r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w;
     } else {
@@ -25,8 +28,9 @@ __device__ __forceinline__ F4 load4(const float* __restrict__ p, long long i0, l
     }
     return r;
 }
+template <bool FULL>
 __device__ __forceinline__ void store4(float* __restrict__ p, long long i0, long long n, const F4& r) {
-    if (i0 + 4 <= n) {
+    if (FULL || i0 + 4 <= n) {
         *reinterpret_cast<float4*>(p + i0) = make_float4(r.v[0], r.v[1], r.v[2], r.v[3]);
     } else {
 #pragma unroll
@@ -36,8 +40,9 @@ __device__ __forceinline__ void store4(float* __restrict__ p, long long i0, long
 }
 
 // ---- NEXT-4 ------------------------------------------------------------------------------------------------------
+template <bool FULL>
 __global__ void __launch_bounds__(kPT)
-extras_kernel(MechDev md, long long n, long long ld, const float* __restrict__ Tg, const float* __restrict__ pg,
+extras_kernel(MechDev md, long long i_first, long long n, long long ld, const float* __restrict__ Tg, const float* __restrict__ pg,
               const float* __restrict__ Yg, const float* __restrict__ cpg, const float* __restrict__ lamg,
               const float* __restrict__ Dg, float* __restrict__ rho_o, float* __restrict__ psi_o,
               float* __restrict__ alpha_o, float* __restrict__ rhoD_o, float* __restrict__ hk_o, float* __restrict__ s_o) {
@@ -52,9 +57,9 @@ extras_kernel(MechDev md, long long n, long long ld, const float* __restrict__ T
     }
     for (int e = threadIdx.x; e < K; e += kPT) sIW[e] = md.invW[e];
     __syncthreads();
-    const long long i0 = ((long long)blockIdx.x * kPT + threadIdx.x) * 4;
-    if (i0 >= n) return;
-    const F4 T = load4(Tg, i0, n, 1000.f), p = load4(pg, i0, n, 101325.f);
+    const long long i0 = i_first + ((long long)blockIdx.x * kPT + threadIdx.x) * 4;
+    if (!FULL && i0 >= n) return;
+    const F4 T = load4<FULL>(Tg, i0, n, 1000.f), p = load4<FULL>(pg, i0, n, 101325.f);
 
     // ONE pass over Y: 1/Wbar and, when the entropy is wanted, sum_k Y_k s_k(T) and sum_k x_k ln x_k (x_k = Y_k/W_k):
     //   s = sum_k Y_k s_k/W_k - R sum_k x_k ln(x_k Wbar) - (R/Wbar) ln(p/p0)
@@ -69,7 +74,7 @@ extras_kernel(MechDev md, long long n, long long ld, const float* __restrict__ T
     }
     float invWbar[4] = {0.f, 0.f, 0.f, 0.f}, sy[4] = {0.f, 0.f, 0.f, 0.f}, sxlx[4] = {0.f, 0.f, 0.f, 0.f};
     for (int k = 0; k < K; ++k) {
-        const F4 y = load4(Yg + (size_t)k * ld, i0, n, 0.f);
+        const F4 y = load4<FULL>(Yg + (size_t)k * ld, i0, n, 0.f);
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
             const float x = y.v[c] * sIW[k];
@@ -89,30 +94,30 @@ extras_kernel(MechDev md, long long n, long long ld, const float* __restrict__ T
         psi.v[c] = 1.0f / (invWbar[c] * Ru * T.v[c]);
         rho.v[c] = p.v[c] * psi.v[c];
     }
-    if (rho_o) store4(rho_o, i0, n, rho);
-    if (psi_o) store4(psi_o, i0, n, psi);
+    if (rho_o) store4<FULL>(rho_o, i0, n, rho);
+    if (psi_o) store4<FULL>(psi_o, i0, n, psi);
     if (alpha_o) {
-        const F4 cp = load4(cpg, i0, n, 1.f), lam = load4(lamg, i0, n, 0.f);
+        const F4 cp = load4<FULL>(cpg, i0, n, 1.f), lam = load4<FULL>(lamg, i0, n, 0.f);
         F4 a;
 #pragma unroll
         for (int c = 0; c < 4; ++c) a.v[c] = lam.v[c] / cp.v[c];
-        store4(alpha_o, i0, n, a);
+        store4<FULL>(alpha_o, i0, n, a);
     }
     if (s_o) {
         F4 o;
 #pragma unroll
         for (int c = 0; c < 4; ++c)
             o.v[c] = sy[c] - Ru * (sxlx[c] - invWbar[c] * logf(invWbar[c])) - Ru * invWbar[c] * logf(p.v[c] * (1.0f / 101325.0f));
-        store4(s_o, i0, n, o);
+        store4<FULL>(s_o, i0, n, o);
     }
     if (!rhoD_o && !hk_o) return;
     for (int k = 0; k < K; ++k) {
         if (rhoD_o) {
-            const F4 d = load4(Dg + (size_t)k * ld, i0, n, 0.f);
+            const F4 d = load4<FULL>(Dg + (size_t)k * ld, i0, n, 0.f);
             F4 o;
 #pragma unroll
             for (int c = 0; c < 4; ++c) o.v[c] = rho.v[c] * d.v[c];
-            store4(rhoD_o + (size_t)k * ld, i0, n, o);
+            store4<FULL>(rhoD_o + (size_t)k * ld, i0, n, o);
         }
         if (hk_o) {
             F4 o;
@@ -121,7 +126,7 @@ extras_kernel(MechDev md, long long n, long long ld, const float* __restrict__ T
                 const float* q = sTh + k * 12 + (lo[c] ? 0 : 6);
                 o.v[c] = fmaf(fmaf(fmaf(fmaf(fmaf(q[5], tau[c], q[4]), tau[c], q[3]), tau[c], q[2]), tau[c], q[1]), tau[c], q[0]);
             }
-            store4(hk_o + (size_t)k * ld, i0, n, o);
+            store4<FULL>(hk_o + (size_t)k * ld, i0, n, o);
         }
     }
 }
@@ -130,20 +135,21 @@ extras_kernel(MechDev md, long long n, long long ld, const float* __restrict__ T
 // One pass over Y and omega: rho factors out of the slowest time scale, tau_c = rho max_k Y_k/|omega_k|; the omega rows
 // are read again for the scaling (a variant that kept them in registers for K <= 24 needed 140 registers and ran 45 %
 // slower: the occupancy is worth more than the 4 K bytes per cell, which come from L2 mostly).
+template <bool FULL>
 __global__ void __launch_bounds__(kPT)
-pasr_kernel(MechDev md, long long n, long long ld, const float* __restrict__ Tg, const float* __restrict__ pg,
+pasr_kernel(MechDev md, long long i_first, long long n, long long ld, const float* __restrict__ Tg, const float* __restrict__ pg,
             const float* __restrict__ Yg, const float* __restrict__ mug, const float* __restrict__ kg,
             const float* __restrict__ eg, float T_gate, float* omega, float* __restrict__ kappa_o) {
     extern __shared__ float sm[];
     const int K = md.K;
     for (int e = threadIdx.x; e < K; e += kPT) sm[e] = md.invW[e];
     __syncthreads();
-    const long long i0 = ((long long)blockIdx.x * kPT + threadIdx.x) * 4;
-    if (i0 >= n) return;
-    const F4 T = load4(Tg, i0, n, 1000.f), p = load4(pg, i0, n, 101325.f);
+    const long long i0 = i_first + ((long long)blockIdx.x * kPT + threadIdx.x) * 4;
+    if (!FULL && i0 >= n) return;
+    const F4 T = load4<FULL>(Tg, i0, n, 1000.f), p = load4<FULL>(pg, i0, n, 101325.f);
     float invWbar[4] = {0.f, 0.f, 0.f, 0.f}, m[4] = {0.f, 0.f, 0.f, 0.f};
     for (int k = 0; k < K; ++k) {
-        const F4 y = load4(Yg + (size_t)k * ld, i0, n, 0.f), w = load4(omega + (size_t)k * ld, i0, n, 0.f);
+        const F4 y = load4<FULL>(Yg + (size_t)k * ld, i0, n, 0.f), w = load4<FULL>(omega + (size_t)k * ld, i0, n, 0.f);
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
             invWbar[c] = fmaf(y.v[c], sm[k], invWbar[c]);
@@ -151,7 +157,7 @@ pasr_kernel(MechDev md, long long n, long long ld, const float* __restrict__ Tg,
             if (a > 0.f) m[c] = fmaxf(m[c], y.v[c] * rcp_approx(a));   // species that do not react do not count
         }
     }
-    const F4 mu = load4(mug, i0, n, 1.f), ks = load4(kg, i0, n, 1.f), ep = load4(eg, i0, n, 1.f);
+    const F4 mu = load4<FULL>(mug, i0, n, 1.f), ks = load4<FULL>(kg, i0, n, 1.f), ep = load4<FULL>(eg, i0, n, 1.f);
     F4 kappa;
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
@@ -163,12 +169,12 @@ pasr_kernel(MechDev md, long long n, long long ld, const float* __restrict__ Tg,
         if (T.v[c] < T_gate) kp = 0.f;
         kappa.v[c] = kp;
     }
-    if (kappa_o) store4(kappa_o, i0, n, kappa);
+    if (kappa_o) store4<FULL>(kappa_o, i0, n, kappa);
     for (int k = 0; k < K; ++k) {
-        F4 w = load4(omega + (size_t)k * ld, i0, n, 0.f);
+        F4 w = load4<FULL>(omega + (size_t)k * ld, i0, n, 0.f);
 #pragma unroll
         for (int c = 0; c < 4; ++c) w.v[c] *= kappa.v[c];
-        store4(omega + (size_t)k * ld, i0, n, w);
+        store4<FULL>(omega + (size_t)k * ld, i0, n, w);
     }
 }
 
@@ -198,9 +204,14 @@ extern "C" df_status df_thermo_extras(const df_mech* mech, long long n, long lon
     const void* ptrs[] = {T, p, Y, cp, lambda, D, rho, psi, alpha, rhoD, hk, s};
     for (const void* q : ptrs)
         if (!aligned16(q)) return df_set_error(DF_ERR_INVALID_ARG, "df_thermo_extras: fields must be 16-byte aligned");
-    const unsigned blocks = (unsigned)((n + 4LL * kPT - 1) / (4LL * kPT));
+    const long long full_blocks = n / (4LL * kPT), tail_first = full_blocks * 4LL * kPT;
     const size_t smem = (size_t)mech->K * 25 * sizeof(float);
-    extras_kernel<<<blocks, kPT, smem, (cudaStream_t)stream>>>(mech->dev, n, ld, T, p, Y, cp, lambda, D, rho, psi, alpha, rhoD, hk, s);
+    if (full_blocks > 0)
+        extras_kernel<true><<<(unsigned)full_blocks, kPT, smem, (cudaStream_t)stream>>>(mech->dev, 0, n, ld, T, p, Y, cp, lambda, D, rho, psi,
+                                                                                       alpha, rhoD, hk, s);
+    if (tail_first < n)
+        extras_kernel<false><<<1, kPT, smem, (cudaStream_t)stream>>>(mech->dev, tail_first, n, ld, T, p, Y, cp, lambda, D, rho, psi, alpha,
+                                                                     rhoD, hk, s);
     DF_CUDA_TRY(cudaGetLastError());
     return DF_OK;
 }
@@ -215,9 +226,13 @@ extern "C" df_status df_chem_pasr_scale(const df_mech* mech, long long n, long l
     const void* ptrs[] = {T, p, Y, mu, k_sgs, eps, omega, kappa};
     for (const void* q : ptrs)
         if (!aligned16(q)) return df_set_error(DF_ERR_INVALID_ARG, "df_chem_pasr_scale: fields must be 16-byte aligned");
-    const unsigned blocks = (unsigned)((n + 4LL * kPT - 1) / (4LL * kPT));
-    pasr_kernel<<<blocks, kPT, (size_t)mech->K * sizeof(float), (cudaStream_t)stream>>>(mech->dev, n, ld, T, p, Y, mu, k_sgs, eps,
-                                                                                       T_gate, omega, kappa);
+    const long long full_blocks = n / (4LL * kPT), tail_first = full_blocks * 4LL * kPT;
+    const size_t smem = (size_t)mech->K * sizeof(float);
+    if (full_blocks > 0)
+        pasr_kernel<true><<<(unsigned)full_blocks, kPT, smem, (cudaStream_t)stream>>>(mech->dev, 0, n, ld, T, p, Y, mu, k_sgs, eps, T_gate,
+                                                                                     omega, kappa);
+    if (tail_first < n)
+        pasr_kernel<false><<<1, kPT, smem, (cudaStream_t)stream>>>(mech->dev, tail_first, n, ld, T, p, Y, mu, k_sgs, eps, T_gate, omega, kappa);
     DF_CUDA_TRY(cudaGetLastError());
     return DF_OK;
 }
