@@ -1,13 +1,17 @@
 // ann_fp32.cu -- K3: the ANN source term on the fp32 FFMA path (precision 0; BASELINE config 1,
 // 11 -> 64 -> 64 -> 9).  Tensor cores cannot meet the 1e-5 tolerance of this path, so it is plain
-// FFMA: one thread per cell, activations ping-pong through shared memory ([feature][thread],
-// conflict-free), weights W^T[in][out] read warp-uniformly through the read-only path as float4,
-// 8 outputs register-blocked per pass over the inputs.  Exact erf GELU (A13).
+// FFMA.  A block owns 32 cells; lane = cell, and the eight warps split every layer's outputs (warp j takes outputs
+// 8j .. 8j+7, then +64, ...: a cell's serial chain is an eighth of the layer), activations ping-pong through shared
+// memory ([feature][cell], conflict-free), weights W^T[in][out] are read warp-uniformly through the read-only path as
+// float4.  Exact erf GELU (A13).  The configuration is launch/latency-bound (4096 cells), so what counts is the length
+// of the per-cell dependency chain, not throughput.
 #include "ann_common.cuh"
 
 namespace {
 
-constexpr int kThreads = 64;
+constexpr int kCells = 32;               // cells per block (one per lane)
+constexpr int kSplit = 8;                // warps per block = output slices
+constexpr int kThreads = kCells * kSplit;
 constexpr int kMaxLayers = 8;
 
 struct Fp32Net {
@@ -24,26 +28,29 @@ ann_fp32_kernel(Fp32Net net, AnnNorm nm, int K, const float* __restrict__ invW, 
                 const float* __restrict__ Tg, const float* __restrict__ pg, const float* __restrict__ Yg,
                 float* __restrict__ omega, float* __restrict__ dY) {
     extern __shared__ float sm[];
-    const int t = threadIdx.x;
+    const int c = threadIdx.x & 31, j = threadIdx.x >> 5;
     float* act0 = sm;
-    float* act1 = sm + (size_t)net.max_dim * kThreads;
-    const long long i = (long long)blockIdx.x * kThreads + t;
-    if (i >= n) return;
+    float* act1 = sm + (size_t)net.max_dim * kCells;
+    const long long i_raw = (long long)blockIdx.x * kCells + c;
+    const bool valid = i_raw < n;
+    const long long i = valid ? i_raw : 0;   // every thread stays for the barriers; cells past the end are not stored
 
     const float T = __ldg(Tg + i), p = __ldg(pg + i);
-    act0[0 * kThreads + t] = (T - nm.x_mean[0]) * nm.x_inv_std[0];
-    act0[1 * kThreads + t] = (p - nm.x_mean[1]) * nm.x_inv_std[1];
-    for (int k = 0; k < K; ++k) {
-        const float y = __ldg(Yg + (size_t)k * ld + i);
-        act0[(2 + k) * kThreads + t] = ann_feature_Y(y, nm.lambda, nm.inv_lambda, nm.x_mean[2 + k], nm.x_inv_std[2 + k]);
+    for (int f = j; f < K + 2; f += kSplit) {
+        float x;
+        if (f == 0) x = (T - nm.x_mean[0]) * nm.x_inv_std[0];
+        else if (f == 1) x = (p - nm.x_mean[1]) * nm.x_inv_std[1];
+        else x = ann_feature_Y(__ldg(Yg + (size_t)(f - 2) * ld + i), nm.lambda, nm.inv_lambda, nm.x_mean[f], nm.x_inv_std[f]);
+        act0[f * kCells + c] = x;
     }
+    __syncthreads();
 
     float* in = act0;
     float* out = act1;
     for (int l = 0; l < net.n_layers; ++l) {
         const int din = net.dims[l], dout = net.dims[l + 1], op = net.out_pad[l];
         const bool last = (l + 1 == net.n_layers);
-        for (int o = 0; o < dout; o += 8) {
+        for (int o = j * 8; o < dout; o += 8 * kSplit) {
             float acc[8];
             const float4 b0 = __ldg(reinterpret_cast<const float4*>(net.b[l] + o));
             const float4 b1 = __ldg(reinterpret_cast<const float4*>(net.b[l] + o + 4));
@@ -52,7 +59,7 @@ ann_fp32_kernel(Fp32Net net, AnnNorm nm, int K, const float* __restrict__ invW, 
             const float* w = net.WT[l] + o;
 #pragma unroll 4
             for (int ii = 0; ii < din; ++ii) {
-                const float a = in[ii * kThreads + t];
+                const float a = in[ii * kCells + c];
                 const float4 w0 = __ldg(reinterpret_cast<const float4*>(w + (size_t)ii * op));
                 const float4 w1 = __ldg(reinterpret_cast<const float4*>(w + (size_t)ii * op + 4));
                 acc[0] = fmaf(a, w0.x, acc[0]); acc[1] = fmaf(a, w0.y, acc[1]);
@@ -61,32 +68,38 @@ ann_fp32_kernel(Fp32Net net, AnnNorm nm, int K, const float* __restrict__ invW, 
                 acc[6] = fmaf(a, w1.z, acc[6]); acc[7] = fmaf(a, w1.w, acc[7]);
             }
 #pragma unroll
-            for (int j = 0; j < 8; ++j)
-                if (o + j < dout) out[(o + j) * kThreads + t] = last ? acc[j] : gelu_erf(acc[j]);
+            for (int q = 0; q < 8; ++q)
+                if (o + q < dout) out[(o + q) * kCells + c] = last ? acc[q] : gelu_erf(acc[q]);
         }
+        __syncthreads();
         float* tmp = in; in = out; out = tmp;
     }
-    // `in` now holds the K network outputs o_k; `out` is scratch for dY*_k.
+    // `in` now holds the K network outputs o_k; `out` is scratch for dY*_k (species k = j, j + 8, ... per warp).
+    for (int k = j; k < K; k += kSplit) {
+        const float y = __ldg(Yg + (size_t)k * ld + i);
+        const float delta = fmaf(nm.u_std[k], in[k * kCells + c], nm.u_mean[k]);
+        out[k * kCells + c] = ann_dystar(y, delta, nm.lambda, nm.inv_lambda);
+    }
+    __syncthreads();
+    // every warp forms the two sums in the same order (bitwise identical in all of them), then finishes its species
     double sumYm1 = -1.0, sumd = 0.0;
     float inv_Wbar = 0.f;
     for (int k = 0; k < K; ++k) {
         const float y = __ldg(Yg + (size_t)k * ld + i);
-        const float delta = fmaf(nm.u_std[k], in[k * kThreads + t], nm.u_mean[k]);
-        const float d = ann_dystar(y, delta, nm.lambda, nm.inv_lambda);
-        out[k * kThreads + t] = d;
         sumYm1 += (double)y;
-        sumd += (double)d;
+        sumd += (double)out[k * kCells + c];
         inv_Wbar = fmaf(y, __ldg(invW + k), inv_Wbar);
     }
     const double Sm1 = sumYm1 + sumd;
     const double inv_S = 1.0 / (1.0 + Sm1);
     const float rho_dt = p / (inv_Wbar * (float)DF_R_UNIVERSAL * T) * nm.inv_dt;  // A17
-    for (int k = 0; k < K; ++k) {
-        const float y = __ldg(Yg + (size_t)k * ld + i);
-        const float d = ann_renorm_dY(out[k * kThreads + t], y, Sm1, inv_S);
-        if (dY) dY[(size_t)k * ld + i] = d;
-        if (omega) omega[(size_t)k * ld + i] = rho_dt * d;
-    }
+    if (valid)
+        for (int k = j; k < K; k += kSplit) {
+            const float y = __ldg(Yg + (size_t)k * ld + i);
+            const float d = ann_renorm_dY(out[k * kCells + c], y, Sm1, inv_S);
+            if (dY) dY[(size_t)k * ld + i] = d;
+            if (omega) omega[(size_t)k * ld + i] = rho_dt * d;
+        }
 }
 
 }  // namespace
@@ -105,11 +118,11 @@ df_status launch_ann_fp32(const df_ann* ann, const df_mech* mech, long long n, l
         net.WT[l] = ann->w32 + ann->w32_off[l];
         net.b[l] = ann->w32 + ann->b32_off[l];
     }
-    const size_t smem = (size_t)2 * net.max_dim * kThreads * sizeof(float);
+    const size_t smem = (size_t)2 * net.max_dim * kCells * sizeof(float);
     static DfPerDevice smem_attr;
     const df_status st = df_ensure_dyn_smem((const void*)ann_fp32_kernel, 200 * 1024, &smem_attr);
     if (st != DF_OK) return st;
-    const long long blocks = (n + kThreads - 1) / kThreads;
+    const long long blocks = (n + kCells - 1) / kCells;
     if (blocks > 0x7fffffffLL) return df_set_error(DF_ERR_UNSUPPORTED, "df_chem_ann_source: n_cells too large");
     ann_fp32_kernel<<<(unsigned)blocks, kThreads, smem, s>>>(net, ann->norm, ann->K, mech->dev.invW, n, ld, T, p, Y,
                                                             omega, dY);
