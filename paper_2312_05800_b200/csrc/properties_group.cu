@@ -18,9 +18,10 @@
 //            the four warps add into the shared S accumulators without atomics and every round is balanced; two more
 //            rounds take the 8 diagonal tiles.  One block barrier per round.  A warp stages its own coefficient tile
 //            (<= 1280 B, in loop order) with cp.async one round ahead.
-//   final    D_k = N_k / S_k, N_k = sum_{j != k} Y_j evaluated as (sum_j Y_j) - Y_k with the sum carried as an
-//            unevaluated float-float pair (TwoSum) over the exact fp32 Y: what A7 warns of is the rounding of the
-//            fp32 sum, amplified by the cancellation; the pair is exact to ~1e-14 sum Y.  Self-diffusion D_kk when S_k = 0.
+//   final    D_k = N_k / S_k, N_k = sum_{j != k} Y_j evaluated as (sum_j Y_j) - Y_k with the sum formed in fp64 over the
+//            exact fp32 Y (phase 1, where Y is converted for the enthalpy anyway) and handed on as an unevaluated
+//            float-float pair: what A7 warns of is the rounding of the fp32 sum, amplified by the cancellation; the
+//            pair is exact to ~1e-14 sum Y.  Self-diffusion D_kk when S_k = 0.
 // A block is one group; it loops over groups (grid-stride) so the tables are staged once per block.
 #include "common.cuh"
 

@@ -68,9 +68,11 @@ def test_T_from_h(B, cfg, n, ld, guess):
 @pytest.mark.parametrize("n,ld", [(1, 4), (127, 128), (129, 132), (257, 260), (1000, 1000)])
 @pytest.mark.parametrize("side", ["lo", "hi", "mid", "mixed"])
 def test_T_from_h_range_sorted_blocks(B, n, ld, side):
-    """The fixed-K kernel sorts each 256-cell block by NASA range before the coefficient pass: blocks that are all
-    lo, all hi, sit on T_mid (either polynomial is right there, A2) or mix both, at sizes around the warp / block
-    boundaries, must all come back to the oracle's root; the pad between n and ld must stay untouched."""
+    """The fixed-K kernel decides the NASA range of a cell before it iterates (hi iff h >= h(T_mid, Y)) and gives
+    low-range cells an fp32 correction on top of the fp64 high-range coefficients: fields that are all lo, all hi, sit on
+    T_mid (either polynomial is right there, A2) or mix both, at sizes around the warp / block boundaries (the ragged
+    last block is a launch of its own), must all come back to the oracle's root; the pad between n and ld must stay
+    untouched."""
     mech, _, cells, om = make_case(3, n, ld)
     rng = np.random.default_rng(n * 7 + len(side))
     if side == "lo":
