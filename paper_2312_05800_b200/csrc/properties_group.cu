@@ -7,8 +7,9 @@
 // in shared memory ([species][lane] float2: 0.5 KB per species), and the species dimension of every phase is split
 // over the four warps -- a quarter of the shared memory per warp (12 warps per SM) and a quarter of the serial work
 // per thread:
-//   phase 1  thermo + x_k = Y_k/W_k            species k = w, w+4, ...; partial sums combined through shared memory
-//   phase 2  X_k, r_k = 1/ghat_k, conductivity  same split
+//   phase 1  x_k = Y_k/W_k, thermo, r_k = 1/ghat_k, conductivity   species k = w, w+4, ...; partial sums combined
+//            through shared memory.  (x_k is never normalised to X_k: Wilke's ratio does not care, the conductivity
+//            and S_k are corrected by sum(x) at the end -- so nothing here waits for a sum over species)
 //   phase 3  Wilke: warp w owns rows k in [w Kp/4, (w+1) Kp/4) (accumulators in registers) and streams all j:
 //            den_k += B_kj (X_j + g_k (2 X_j r_j + g_k X_j r_j^2)) -- three FFMA2 per (k, j), B_kj from a table re-tiled
 //            per warp so that a row segment is four broadcast LDS.128
@@ -188,6 +189,8 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
         }
         const f2 tau = mul2(add2(T, bc(-md.sc.T_mid)), md.sc.inv_S);
         const bool lo0 = T.x < md.sc.T_mid, lo1 = T.y < md.sc.T_mid;   // A2: hi for T >= T_mid
+        const f2 u = mul2(add2(make_float2(logf(T.x), logf(T.y)), bc(-md.sc.Lc)), md.sc.inv_Ls);
+        const f2 sqrtT = make_float2(sqrtf(T.x), sqrtf(T.y));
 
         // ---- phase 1: x_k = Y_k / W_k and the thermo sums of this warp's species --------------------------------
         {
@@ -197,14 +200,23 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
 #pragma unroll
             for (int m = 0; m < 5; ++m) Cl[m] = Ch[m] = bc(0.f);
             double H0la = 0.0, H0ha = 0.0, H0lb = 0.0, H0hb = 0.0, Yta = 0.0, Ytb = 0.0;
-            f2 sumx = bc(0.f);
+            f2 sumx = bc(0.f), s1 = bc(0.f), s2 = bc(0.f);
 #pragma unroll
             for (int a = 0; a < KW; ++a) {
                 const int k = w + 4 * a;
                 const f2 y = yv[a];
-                const f2 x = mul2(y, sSmall[k * kSmallStride]);
+                const float4 ta = *reinterpret_cast<const float4*>(sSmall + k * kSmallStride);   // invW sqrtW v0 v1
+                const f2 x = mul2(y, ta.x);
                 sX[k * 32 + lane] = x;
                 sumx = add2(sumx, x);
+                if (want_transport) {   // r_k = 1/ghat_k and the conductivity sums, on the unnormalised x_k
+                    const float4 tb = *reinterpret_cast<const float4*>(sSmall + k * kSmallStride + 4),   // v2 v3 v4 c0
+                                 tc = *reinterpret_cast<const float4*>(sSmall + k * kSmallStride + 8);   // c1 c2 c3 c4
+                    sR[k * 32 + lane] = rcp2(poly4_2(ta.z, ta.w, tb.x, tb.y, tb.z, u));
+                    const f2 lk = poly4_2(tb.w, tc.x, tc.y, tc.z, tc.w, u);
+                    s1 = fma2(x, lk, s1);
+                    s2 = fma2(x, rcp2(lk), s2);
+                }
                 if ((want_thermo && h_o) || D_o) {
                     const double ya = (double)y.x, yb = (double)y.y;
                     if (D_o) {   // sum_j Y_j in fp64 (exact on the fp32 inputs to 1e-16): N_k = sum - Y_k without the fp32 rounding of the sum
@@ -228,6 +240,8 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
             }
             f2* my = sScr + (w * kScrSlots) * 32 + lane;
             my[0] = sumx;
+            my[8 * 32] = s1;
+            my[9 * 32] = s2;
             if (D_o) {   // the warp's share of sum Y as a float-float pair
                 const f2 hi = make_float2((float)Yta, (float)Ytb);
                 my[11 * 32] = hi;
@@ -272,28 +286,9 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
             continue;
         }
 
-        // ---- phase 2: X_k, r_k = 1/ghat_k, conductivity sums -----------------------------------------------------
-        const f2 inv_sumx = make_float2(1.0f / sumx.x, 1.0f / sumx.y);
-        const f2 u = mul2(add2(make_float2(logf(T.x), logf(T.y)), bc(-md.sc.Lc)), md.sc.inv_Ls);
-        const f2 sqrtT = make_float2(sqrtf(T.x), sqrtf(T.y));
-        {
-            f2 s1 = bc(0.f), s2 = bc(0.f);
-#pragma unroll 2
-            for (int k = w; k < Kp; k += 4) {
-                const f2 X = mul2(sX[k * 32 + lane], inv_sumx);
-                sX[k * 32 + lane] = X;
-                const float4 a = *reinterpret_cast<const float4*>(sSmall + k * kSmallStride), b = *reinterpret_cast<const float4*>(sSmall + k * kSmallStride + 4),
-                             c = *reinterpret_cast<const float4*>(sSmall + k * kSmallStride + 8);   // invW sqrtW v0 v1 | v2 v3 v4 c0 | c1 c2 c3 c4
-                sR[k * 32 + lane] = rcp2(poly4_2(a.z, a.w, b.x, b.y, b.z, u));
-                const f2 lk = poly4_2(b.w, c.x, c.y, c.z, c.w, u);
-                s1 = fma2(X, lk, s1);
-                s2 = fma2(X, rcp2(lk), s2);
-            }
-            f2* my = sScr + (w * kScrSlots + 8) * 32 + lane;   // slots 8, 9 (slot 0..7 may still be read by warp 1)
-            my[0] = s1;
-            my[32] = s2;
-        }
-        __syncthreads();
+        // Mole fractions are never normalised: with x_k = Y_k/W_k = X_k sum(x), Wilke's ratio is unchanged (numerator and
+        // denominator both carry sum(x)), and the conductivity sums and S_k are corrected by sum(x) where they are used.
+        // That makes phase 2 (r_k, conductivity) independent of any sum over species: it runs inside phase 1's loop.
         if (lam_o && w == 0) {
             f2 s1 = bc(0.f), s2 = bc(0.f);
 #pragma unroll
@@ -301,7 +296,8 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
                 s1 = add2(s1, sScr[(v * kScrSlots + 8) * 32 + lane]);
                 s2 = add2(s2, sScr[(v * kScrSlots + 9) * 32 + lane]);
             }
-            st2(lam_o, mul2(mul2(sqrtT, 0.5f), add2(s1, rcp2(s2))));   // A6
+            // A6 with X = x / sum(x): sum X lk = s1 / sum(x), 1 / sum(X / lk) = sum(x) / s2
+            st2(lam_o, mul2(mul2(sqrtT, 0.5f), add2(mul2(s1, rcp2(sumx)), mul2(sumx, rcp2(s2)))));
         }
 
         // ---- phase 3: Wilke; this warp owns rows k0 .. k0 + KW - 1 ------------------------------------------------
@@ -412,7 +408,7 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
                     const f2 S = sR[k * 32 + lane];
                     const float* dd = sSmall + k * kSmallStride + 12;
                     const f2 dk = poly4_2(dd[0], dd[1], dd[2], dd[3], dd[4], u);
-                    const f2 q = mul2(Nk, rcp2x(S));
+                    const f2 q = mul2(mul2(Nk, sumx), rcp2x(S));   // S was accumulated on x = X sum(x)
                     const f2 Dk = make_float2(S.x > 0.f ? q.x : dk.x, S.y > 0.f ? q.y : dk.y);   // A7
                     st2(D_o + (size_t)k * ld, mul2(Dk, scale));
                 }
