@@ -33,6 +33,11 @@ __device__ __forceinline__ f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
 // one MUFU.RCP per half (the shared-reciprocal form 1/x = y/(xy) measured 4 % slower here: its three extra
 // multiplies cannot be packed)
 __device__ __forceinline__ f2 rcp2(f2 a) { return make_float2(rcp_approx(a.x), rcp_approx(a.y)); }
+__device__ __forceinline__ float sqrt_approx(float x) {
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
 __device__ __forceinline__ f2 poly4_2(const float* c, f2 u) {
     return fma2(fma2(fma2(fma2(u, c[4], c[3]), u, bc(c[2])), u, bc(c[1])), u, bc(c[0]));
 }
@@ -114,24 +119,29 @@ props_fixed_kernel(const __grid_constant__ PropTables<K> tab, long long i_first,
 
     // ---- Wilke viscosity ----------------------------------------------------------------------
     if (mu_o) {
-        // Phi_kj = B_kj (1 + g_k/g_j)^2 with only two per-species vectors live (X_j and r_j = 1/g_j): 4 packed
-        // instructions per (k,j) instead of the 3 of the three-vector form, but 76 registers less, which buys the
-        // occupancy this latency-sensitive kernel needs
-        f2 r[K];
-#pragma unroll
-        for (int k = 0; k < K; ++k) r[k] = rcp2(poly4_2(tab.visc[k], u));
+        // x_j Phi_kj = B_kj (sqrt(x_j) + g_k sqrt(x_j)/g_j)^2: two per-species vectors (a_j = sqrt(x_j), b_j = a_j/g_j) and
+        // 3 packed instructions per (k,j) -- the register footprint of the two-vector form at the instruction count of the
+        // three-vector one.  X_j is rebuilt as a_j^2 afterwards (1 ulp; exact for x_j = 0).
+        f2 b[K];
         f2 acc = bc(0.f);
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-            const f2 gk = rcp2(r[k]);
+            X[k] = make_float2(sqrt_approx(X[k].x), sqrt_approx(X[k].y));
+            b[k] = mul2(X[k], rcp2(poly4_2(tab.visc[k], u)));
+        }
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const f2 gk = poly4_2(tab.visc[k], u);
             f2 den = bc(0.f);
 #pragma unroll
             for (int j = 0; j < K; ++j) {
-                const f2 t = fma2(gk, r[j], bc(1.0f));
-                den = fma2(mul2(X[j], mul2(t, t)), tab.B[k][j], den);
+                const f2 t = fma2(gk, b[j], X[j]);
+                den = fma2(mul2(t, t), tab.B[k][j], den);
             }
-            acc = fma2(mul2(mul2(X[k], tab.sqrtW[k]), mul2(gk, gk)), rcp2(den), acc);
+            acc = fma2(mul2(mul2(mul2(X[k], X[k]), tab.sqrtW[k]), mul2(gk, gk)), rcp2(den), acc);
         }
+#pragma unroll
+        for (int k = 0; k < K; ++k) X[k] = mul2(X[k], X[k]);
         st2(mu_o, mul2(sqrtT, acc));
     }
 
@@ -155,6 +165,8 @@ props_fixed_kernel(const __grid_constant__ PropTables<K> tab, long long i_first,
 #pragma unroll
         for (int k = 0; k < K; ++k) S[k] = bc(0.f);
         {
+            // one MUFU per half and pair; sharing a reciprocal between two pairs (1/a = b/(ab): 2 MUFU + 3 packed multiplies
+            // for 4 MUFU) on any share of the pairs measured no faster (0.273-0.277 ms): the loop waits on latency, not on the XU
             int idx = 0;
 #pragma unroll
             for (int j = 0; j < K; ++j)
