@@ -134,6 +134,25 @@ DF_API df_status df_chem_ann_source(const df_ann* ann, const df_mech* mech, long
                              float* omega, float* dY,
                              void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- hot call 3 without a workspace, for callers that may not allocate device memory --------------------------
+ * Same operation, kernel and results as df_chem_ann_source for a precision-1 (tensor path) handle; the kernel's
+ * per-CTA scratch is a static device array inside the library instead of a caller-supplied workspace.  The call
+ * allocates nothing (no cudaMalloc/cudaFree, no allocating library routine).
+ *   - Every GPU that loads the library holds DF_ANN_STATIC_SCRATCH_BYTES of device memory until the process exits.
+ *   - DF_ERR_UNSUPPORTED when df_ann_workspace_bytes(ann, n_cells) exceeds that (the 21-1600-800-400-19 network
+ *     needs 29.4 MiB at any n_cells on a 148-SM device: it fits), or when the handle is not precision 1 (the fp32
+ *     path needs no workspace: df_chem_ann_source with workspace = NULL allocates nothing either).
+ *   - All calls on a device share the one array: calls that overlap on the GPU (different streams with no ordering
+ *     between them) race on it.  Calls on one stream or ordered by events are safe; nothing in the array has to
+ *     start at zero and nothing is carried between calls (every tile writes its chunks before it reads them).
+ *   - The first call on a device looks the array's address up (once per device, not capturable); a call with
+ *     n_cells = 0 does only that, so a caller can run it ahead of a stream capture. */
+#define DF_ANN_STATIC_SCRATCH_BYTES (32u << 20)
+DF_API size_t df_ann_static_scratch_bytes(void);
+DF_API df_status df_chem_ann_source_static(const df_ann* ann, const df_mech* mech, long long n_cells, long long ld,
+                                    const float* T, const float* p, const float* Y,
+                                    float* omega, float* dY, void* stream);
+
 /* ---- one MLP per species ("individual training and prediction are carried out for each
  * species mass fraction", "multiple multilayer perceptrons") --------------------------------------------------
  * K independent networks with dims = {K+2, d1, d2, d3, 1} (n_layers = 4, the tensor path's shapes, see df_ann_create

@@ -27,6 +27,7 @@ SYMBOLS = (
     "df_step_plan_create", "df_thermochem_step", "df_step_plan_destroy",
     "df_host_ctx_create", "df_host_ctx_destroy", "df_step_host",
     "df_probe_fp32_peak",
+    "df_ann_static_scratch_bytes", "df_chem_ann_source_static",
 )
 
 DF_OK, DF_ERR_INVALID_ARG, DF_ERR_UNSUPPORTED, DF_ERR_ALLOC, DF_ERR_CUDA = range(5)
@@ -56,6 +57,9 @@ _lib.df_ann_workspace_bytes.argtypes = [_vp, _ll]
 _lib.df_thermo_T_from_h.argtypes = [_vp, _ll, _ll, _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.df_thermo_properties.argtypes = [_vp, _ll, _ll, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.df_chem_ann_source.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+_lib.df_ann_static_scratch_bytes.restype = _sz
+_lib.df_ann_static_scratch_bytes.argtypes = []
+_lib.df_chem_ann_source_static.argtypes = [_vp, _vp, _ll, _ll, _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.df_thermo_extras.argtypes = [_vp, _ll, _ll] + [_vp] * 13
 _lib.df_chem_pasr_scale.argtypes = [_vp, _ll, _ll, _vp, _vp, _vp, _vp, _vp, _vp, C.c_float, _vp, _vp, _vp]
 _lib.df_ann_mmlp_create.argtypes = [C.POINTER(_vp), _i, _i, _vp, C.POINTER(_vp), C.POINTER(_vp), _vp, _vp, _vp, _vp, _d, _d]
@@ -226,6 +230,17 @@ def df_chem_ann_source(ann: Ann, mech: Mech, T, p, Y, omega=None, dY=None, works
     ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
     _check(_lib.df_chem_ann_source(ann.handle, mech.handle, n, int(Y.shape[1]), _dp(T), _dp(p), _dp(Y), _dp(omega),
                                    _dp(dY), _dp(workspace), ws_bytes, _stream(stream)))
+
+
+def df_ann_static_scratch_bytes() -> int:
+    return int(_lib.df_ann_static_scratch_bytes())
+
+
+def df_chem_ann_source_static(ann: Ann, mech: Mech, T, p, Y, omega=None, dY=None, n_cells=None, stream=None) -> None:
+    """df_chem_ann_source on the library's static device scratch: no workspace argument, no allocation."""
+    n = int(T.shape[0]) if n_cells is None else int(n_cells)
+    _check(_lib.df_chem_ann_source_static(ann.handle, mech.handle, n, int(Y.shape[1]), _dp(T), _dp(p), _dp(Y), _dp(omega),
+                                          _dp(dY), _stream(stream)))
 
 
 def df_thermo_extras(mech: Mech, T, p, Y, cp=None, lam=None, D=None, rho=None, psi=None, alpha=None, rhoD=None, hk=None,
