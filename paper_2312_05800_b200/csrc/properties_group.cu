@@ -56,9 +56,6 @@ __device__ __forceinline__ f2 rcp2x(f2 a) { return make_float2(rcp_approx(a.x), 
 __device__ __forceinline__ f2 poly4_2(float c0, float c1, float c2, float c3, float c4, f2 u) {
     return fma2(fma2(fma2(fma2(u, c4, c3), u, bc(c2)), u, bc(c1)), u, bc(c0));
 }
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
-}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
@@ -66,11 +63,17 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 constexpr int kTileFloatsMax = 8 * 40;   // ring slot: the largest tile (TS = 8: 8 rows of 8 pairs x 5 coefficients)
 __host__ __device__ constexpr int tile_row_floats(int TS) { return (TS * 5 + 3) / 4 * 4; }   // rows start 16-byte aligned
 
-// round-robin tournament of the 8 species tiles (circle method), then the diagonal tiles: [round][warp]
-__constant__ signed char kSchedK[9][4] = {{0, 1, 2, 3}, {0, 5, 1, 2}, {0, 4, 3, 1}, {0, 3, 2, 1}, {0, 2, 1, 6}, {0, 1, 4, 5}, {0, 2, 3, 4}, {0, 1, 2, 3}, {4, 5, 6, 7}};
-__constant__ signed char kSchedJ[9][4] = {{7, 6, 5, 4}, {6, 7, 4, 3}, {5, 6, 7, 2}, {4, 5, 6, 7}, {3, 4, 5, 7}, {2, 3, 7, 6}, {1, 7, 6, 5}, {0, 1, 2, 3}, {4, 5, 6, 7}};
+// round-robin tournament of the 8 species tiles (circle method), then the diagonal tiles: [round][warp], one word per
+// entry: kt | jt << 4 | tile << 8, tile = kt * 8 - kt (kt - 1) / 2 + (jt - kt) the index of the (kt <= jt) tile in the table
+#define DF_T(kt, jt) ((kt) | ((jt) << 4) | (((kt) * 8 - (kt) * ((kt) - 1) / 2 + ((jt) - (kt))) << 8))
+__constant__ int kSched[9][4] = {
+    {DF_T(0, 7), DF_T(1, 6), DF_T(2, 5), DF_T(3, 4)}, {DF_T(0, 6), DF_T(5, 7), DF_T(1, 4), DF_T(2, 3)},
+    {DF_T(0, 5), DF_T(4, 6), DF_T(3, 7), DF_T(1, 2)}, {DF_T(0, 4), DF_T(3, 5), DF_T(2, 6), DF_T(1, 7)},
+    {DF_T(0, 3), DF_T(2, 4), DF_T(1, 5), DF_T(6, 7)}, {DF_T(0, 2), DF_T(1, 3), DF_T(4, 7), DF_T(5, 6)},
+    {DF_T(0, 1), DF_T(2, 7), DF_T(3, 6), DF_T(4, 5)}, {DF_T(0, 0), DF_T(1, 1), DF_T(2, 2), DF_T(3, 3)},
+    {DF_T(4, 4), DF_T(5, 5), DF_T(6, 6), DF_T(7, 7)}};
+#undef DF_T
 constexpr int kRounds = 9;
-__device__ __forceinline__ int tile_index(int kt, int jt) { return kt * 8 - kt * (kt - 1) / 2 + (jt - kt); }   // kt <= jt
 
 // One TS x TS tile of species pairs.  coef: [a][b][5] in shared memory (warp-uniform addresses: broadcast loads).
 template <int TS, bool DIAG>
@@ -119,9 +122,12 @@ __host__ __device__ inline GroupSmem group_smem(int Kp) {
     return g;
 }
 
-template <int KW>   // Wilke rows per warp = Kp / 4
+// KW: Wilke rows per warp = Kp / 4.  FULL: every group of the launch lies inside the field (the host launches the ragged
+// last group separately), so loads and stores are plain float2 accesses.  ALL: all five outputs are wanted (the solver's
+// call), so none of the per-species code is guarded by a runtime flag.
+template <int KW, bool FULL, bool ALL>
 __global__ void __launch_bounds__(kGT, 3)
-props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld, const float* __restrict__ Tg,
+props_group_kernel(const __grid_constant__ MechDev md, long long g_first, long long g_end, long long n, long long ld, const float* __restrict__ Tg,
                    const float* __restrict__ pg, const float* __restrict__ Yg, float* __restrict__ cp_o,
                    float* __restrict__ h_o, float* __restrict__ mu_o, float* __restrict__ lam_o, float* __restrict__ D_o) {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -148,44 +154,45 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
         reinterpret_cast<float4*>(smem + L.BW)[e] = __ldg(reinterpret_cast<const float4*>(md.BW) + e);
     __syncthreads();
 
-    const bool want_thermo = cp_o || h_o, want_transport = mu_o || lam_o || D_o;
-    const long long ngroups = (n + kGroupCells - 1) / kGroupCells;
+    const bool want_h = ALL || h_o, want_cp = ALL || cp_o, want_mu = ALL || mu_o, want_lam = ALL || lam_o, want_D = ALL || D_o;
+    const bool want_thermo = want_cp || want_h, want_transport = want_mu || want_lam || want_D;
+    const long long ngroups = g_end;
+    const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(sRing + w * 2 * kTileFloatsMax);   // this warp's two coefficient slots
     // T and p of a group are loaded one group ahead (their latency would otherwise open every group)
     auto ld2_at = [&](const float* p, long long grp) -> f2 {
         const long long ir = grp * kGroupCells + 2 * lane;
-        if (ir + 1 < n) return __ldg(reinterpret_cast<const float2*>(p + ir));
+        if (FULL || ir + 1 < n) return __ldg(reinterpret_cast<const float2*>(p + ir));
         const float v = __ldg(p + (ir < n ? ir : 0));
         return make_float2(v, v);
     };
     f2 T_next = bc(1000.f), p_next = bc(1.f);
-    if ((long long)blockIdx.x < ngroups) {
-        T_next = ld2_at(Tg, blockIdx.x);
-        if (D_o) p_next = ld2_at(pg, blockIdx.x);
+    if (g_first + blockIdx.x < ngroups) {
+        T_next = ld2_at(Tg, g_first + blockIdx.x);
+        if (want_D) p_next = ld2_at(pg, g_first + blockIdx.x);
     }
-    for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+    for (long long grp = g_first + blockIdx.x; grp < ngroups; grp += gridDim.x) {
         // every thread stays alive through the barriers; lanes past the end of the field work on cell 0 and do not store
         const long long i_raw = grp * kGroupCells + 2 * lane;
-        const bool valid = i_raw < n;
+        const bool valid = FULL || i_raw < n;
         const long long i = valid ? i_raw : 0;
-        const bool two = valid && (i + 1 < n);
-        const bool full = (grp + 1) * kGroupCells <= n;   // block-uniform: all but the last group take the plain float2 path
+        const bool two = FULL || (valid && (i + 1 < n));
         auto ld2 = [&](const float* p) -> f2 {
-            if (full || two) return __ldg(reinterpret_cast<const float2*>(p + i));
+            if (two) return __ldg(reinterpret_cast<const float2*>(p + i));
             const float v = __ldg(p + i);
             return make_float2(v, v);
         };
         auto st2 = [&](float* p, f2 v) {
-            if (full || two) *reinterpret_cast<float2*>(p + i) = v;
+            if (two) *reinterpret_cast<float2*>(p + i) = v;
             else if (valid) p[i] = v.x;
         };
         const f2 T = T_next, p_cell = p_next;
         // all of this warp's Y rows in flight at once, then the next group's T and p
         f2 yv[KW];
 #pragma unroll
-        for (int a = 0; a < KW; ++a) yv[a] = (w + 4 * a < K) ? ld2(Yg + (size_t)(w + 4 * a) * ld) : bc(0.f);
+        for (int a = 0; a < KW; ++a) yv[a] = (a < KW - 2 || w + 4 * a < K) ? ld2(Yg + (size_t)(w + 4 * a) * ld) : bc(0.f);   // K > Kp - 8
         if (grp + gridDim.x < ngroups) {
             T_next = ld2_at(Tg, grp + gridDim.x);
-            if (D_o) p_next = ld2_at(pg, grp + gridDim.x);
+            if (want_D) p_next = ld2_at(pg, grp + gridDim.x);
         }
         const f2 tau = mul2(add2(T, bc(-md.sc.T_mid)), md.sc.inv_S);
         const bool lo0 = T.x < md.sc.T_mid, lo1 = T.y < md.sc.T_mid;   // A2: hi for T >= T_mid
@@ -217,13 +224,13 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
                     s1 = fma2(x, lk, s1);
                     s2 = fma2(x, rcp2(lk), s2);
                 }
-                if ((want_thermo && h_o) || D_o) {
+                if (want_h || want_D) {
                     const double ya = (double)y.x, yb = (double)y.y;
-                    if (D_o) {   // sum_j Y_j in fp64 (exact on the fp32 inputs to 1e-16): N_k = sum - Y_k without the fp32 rounding of the sum
+                    if (want_D) {   // sum_j Y_j in fp64 (exact on the fp32 inputs to 1e-16): N_k = sum - Y_k without the fp32 rounding of the sum
                         Yta += ya;
                         Ytb += yb;
                     }
-                    if (want_thermo && h_o) {   // formation-enthalpy term in fp64 (|h| ~ 1e7 J/kg against a 1e-5 tolerance)
+                    if (want_h) {   // formation-enthalpy term in fp64 (|h| ~ 1e7 J/kg against a 1e-5 tolerance)
                         const double hl = sH0[2 * k], hh = sH0[2 * k + 1];
                         H0la = fma(ya, hl, H0la); H0ha = fma(ya, hh, H0ha);
                         H0lb = fma(yb, hl, H0lb); H0hb = fma(yb, hh, H0hb);
@@ -242,7 +249,7 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
             my[0] = sumx;
             my[8 * 32] = s1;
             my[9 * 32] = s2;
-            if (D_o) {   // the warp's share of sum Y as a float-float pair
+            if (want_D) {   // the warp's share of sum Y as a float-float pair
                 const f2 hi = make_float2((float)Yta, (float)Ytb);
                 my[11 * 32] = hi;
                 my[12 * 32] = make_float2((float)(Yta - (double)hi.x), (float)(Ytb - (double)hi.y));
@@ -266,11 +273,11 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
 #pragma unroll
                 for (int v = 0; v < 4; ++v) q[m] = add2(q[m], sScr[(v * kScrSlots + 1 + m) * 32 + lane]);
             }
-            if (cp_o)
+            if (want_cp)
                 st2(cp_o, mul2(fma2(fma2(fma2(fma2(mul2(q[4], 5.f), tau, mul2(q[3], 4.f)), tau, mul2(q[2], 3.f)), tau,
                                          mul2(q[1], 2.f)), tau, q[0]),
                                md.sc.inv_S));
-            if (h_o) {
+            if (want_h) {
                 double Ha = 0.0, Hb = 0.0;
 #pragma unroll
                 for (int v = 0; v < 4; ++v) {
@@ -289,7 +296,7 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
         // Mole fractions are never normalised: with x_k = Y_k/W_k = X_k sum(x), Wilke's ratio is unchanged (numerator and
         // denominator both carry sum(x)), and the conductivity sums and S_k are corrected by sum(x) where they are used.
         // That makes phase 2 (r_k, conductivity) independent of any sum over species: it runs inside phase 1's loop.
-        if (lam_o && w == 0) {
+        if (want_lam && w == 0) {
             f2 s1 = bc(0.f), s2 = bc(0.f);
 #pragma unroll
             for (int v = 0; v < 4; ++v) {
@@ -301,7 +308,7 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
         }
 
         // ---- phase 3: Wilke; this warp owns rows k0 .. k0 + KW - 1 ------------------------------------------------
-        if (mu_o) {
+        if (want_mu) {
             const int k0 = w * KW;
             f2 gk[KW], den[KW];
 #pragma unroll
@@ -332,13 +339,13 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
             sScr[(w * kScrSlots + 10) * 32 + lane] = acc;
         }
         __syncthreads();   // every warp is done reading r: sR becomes the S accumulators
-        if (mu_o && w == 0) {
+        if (want_mu && w == 0) {
             f2 acc = bc(0.f);
 #pragma unroll
             for (int v = 0; v < 4; ++v) acc = add2(acc, sScr[(v * kScrSlots + 10) * 32 + lane]);
             st2(mu_o, mul2(sqrtT, acc));
         }
-        if (!D_o) continue;   // block-uniform; the barrier above also protects the scratch
+        if (!want_D) continue;   // block-uniform; the barrier above also protects the scratch
 
         // ---- phase 4: mixture-averaged diffusivities ---------------------------------------------------------------
         for (int k = w; k < Kp; k += 4) sR[k * 32 + lane] = bc(0.f);
@@ -348,40 +355,51 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
             if (in < n) {
 #pragma unroll
                 for (int a = 0; a < KW; ++a)
-                    if (w + 4 * a < K) asm volatile("prefetch.global.L2 [%0];" ::"l"(Yg + (size_t)(w + 4 * a) * ld + in));
+                    if (a < KW - 2 || w + 4 * a < K) asm volatile("prefetch.global.L2 [%0];" ::"l"(Yg + (size_t)(w + 4 * a) * ld + in));
             }
         }
-        constexpr int kTileFloats = TS * tile_row_floats(TS);
-        float* ring = sRing + w * 2 * kTileFloatsMax;
-        auto stage = [&](int round, int buf) {
-            const float* src = md.dtile + (size_t)tile_index(kSchedK[round][w], kSchedJ[round][w]) * kTileFloats;
-            for (int c16 = lane; c16 < kTileFloats / 4; c16 += 32) cp_async16(ring + buf * kTileFloatsMax + 4 * c16, src + 4 * c16);
+        constexpr int kTileFloats = TS * tile_row_floats(TS), kTile16 = kTileFloats / 4;
+        const float* ring = sRing + w * 2 * kTileFloatsMax;
+        auto stage = [&](int sched, int buf) {   // the whole tile is one or two 16-byte pieces per lane
+            const float* src = md.dtile + (size_t)(sched >> 8) * kTileFloats + 4 * lane;
+            const uint32_t dst = ring_s + (buf * kTileFloatsMax + 4 * lane) * 4;
+#pragma unroll
+            for (int c = 0; c < (kTile16 + 31) / 32; ++c)
+                if ((c + 1) * 32 <= kTile16 || lane + c * 32 < kTile16)
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst + c * 512), "l"(src + c * 128) : "memory");
             cp_async_commit();
         };
-        stage(0, 0);
+        int sched = kSched[0][w];
+        stage(sched, 0);
         __syncthreads();   // S is zeroed everywhere
         for (int r = 0; r < kRounds; ++r) {
-            if (r + 1 < kRounds) stage(r + 1, (r + 1) & 1);
+            const int sched_next = kSched[r + 1 < kRounds ? r + 1 : r][w];
+            if (r + 1 < kRounds) stage(sched_next, (r + 1) & 1);
             else cp_async_commit();
             cp_async_wait<1>();
             __syncwarp();
-            const int kt = kSchedK[r][w], jt = kSchedJ[r][w];
+            const int kt = sched & 15, jt = (sched >> 4) & 15;
+            sched = sched_next;
             const float* coef = ring + (r & 1) * kTileFloatsMax;
             f2 Xk[TS], Xj[TS], Sk[TS], Sj[TS];
+            const f2* xk = sX + kt * TS * 32 + lane;
+            const f2* xj = sX + jt * TS * 32 + lane;
 #pragma unroll
             for (int a = 0; a < TS; ++a) {
-                Xk[a] = sX[(kt * TS + a) * 32 + lane];
-                Xj[a] = sX[(jt * TS + a) * 32 + lane];
+                Xk[a] = xk[a * 32];
+                Xj[a] = xj[a * 32];
                 Sk[a] = Sj[a] = bc(0.f);
             }
             if (r >= 7) diff_tile<TS, true>(coef, u, Xk, Xj, Sk, Sj);    // block-uniform: the two diagonal rounds
             else diff_tile<TS, false>(coef, u, Xk, Xj, Sk, Sj);
             // tiles kt and jt of S belong to this warp alone in this round
+            f2* sk = sR + kt * TS * 32 + lane;
 #pragma unroll
-            for (int a = 0; a < TS; ++a) sR[(kt * TS + a) * 32 + lane] = add2(sR[(kt * TS + a) * 32 + lane], Sk[a]);
+            for (int a = 0; a < TS; ++a) sk[a * 32] = add2(sk[a * 32], Sk[a]);
             if (r < 7) {
+                f2* sj = sR + jt * TS * 32 + lane;
 #pragma unroll
-                for (int a = 0; a < TS; ++a) sR[(jt * TS + a) * 32 + lane] = add2(sR[(jt * TS + a) * 32 + lane], Sj[a]);
+                for (int a = 0; a < TS; ++a) sj[a * 32] = add2(sj[a * 32], Sj[a]);
             }
             __syncthreads();
         }
@@ -390,7 +408,7 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
         // ---- final: D_k = N_k / S_k for this warp's species k = w, w + 4, ... (its Y rows again: L2 hits) ------------
         {
 #pragma unroll
-            for (int a = 0; a < KW; ++a) yv[a] = (w + 4 * a < K) ? ld2(Yg + (size_t)(w + 4 * a) * ld) : bc(0.f);
+            for (int a = 0; a < KW; ++a) yv[a] = (a < KW - 2 || w + 4 * a < K) ? ld2(Yg + (size_t)(w + 4 * a) * ld) : bc(0.f);
             f2 thi = bc(0.f), tlo = bc(0.f);
 #pragma unroll
             for (int v = 0; v < 4; ++v) {
@@ -401,7 +419,7 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
 #pragma unroll
             for (int a = 0; a < KW; ++a) {
                 const int k = w + 4 * a;
-                if (k < K) {
+                if (a < KW - 2 || k < K) {
                     // (hi - Y_k) loses nothing that matters: an fp32 difference is exact to 2^-24 of its RESULT; what
                     // cancellation would amplify is the rounding of the sum itself, and that sits in lo
                     const f2 Nk = add2(add2(thi, make_float2(-yv[a].x, -yv[a].y)), tlo);
@@ -418,19 +436,34 @@ props_group_kernel(const __grid_constant__ MechDev md, long long n, long long ld
     }
 }
 
+template <int KW, bool FULL, bool ALL>
+df_status launch_one(const MechDev& md, long long g_first, long long g_end, long long n, long long ld, const float* T, const float* p,
+                     const float* Y, float* cp, float* h, float* mu, float* lam, float* D, cudaStream_t s) {
+    const int smem = group_smem(4 * KW).total;
+    static DfPerDevice smem_attr;
+    const df_status st = df_ensure_dyn_smem((const void*)props_group_kernel<KW, FULL, ALL>, smem, &smem_attr);
+    if (st != DF_OK) return st;
+    const long long ngroups = g_end - g_first;
+    const long long cap = (long long)df_device_sm_count() * 3 * 4;   // 3 resident blocks per SM, ~4 waves
+    const long long blocks = ngroups < cap ? ngroups : cap;
+    props_group_kernel<KW, FULL, ALL><<<(unsigned)(blocks > 0 ? blocks : 1), kGT, smem, s>>>(md, g_first, g_end, n, ld, T, p, Y, cp, h, mu, lam, D);
+    DF_CUDA_TRY(cudaGetLastError());
+    return DF_OK;
+}
+
+// the full groups in one launch, the ragged last group (if any) in a launch of its own
 template <int KW>
 df_status launch_kw(const MechDev& md, long long n, long long ld, const float* T, const float* p, const float* Y, float* cp,
                     float* h, float* mu, float* lam, float* D, cudaStream_t s) {
-    const int smem = group_smem(4 * KW).total;
-    static DfPerDevice smem_attr;
-    const df_status st = df_ensure_dyn_smem((const void*)props_group_kernel<KW>, smem, &smem_attr);
-    if (st != DF_OK) return st;
-    const long long ngroups = (n + kGroupCells - 1) / kGroupCells;
-    const long long cap = (long long)df_device_sm_count() * 3 * 4;   // 3 resident blocks per SM, ~4 waves
-    const long long blocks = ngroups < cap ? ngroups : cap;
-    props_group_kernel<KW><<<(unsigned)(blocks > 0 ? blocks : 1), kGT, smem, s>>>(md, n, ld, T, p, Y, cp, h, mu, lam, D);
-    DF_CUDA_TRY(cudaGetLastError());
-    return DF_OK;
+    const long long full_groups = n / kGroupCells, ngroups = (n + kGroupCells - 1) / kGroupCells;
+    const bool all = cp && h && mu && lam && D;
+    df_status st = DF_OK;
+    if (full_groups > 0)
+        st = all ? launch_one<KW, true, true>(md, 0, full_groups, n, ld, T, p, Y, cp, h, mu, lam, D, s)
+                 : launch_one<KW, true, false>(md, 0, full_groups, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+    if (st == DF_OK && ngroups > full_groups)
+        st = launch_one<KW, false, false>(md, full_groups, ngroups, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+    return st;
 }
 
 }  // namespace
