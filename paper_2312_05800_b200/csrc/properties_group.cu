@@ -38,11 +38,9 @@ __device__ __forceinline__ f2 fma2(f2 a, float s, float c) { return __ffma2_rn(a
 __device__ __forceinline__ f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
 __device__ __forceinline__ f2 mul2(f2 a, float s) { return __fmul2_rn(a, bc(s)); }
 __device__ __forceinline__ f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
-// reciprocals of both halves from one MUFU: 1/x = y/(xy), 1/y = x/(xy)
-__device__ __forceinline__ f2 rcp2(f2 a) {
-    const float r = rcp_approx(a.x * a.y);
-    return make_float2(r * a.y, r * a.x);
-}
+// one MUFU.RCP per half (B200's XU pipe is far from full here: the shared form 1/x = y/(xy), one MUFU + three FMUL, on any
+// share of the pairs measured 0-1.5 % slower)
+__device__ __forceinline__ f2 rcp2(f2 a) { return make_float2(rcp_approx(a.x), rcp_approx(a.y)); }
 // hi + lo += y with the rounding error of the addition kept (Knuth's TwoSum, packed for two cells)
 __device__ __forceinline__ void two_sum_acc(f2& hi, f2& lo, f2 y) {
     const f2 s = add2(hi, y);
@@ -51,8 +49,6 @@ __device__ __forceinline__ void two_sum_acc(f2& hi, f2& lo, f2 y) {
     hi = s;
     lo = add2(lo, e);
 }
-// one MUFU per half: in the FMA-bound pair loop the XU pipe is idle and the three multiplies of rcp2 are not
-__device__ __forceinline__ f2 rcp2x(f2 a) { return make_float2(rcp_approx(a.x), rcp_approx(a.y)); }
 __device__ __forceinline__ f2 poly4_2(float c0, float c1, float c2, float c3, float c4, f2 u) {
     return fma2(fma2(fma2(fma2(u, c4, c3), u, bc(c2)), u, bc(c1)), u, bc(c0));
 }
@@ -90,10 +86,8 @@ __device__ __forceinline__ void diff_tile(const float* __restrict__ coef, f2 u, 
         }
 #pragma unroll
         for (int b = DIAG ? a + 1 : 0; b < TS; ++b) {
-            // both pipes at work: two MUFU (XU: 16 clk per pair and SMSP) for five pairs of eight, one MUFU + three
-            // FMUL (FMA pipe: +3 clk) for the rest -- ~13 clk per pair on either pipe
             const f2 P = poly4_2(q[5 * b], q[5 * b + 1], q[5 * b + 2], q[5 * b + 3], q[5 * b + 4], u);
-            const f2 r = ((a * TS + b) % 8 < 5) ? rcp2x(P) : rcp2(P);
+            const f2 r = rcp2(P);
             Sk[a] = fma2(Xj[b], r, Sk[a]);
             if (DIAG) Sk[b] = fma2(Xk[a], r, Sk[b]);
             else Sj[b] = fma2(Xk[a], r, Sj[b]);
@@ -426,7 +420,7 @@ props_group_kernel(const __grid_constant__ MechDev md, long long g_first, long l
                     const f2 S = sR[k * 32 + lane];
                     const float* dd = sSmall + k * kSmallStride + 12;
                     const f2 dk = poly4_2(dd[0], dd[1], dd[2], dd[3], dd[4], u);
-                    const f2 q = mul2(mul2(Nk, sumx), rcp2x(S));   // S was accumulated on x = X sum(x)
+                    const f2 q = mul2(mul2(Nk, sumx), rcp2(S));   // S was accumulated on x = X sum(x)
                     const f2 Dk = make_float2(S.x > 0.f ? q.x : dk.x, S.y > 0.f ? q.y : dk.y);   // A7
                     st2(D_o + (size_t)k * ld, mul2(Dk, scale));
                 }
