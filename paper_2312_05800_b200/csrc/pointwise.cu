@@ -39,6 +39,9 @@ __device__ __forceinline__ void store4(float* __restrict__ p, long long i0, long
     }
 }
 
+// species rows (float4 per thread) loaded ahead of their use in every pass: the passes are HBM-bound and a row-at-a-time
+// loop leaves too few bytes in flight (extras 0.165 -> 0.135 ms, pasr -7 %; 2 and 8 rows measured slower)
+constexpr int kRowsAhead = 4;
 // ---- NEXT-4 ------------------------------------------------------------------------------------------------------
 template <bool FULL>
 __global__ void __launch_bounds__(kPT)
@@ -73,17 +76,26 @@ extras_kernel(MechDev md, long long i_first, long long n, long long ld, const fl
         lo[c] = T.v[c] < md.sc.T_mid;   // A2
     }
     float invWbar[4] = {0.f, 0.f, 0.f, 0.f}, sy[4] = {0.f, 0.f, 0.f, 0.f}, sxlx[4] = {0.f, 0.f, 0.f, 0.f};
-    for (int k = 0; k < K; ++k) {
-        const F4 y = load4<FULL>(Yg + (size_t)k * ld, i0, n, 0.f);
+    for (int k0 = 0; k0 < K; k0 += kRowsAhead) {   // kRowsAhead rows of Y in flight at once
+        F4 yq[kRowsAhead];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            const float x = y.v[c] * sIW[k];
-            invWbar[c] += x;
-            if (s_o) {
-                const float* q = sS + k * 12 + (lo[c] ? 0 : 6);
-                const float sk = fmaf(q[0], lnT[c], fmaf(fmaf(fmaf(fmaf(q[5], tau[c], q[4]), tau[c], q[3]), tau[c], q[2]), tau[c], q[1]));
-                sy[c] = fmaf(y.v[c], sk, sy[c]);
-                sxlx[c] += x > 0.f ? x * __logf(x) : 0.f;   // x ln x -> 0; MUFU lg2: |err| < 1e-6 on a term that is ~1 % of s
+        for (int q = 0; q < kRowsAhead; ++q)
+            if (k0 + q < K) yq[q] = load4<FULL>(Yg + (size_t)(k0 + q) * ld, i0, n, 0.f);
+#pragma unroll
+        for (int q = 0; q < kRowsAhead; ++q) {
+            const int k = k0 + q;
+            if (k >= K) break;
+            const F4 y = yq[q];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const float x = y.v[c] * sIW[k];
+                invWbar[c] += x;
+                if (s_o) {
+                    const float* q6 = sS + k * 12 + (lo[c] ? 0 : 6);
+                    const float sk = fmaf(q6[0], lnT[c], fmaf(fmaf(fmaf(fmaf(q6[5], tau[c], q6[4]), tau[c], q6[3]), tau[c], q6[2]), tau[c], q6[1]));
+                    sy[c] = fmaf(y.v[c], sk, sy[c]);
+                    sxlx[c] += x > 0.f ? x * __logf(x) : 0.f;   // x ln x -> 0; MUFU lg2: |err| < 1e-6 on a term that is ~1 % of s
+                }
             }
         }
     }
@@ -111,22 +123,33 @@ extras_kernel(MechDev md, long long i_first, long long n, long long ld, const fl
         store4<FULL>(s_o, i0, n, o);
     }
     if (!rhoD_o && !hk_o) return;
-    for (int k = 0; k < K; ++k) {
+    // kRowsAhead rows of D in flight at once
+    for (int k0 = 0; k0 < K; k0 += kRowsAhead) {
+        F4 d[kRowsAhead];
         if (rhoD_o) {
-            const F4 d = load4<FULL>(Dg + (size_t)k * ld, i0, n, 0.f);
-            F4 o;
 #pragma unroll
-            for (int c = 0; c < 4; ++c) o.v[c] = rho.v[c] * d.v[c];
-            store4<FULL>(rhoD_o + (size_t)k * ld, i0, n, o);
+            for (int q = 0; q < kRowsAhead; ++q)
+                if (k0 + q < K) d[q] = load4<FULL>(Dg + (size_t)(k0 + q) * ld, i0, n, 0.f);
         }
-        if (hk_o) {
-            F4 o;
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                const float* q = sTh + k * 12 + (lo[c] ? 0 : 6);
-                o.v[c] = fmaf(fmaf(fmaf(fmaf(fmaf(q[5], tau[c], q[4]), tau[c], q[3]), tau[c], q[2]), tau[c], q[1]), tau[c], q[0]);
+        for (int q = 0; q < kRowsAhead; ++q) {
+            const int k = k0 + q;
+            if (k >= K) break;
+            if (rhoD_o) {
+                F4 o;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) o.v[c] = rho.v[c] * d[q].v[c];
+                store4<FULL>(rhoD_o + (size_t)k * ld, i0, n, o);
             }
-            store4<FULL>(hk_o + (size_t)k * ld, i0, n, o);
+            if (hk_o) {
+                F4 o;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const float* q6 = sTh + k * 12 + (lo[c] ? 0 : 6);
+                    o.v[c] = fmaf(fmaf(fmaf(fmaf(fmaf(q6[5], tau[c], q6[4]), tau[c], q6[3]), tau[c], q6[2]), tau[c], q6[1]), tau[c], q6[0]);
+                }
+                store4<FULL>(hk_o + (size_t)k * ld, i0, n, o);
+            }
         }
     }
 }
@@ -148,13 +171,23 @@ pasr_kernel(MechDev md, long long i_first, long long n, long long ld, const floa
     if (!FULL && i0 >= n) return;
     const F4 T = load4<FULL>(Tg, i0, n, 1000.f), p = load4<FULL>(pg, i0, n, 101325.f);
     float invWbar[4] = {0.f, 0.f, 0.f, 0.f}, m[4] = {0.f, 0.f, 0.f, 0.f};
-    for (int k = 0; k < K; ++k) {
-        const F4 y = load4<FULL>(Yg + (size_t)k * ld, i0, n, 0.f), w = load4<FULL>(omega + (size_t)k * ld, i0, n, 0.f);
+    for (int k0 = 0; k0 < K; k0 += kRowsAhead) {   // kRowsAhead rows of Y and omega in flight at once
+        F4 yq[kRowsAhead], wq[kRowsAhead];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            invWbar[c] = fmaf(y.v[c], sm[k], invWbar[c]);
-            const float a = fabsf(w.v[c]);
-            if (a > 0.f) m[c] = fmaxf(m[c], y.v[c] * rcp_approx(a));   // species that do not react do not count
+        for (int q = 0; q < kRowsAhead; ++q)
+            if (k0 + q < K) {
+                yq[q] = load4<FULL>(Yg + (size_t)(k0 + q) * ld, i0, n, 0.f);
+                wq[q] = load4<FULL>(omega + (size_t)(k0 + q) * ld, i0, n, 0.f);
+            }
+#pragma unroll
+        for (int q = 0; q < kRowsAhead; ++q) {
+            if (k0 + q >= K) break;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                invWbar[c] = fmaf(yq[q].v[c], sm[k0 + q], invWbar[c]);
+                const float a = fabsf(wq[q].v[c]);
+                if (a > 0.f) m[c] = fmaxf(m[c], yq[q].v[c] * rcp_approx(a));   // species that do not react do not count
+            }
         }
     }
     const F4 mu = load4<FULL>(mug, i0, n, 1.f), ks = load4<FULL>(kg, i0, n, 1.f), ep = load4<FULL>(eg, i0, n, 1.f);
@@ -170,11 +203,18 @@ pasr_kernel(MechDev md, long long i_first, long long n, long long ld, const floa
         kappa.v[c] = kp;
     }
     if (kappa_o) store4<FULL>(kappa_o, i0, n, kappa);
-    for (int k = 0; k < K; ++k) {
-        F4 w = load4<FULL>(omega + (size_t)k * ld, i0, n, 0.f);
+    for (int k0 = 0; k0 < K; k0 += kRowsAhead) {
+        F4 wq[kRowsAhead];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) w.v[c] *= kappa.v[c];
-        store4<FULL>(omega + (size_t)k * ld, i0, n, w);
+        for (int q = 0; q < kRowsAhead; ++q)
+            if (k0 + q < K) wq[q] = load4<FULL>(omega + (size_t)(k0 + q) * ld, i0, n, 0.f);
+#pragma unroll
+        for (int q = 0; q < kRowsAhead; ++q) {
+            if (k0 + q >= K) break;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) wq[q].v[c] *= kappa.v[c];
+            store4<FULL>(omega + (size_t)(k0 + q) * ld, i0, n, wq[q]);
+        }
     }
 }
 
