@@ -197,6 +197,35 @@ def test_properties_subset_outputs(B):
     assert helpers.rel_err(mu.cpu().numpy(), ref["mu"]).max() <= 1e-5
 
 
+@pytest.mark.parametrize("K,n,ld", [(24, 200, 200), (53, 131, 132)])
+def test_properties_subset_outputs_generic_K(B, K, n, ld):
+    """The any-K kernel's instantiations for calls that want only some outputs, on full groups and a ragged last one."""
+    from oracle import oracle
+    from paper_2312_05800_b200 import synth
+    mech = synth.make_mechanism(K, 500 + K)
+    cells = synth.cells_stratified(K, n, 600 + K, ld=ld)
+    om = oracle.Mech(mech)
+    gm = B.Mech(mech)
+    T, p, Y = dev(cells.T), dev(cells.p), dev(cells.Y)
+    ref = om.properties(cells.T, cells.p, cells.Y[:, :n])
+    for names in (("cp",), ("mu",), ("D",), ("h", "lam"), ("cp", "h", "mu", "lam")):
+        out = {k: (torch.full((K, ld), -1.0, device="cuda") if k == "D" else torch.full((ld,), -1.0, device="cuda")) for k in names}
+        B.df_thermo_properties(gm, T, p, Y, n_cells=n, **out)
+        torch.cuda.synchronize()
+        for k, v in out.items():
+            g = v.cpu().numpy()
+            if k == "D":
+                assert helpers.rel_err(g[:, :n], ref["D"]).max() <= 1e-5, (names, k)
+                assert (g[:, n:] == -1.0).all()
+            elif k == "h":
+                scale = np.maximum(np.abs(ref["h"]), ref["cp"] * cells.T[:n])
+                assert (np.abs(g[:n] - ref["h"]) / scale).max() <= 1e-5, (names, k)
+            else:
+                assert helpers.rel_err(g[:n], ref[k]).max() <= 1e-5, (names, k)
+            if k != "D":
+                assert (g[n:] == -1.0).all()
+
+
 # --------------------------------------------------------------------------------------------
 # H3: ANN source, fp32 path
 # --------------------------------------------------------------------------------------------
