@@ -89,7 +89,8 @@ DF_API int df_mech_num_species(const df_mech* mech);
  *              "bf16 weights": low 16 bits of the fp32 pattern zero, else DF_ERR_INVALID_ARG) and, like the biases,
  *              finite with magnitude <= 65504 (else DF_ERR_UNSUPPORTED): tcgen05 kind::f16 needs both operands in one
  *              format, so the weights are held in fp16 (exact for bf16 values >= 2^-14, within 2^-25 below) and the
- *              activations are rounded to fp16, saturating at +-65504 (A21).
+ *              activations are rounded to fp16 (A21).  A hidden activation is held as 2 GELU(v) with the factor 1/2 in the
+ *              next layer's stored weights (a power of two: same results), so it saturates at |GELU(v)| = 32752.
  *              n_layers == 4, dims[1] % 64 == 0, dims[2] % 32 == 0 with 64 <= dims[2] <= 800,
  *              dims[3] % 16 == 0 with 32 <= dims[3] <= 400, K <= 28.
  * x_mean/x_std [K+2] and u_mean/u_std [K] are the Z-score statistics; the network output

@@ -200,8 +200,9 @@ __device__ __forceinline__ uint32_t gelu_pair(float a, float b) {
     const float2 v = make_float2(a, b);
     const float2 t = __ffma2_rn(__fmul2_rn(v, v), make_float2(0.0356774081f, 0.0356774081f), make_float2(0.7978845608f, 0.7978845608f));
     const float2 u = __fmul2_rn(t, v);
-    const float2 hv = __fmul2_rn(v, make_float2(0.5f, 0.5f));
-    const float2 r = __ffma2_rn(hv, make_float2(tanh_approx(u.x), tanh_approx(u.y)), hv);
+    // the activation is held as 2 GELU(v) = v + v tanh(u): the factor 1/2 sits in the next layer's weights (exact: a power of
+    // two), which saves one of eight instructions per pair
+    const float2 r = __ffma2_rn(v, make_float2(tanh_approx(u.x), tanh_approx(u.y)), v);
     return pack_act(r.x, r.y);
 }
 // dY*_k of ann_common.cuh with MUFU-grade transcendentals (ex2/lg2/rcp.approx): 5 MUFU + a few FMA per species
@@ -774,8 +775,8 @@ df_status ann_bf16_create(df_ann* ann, const float* const* W, const float* const
     if (d3 % 16 || d3 < 32 || d3 > 400) return df_set_error(DF_ERR_UNSUPPORTED, "bf16 path: dims[3] %% 16 == 0, 32..400 (got %d)", d3);
 
     // The contract of precision 1 (include/df_thermo.h): weights are bf16-valued and, like the biases, inside the
-    // fp16 range, because the tensor path holds them in fp16 (A21) -- exact for bf16 values in [2^-14, 65504], within
-    // 2^-25 absolute below that.  Anything else would be re-rounded silently (or become inf): refuse it.
+    // fp16 range, because the tensor path holds them in fp16 (A21; layers 2-4 halved, see gelu_pair) -- exact for bf16
+    // values in [2^-14, 65504], within 2^-25 absolute below that.  Anything else would be re-rounded silently (or become inf): refuse it.
     for (int l = 0; l < 4; ++l) {
         const size_t nw = (size_t)ann->dims[l] * ann->dims[l + 1];
         for (size_t i = 0; i < nw; ++i) {
@@ -854,26 +855,28 @@ df_status ann_bf16_create(df_ann* ann, const float* const* W, const float* const
         for (int r = 0; r < g.n3a; ++r) put_bias(t, r, 0, b[2][r]);
         for (int r = 0; r < g.n3b; ++r) put_bias(t, r, 32, b[2][g.n3a + r]);
     }
+    // layers 2-4 read activations held as 2 GELU (gelu_pair): their weights are stored halved (the bias tiles are not: they
+    // multiply the ones columns of A0)
     for (int h = 0; h < 2; ++h)
         for (int c = 0; c < g.NC; ++c) {
             uint8_t* t = blob.data() + o_w2 + (size_t)(h * (g.NC + 1) + 1 + c) * g.w2_tile_bytes;
             const int k0 = c * 32;
             for (int kk = 0; kk < 32; ++kk) {
-                for (int r = 0; r < g.na2; ++r) put(t, r, kk, W[1][(size_t)(h * g.NH + r) * d1 + k0 + kk]);
-                for (int r = 0; r < g.nb2; ++r) put(t, r, 32 + kk, W[1][(size_t)(h * g.NH + g.na2 + r) * d1 + k0 + kk]);
+                for (int r = 0; r < g.na2; ++r) put(t, r, kk, 0.5f * W[1][(size_t)(h * g.NH + r) * d1 + k0 + kk]);
+                for (int r = 0; r < g.nb2; ++r) put(t, r, 32 + kk, 0.5f * W[1][(size_t)(h * g.NH + g.na2 + r) * d1 + k0 + kk]);
             }
         }
     for (int ks = 0; ks < g.NKS; ++ks) {
         uint8_t* t = blob.data() + o_w3 + (size_t)(ks + 1) * g.w3_tile_bytes;
         for (int kk = 0; kk < 32; ++kk) {
-            for (int r = 0; r < g.n3a; ++r) put(t, r, kk, W[2][(size_t)r * d2 + ks * 32 + kk]);
-            for (int r = 0; r < g.n3b; ++r) put(t, r, 32 + kk, W[2][(size_t)(g.n3a + r) * d2 + ks * 32 + kk]);
+            for (int r = 0; r < g.n3a; ++r) put(t, r, kk, 0.5f * W[2][(size_t)r * d2 + ks * 32 + kk]);
+            for (int r = 0; r < g.n3b; ++r) put(t, r, 32 + kk, 0.5f * W[2][(size_t)(g.n3a + r) * d2 + ks * 32 + kk]);
         }
     }
     for (int jj = 0; jj < g.NJ; ++jj) {
         uint8_t* t = blob.data() + o_w4 + (size_t)jj * 4096;
         for (int r = 0; r < K; ++r)
-            for (int c = 0; c < 64 && jj * 64 + c < d3; ++c) put(t, r, c, W[3][(size_t)r * d3 + jj * 64 + c]);
+            for (int c = 0; c < 64 && jj * 64 + c < d3; ++c) put(t, r, c, 0.5f * W[3][(size_t)r * d3 + jj * 64 + c]);
     }
     float* hb = reinterpret_cast<float*>(blob.data() + o_b);
     memcpy(hb, b[0], sizeof(float) * d1);
