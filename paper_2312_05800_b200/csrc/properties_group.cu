@@ -72,20 +72,21 @@ __constant__ int kSched[9][4] = {
 constexpr int kRounds = 9;
 
 // One TS x TS tile of species pairs.  coef: [a][b][5] in shared memory (warp-uniform addresses: broadcast loads).
-template <int TS, bool DIAG>
+// NB: columns b < NB of the j tile are evaluated -- TS, or the first half when the rest of the last tile is padding.
+template <int TS, bool DIAG, int NB>
 __device__ __forceinline__ void diff_tile(const float* __restrict__ coef, f2 u, const f2 (&Xk)[TS], const f2 (&Xj)[TS],
                                           f2 (&Sk)[TS], f2 (&Sj)[TS]) {
-    constexpr int RS = tile_row_floats(TS);
+    constexpr int RS = tile_row_floats(TS), NQ = (5 * NB + 3) / 4;
 #pragma unroll
     for (int a = 0; a < (DIAG ? TS - 1 : TS); ++a) {
-        float q[RS];
+        float q[4 * NQ];
 #pragma unroll
-        for (int i = 0; i < RS / 4; ++i) {
+        for (int i = 0; i < NQ; ++i) {
             const float4 v = reinterpret_cast<const float4*>(coef + a * RS)[i];
             q[4 * i] = v.x; q[4 * i + 1] = v.y; q[4 * i + 2] = v.z; q[4 * i + 3] = v.w;
         }
 #pragma unroll
-        for (int b = DIAG ? a + 1 : 0; b < TS; ++b) {
+        for (int b = DIAG ? a + 1 : 0; b < NB; ++b) {
             const f2 P = poly4_2(q[5 * b], q[5 * b + 1], q[5 * b + 2], q[5 * b + 3], q[5 * b + 4], u);
             const f2 r = rcp2(P);
             Sk[a] = fma2(Xj[b], r, Sk[a]);
@@ -384,8 +385,13 @@ props_group_kernel(const __grid_constant__ MechDev md, long long g_first, long l
                 Xj[a] = xj[a * 32];
                 Sk[a] = Sj[a] = bc(0.f);
             }
-            if (r >= 7) diff_tile<TS, true>(coef, u, Xk, Xj, Sk, Sj);    // block-uniform: the two diagonal rounds
-            else diff_tile<TS, false>(coef, u, Xk, Xj, Sk, Sj);
+            // block-uniform: the two diagonal rounds.  Warp-uniform: the tile whose j side is the last species tile, when at
+            // least half of that tile is padding (K = 53: species 53..55 of 49..55), evaluates the first half only -- that warp
+            // waits at the round's barrier either way, but the SM's other blocks get its issue slots
+            constexpr int NBH = (TS + 1) / 2;
+            if (r >= 7) diff_tile<TS, true, TS>(coef, u, Xk, Xj, Sk, Sj);
+            else if (jt == 7 && K - 7 * TS <= NBH) diff_tile<TS, false, NBH>(coef, u, Xk, Xj, Sk, Sj);
+            else diff_tile<TS, false, TS>(coef, u, Xk, Xj, Sk, Sj);
             // tiles kt and jt of S belong to this warp alone in this round
             f2* sk = sR + kt * TS * 32 + lane;
 #pragma unroll
