@@ -294,6 +294,24 @@ def measure_fp32_peak(torch, B, stream):
         out[name] = flops[0] / (mn * 1e-3) / 1e12
         out[name + "_median"] = flops[0] / (med * 1e-3) / 1e12
     out["measured"] = max(out["ffma"], out["ffma2"])
+    # issue rates behind the property kernels' pair loops: time per warp-iteration and SMSP of eight
+    # MUFU.RCP, and of the pair loop's mix (2 MUFU.RCP + 6 FFMA2), in units of one FFMA2 of the same run and in clocks under
+    # the architectural figure MUFU.RCP = 8 clocks per warp and SMSP (4 lanes per clock)
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    iblocks, iiters = sms * 4, 20000          # 16 warps per SM: 4 per SMSP
+    per = {}
+    for name, variant in (("mufu8", 2), ("pair_mix", 3)):
+        wi = [0.0]
+
+        def launch_i(_i):
+            wi[0] = B.df_probe_fp32_peak(variant, iblocks, iiters)
+        _med, mn = _median_launch_ms(torch, stream, launch_i, reps=5, warm=1)
+        per[name] = mn * 1e-3 / (wi[0] / (sms * 4))          # seconds per warp-iteration on one SMSP
+    t_ffma2 = 128.0 / (out["ffma2"] * 1e12 / (sms * 4))       # seconds per warp-wide FFMA2 (64 FMA = 128 flop) on one SMSP
+    t_mufu = per["mufu8"] / 8.0
+    out["issue"] = {"mufu_rcp_per_ffma2": t_mufu / t_ffma2, "pair_mix_per_ffma2": per["pair_mix"] / t_ffma2,
+                    "clk_if_mufu_is_8": {"ffma2": 8.0 * t_ffma2 / t_mufu, "pair_mix_2mufu_6ffma2": 8.0 * per["pair_mix"] / t_mufu},
+                    "how": "df_probe_fp32_peak variants 2, 3: 4 warps per SMSP, 20000 iterations, best of 5"}
     out["nominal"] = FP32_NOMINAL_TFLOPS
     out["unit"] = "TFLOP/s"
     out["how"] = ("df_probe_fp32_peak: 148 x 16 blocks x 256 threads, 16 register-only dependent FMA chains per thread "

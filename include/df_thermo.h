@@ -233,7 +233,10 @@ DF_API df_status df_step_host(df_host_ctx* ctx, long long n_cells, long long ld,
  * Launches a register-only dependent-FMA kernel on `stream` (blocks x 256 threads, 16 FMAs per thread per iteration):
  * variant 0 = scalar FFMA, 1 = packed FFMA2 (the form the property kernels use).  *flops (host, optional) receives
  * the floating-point operations of the launch (FMA = 2); out (device, optional) receives blocks*256 floats.
- * bench.py times it with CUDA events: the FP32 "alu" roofline peak measured in the same run. */
+ * bench.py times it with CUDA events: the FP32 "alu" roofline peak measured in the same run.
+ * variants 2 and 3 are issue-rate probes for the property kernels' pair loops (blocks x 128 threads, out = blocks*128
+ * floats): 2 = eight MUFU.RCP (+ eight FADD) per thread and iteration, 3 = the pair loop's mix of 2 MUFU.RCP + 6 FFMA2;
+ * for them *flops receives the number of warp-iterations of the launch (iters x blocks x 4). */
 DF_API df_status df_probe_fp32_peak(int variant, int blocks, long long iters, float* out, double* flops, void* stream);
 
 #ifdef __cplusplus
