@@ -124,3 +124,48 @@ def test_cfg5_T_from_h_robustness(B, guess):
     assert np.abs(T.cpu().numpy()[idx] - T_ref).max() <= 1e-3
     cp_ref, _ = om.mixture_cp_h(T.cpu().numpy()[idx], Ys)
     assert helpers.rel_err(cp.cpu().numpy()[idx], cp_ref).max() <= 1e-5
+
+
+def test_full_size_extras_and_pasr(B):
+    """NEXT-4 / NEXT-3 at the size bench.py times them (2,097,152 cells, K = 19): kernels on the whole field, the oracle on
+    sampled cells; kappa in [0, 1) and the gate on every cell."""
+    from oracle import oracle
+    from paper_2312_05800_b200 import synth
+    mech, _, cells = synth.make_config(3)
+    n, K = cells.n, mech.K
+    om, gm = oracle.Mech(mech), B.Mech(mech)
+    T, p, Y = dev(cells.T), dev(cells.p), dev(cells.Y)
+    cp, lam = torch.empty(n, device="cuda"), torch.empty(n, device="cuda")
+    D = torch.empty(K, n, device="cuda")
+    B.df_thermo_properties(gm, T, p, Y, cp=cp, lam=lam, D=D)
+    rho, psi, alpha, s = (torch.empty(n, device="cuda") for _ in range(4))
+    rhoD, hk = torch.empty(K, n, device="cuda"), torch.empty(K, n, device="cuda")
+    B.df_thermo_extras(gm, T, p, Y, cp=cp, lam=lam, D=D, rho=rho, psi=psi, alpha=alpha, rhoD=rhoD, hk=hk, s=s)
+    idx = sample_idx(n)
+    it = torch.from_numpy(idx).cuda()
+    pick = lambda t: t[..., it].cpu().numpy()
+    ref = om.extras(cells.T[idx], cells.p[idx], np.ascontiguousarray(cells.Y[:, idx]), cp=pick(cp), lam=pick(lam), D=pick(D))
+    for name, got in (("rho", rho), ("psi", psi), ("alpha", alpha), ("s", s)):
+        e = helpers.rel_err(pick(got), ref[name])
+        assert e.max() <= 1e-5, f"{name}: {e.max():.3e}"
+    assert helpers.rel_err(pick(rhoD), ref["rhoD"][:, :len(idx)]).max() <= 1e-5
+    scale = np.maximum(np.abs(ref["hk"][:, :len(idx)]), 3.5 * helpers.R * cells.T[idx][None, :].astype(np.float64) / mech.W[:, None])
+    assert (np.abs(pick(hk) - ref["hk"][:, :len(idx)]) / scale).max() <= 1e-5
+    assert bool((rho > 0).all()) and bool(torch.isfinite(s).all())
+
+    g = torch.Generator(device="cuda").manual_seed(11)
+    mu = torch.rand(n, device="cuda", generator=g) * 7e-5 + 1e-5
+    ks = torch.rand(n, device="cuda", generator=g) * 10 + 0.01
+    eps = torch.rand(n, device="cuda", generator=g) * 1e4 + 0.1
+    omega = torch.randn(K, n, device="cuda", generator=g) * 50
+    omega[:, :7] = 0.0
+    om_in = pick(omega)
+    kappa = torch.full((n,), -7.0, device="cuda")
+    B.df_chem_pasr_scale(gm, T, p, Y, mu, ks, eps, 500.0, omega, kappa=kappa)
+    torch.cuda.synchronize()
+    oref, kref = om.pasr(cells.T[idx], cells.p[idx], np.ascontiguousarray(cells.Y[:, idx]), pick(mu), pick(ks), pick(eps), 500.0, om_in)
+    assert np.abs(pick(kappa) - kref).max() <= 1e-5
+    mixed, norm = helpers.mixed_err(pick(omega), oref[:, :len(idx)])
+    assert mixed <= 1e-5 and norm <= 1e-5, (mixed, norm)
+    assert bool(((kappa >= 0) & (kappa < 1)).all())
+    assert bool((kappa[T < 500.0] == 0).all()) and bool((kappa[:7] == 0).all())
