@@ -69,3 +69,40 @@ def test_mmlp_errors(B):
     nets[3].W[1][0, 0] = np.float32(0.1)     # not bf16-valued: refused like the single network
     with pytest.raises(B.DfError):
         B.AnnMmlp(nets)
+
+
+def test_mmlp_source_bench_size(B):
+    """NEXT-1 at the size bench.py times it (262,144 cells, 19 networks 21-1600-800-400-1): kernels on the whole field, oracle and
+    fp16-chain floor on sampled cells (plus the end of the field), sum-to-one on every cell."""
+    from oracle import oracle
+    from paper_2312_05800_b200 import synth
+    K, hidden, n = 19, [1600, 800, 400], 262144
+    seed = synth.config_seed(2)
+    mech = synth.make_mechanism(K, seed)
+    nets = synth.make_mmlp(K, hidden, 1, seed)
+    cells = synth.cells_stratified(K, n, seed)
+    gm, gn = B.Mech(mech), B.AnnMmlp(nets)
+    T, p, Y = dev(cells.T), dev(cells.p), dev(cells.Y)
+    om_g, dY_g = torch.zeros(K, n, device="cuda"), torch.zeros(K, n, device="cuda")
+    ws = B.alloc_workspace_mmlp(gn, n, n)
+    B.df_chem_ann_source_mmlp(gn, gm, T, p, Y, omega=om_g, dY=dY_g, workspace=ws, n_cells=n)
+    torch.cuda.synchronize()
+    s = (Y.double() + dY_g.double()).sum(dim=0)
+    sum_err = float((s - 1.0).abs().max())
+    assert sum_err <= 1e-6
+    idx = np.unique(np.concatenate([np.arange(0, n, n // 160), np.arange(n - 40, n)]))
+    it = torch.from_numpy(idx).cuda()
+    Ys = np.ascontiguousarray(cells.Y[:, idx])
+    om_r, dY_r = oracle.Mmlp(nets).source(oracle.Mech(mech), cells.T[idx], cells.p[idx], Ys)
+    floor_om, floor_dY = ideal16.ideal_chain_source_mmlp(mech, nets, cells.T[idx], cells.p[idx], Ys, "fp16")
+    failures = []
+    for name, got, ref, ideal in (("dY", dY_g[:, it].cpu().numpy(), dY_r[:, :len(idx)], floor_dY),
+                                  ("omega", om_g[:, it].cpu().numpy(), om_r[:, :len(idx)], floor_om)):
+        table = helpers.mixed_err_table(got, ref)
+        bound, floor = helpers.bounds_16bit(ref, ideal, 2e-2)
+        helpers.record("mmlp_bench_size", dict(quantity=name, dims=[K + 2] + hidden + [1], precision=1, n=n, cells_compared=int(len(idx)),
+                                               sum_to_one=sum_err, tol=2e-2, per_species=table, ideal_fp16_chain=floor))
+        for t in table:
+            if t["mixed"] > bound[t["k"]] or t["normwise"] > 2e-2:
+                failures.append(f"{name}[k={t['k']}]: mixed {t['mixed']:.3e} (bound {bound[t['k']]:.3e}) normwise {t['normwise']:.3e}")
+    assert not failures, "; ".join(failures)
