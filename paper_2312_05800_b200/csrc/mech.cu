@@ -25,6 +25,55 @@ void shift_poly(const long double* p, int n, long double c, long double s, long 
     }
 }
 
+// One-sided Jacobi SVD (Hestenes) of a K x K matrix in fp64: A = U diag(s) V^T, s descending.  A is overwritten by U diag(s).
+void jacobi_svd(int K, std::vector<double>& A, std::vector<double>& V, std::vector<double>& s) {
+    V.assign((size_t)K * K, 0.0);
+    for (int i = 0; i < K; ++i) V[(size_t)i * K + i] = 1.0;
+    for (int sweep = 0; sweep < 60; ++sweep) {
+        double off = 0.0;
+        for (int p = 0; p < K - 1; ++p)
+            for (int q = p + 1; q < K; ++q) {
+                double a = 0.0, b = 0.0, c = 0.0;
+                for (int i = 0; i < K; ++i) {
+                    const double x = A[(size_t)i * K + p], y = A[(size_t)i * K + q];
+                    a += x * x; b += y * y; c += x * y;
+                }
+                if (fabs(c) <= 1e-300) continue;
+                off = fmax(off, fabs(c) / sqrt(fmax(a * b, 1e-300)));
+                const double zeta = (b - a) / (2.0 * c);
+                const double tq = (zeta >= 0.0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
+                const double cs = 1.0 / sqrt(1.0 + tq * tq), sn = cs * tq;
+                for (int i = 0; i < K; ++i) {
+                    double x = A[(size_t)i * K + p], y = A[(size_t)i * K + q];
+                    A[(size_t)i * K + p] = cs * x - sn * y;
+                    A[(size_t)i * K + q] = sn * x + cs * y;
+                    x = V[(size_t)i * K + p]; y = V[(size_t)i * K + q];
+                    V[(size_t)i * K + p] = cs * x - sn * y;
+                    V[(size_t)i * K + q] = sn * x + cs * y;
+                }
+            }
+        if (off < 1e-15) break;
+    }
+    s.assign(K, 0.0);   // column norms = singular values; then sort descending
+    for (int j = 0; j < K; ++j) {
+        double n2 = 0.0;
+        for (int i = 0; i < K; ++i) n2 += A[(size_t)i * K + j] * A[(size_t)i * K + j];
+        s[j] = sqrt(n2);
+    }
+    for (int j = 0; j < K; ++j) {
+        int best = j;
+        for (int l = j + 1; l < K; ++l)
+            if (s[l] > s[best]) best = l;
+        if (best != j) {
+            std::swap(s[j], s[best]);
+            for (int i = 0; i < K; ++i) {
+                std::swap(A[(size_t)i * K + j], A[(size_t)i * K + best]);
+                std::swap(V[(size_t)i * K + j], V[(size_t)i * K + best]);
+            }
+        }
+    }
+}
+
 template <typename T>
 df_status to_device(T** dst, const std::vector<T>& src) {
     *dst = nullptr;
@@ -203,6 +252,46 @@ extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const
                     const int k = w * KW + a;
                     if (k < K) BW[((size_t)w * Kp + j) * 16 + a] = t.wilkeB[(size_t)k * K + j];
                 }
+        // Wilke's B factored (common.cuh): B = U diag(s) V^T from the fp64 weights, truncated after kWilkeRank terms, accepted
+        // when every element of the truncated product is within 2e-7 of B (relative) and the factored form is cheaper
+        std::vector<float> VW, UW;
+        if (K > 28) {
+            std::vector<double> A((size_t)K * K), Bd((size_t)K * K), V, sv;
+            for (int k = 0; k < K; ++k)
+                for (int j = 0; j < K; ++j) Bd[(size_t)k * K + j] = 1.0 / sqrt(8.0 * (1.0 + W[k] / W[j]));
+            A = Bd;
+            jacobi_svd(K, A, V, sv);   // A = U diag(s)
+            double worst = 0.0;
+            for (int k = 0; k < K; ++k)
+                for (int j = 0; j < K; ++j) {
+                    double acc = 0.0;
+                    for (int m = 0; m < kWilkeRank; ++m) acc += A[(size_t)k * K + m] * V[(size_t)j * K + m];
+                    worst = fmax(worst, fabs(acc / Bd[(size_t)k * K + j] - 1.0));
+                }
+            if (worst <= 2e-7) {
+                // the leading pair of singular vectors of a positive matrix has one sign: make it +, so that the m = 0 term
+                // of a denominator is positive (the padding rows' denominators consist of it alone)
+                double sg = 0.0;
+                for (int j = 0; j < K; ++j) sg += V[(size_t)j * K];
+                const double flip = sg < 0.0 ? -1.0 : 1.0;
+                VW.assign((size_t)4 * Kp * 4, 0.f);
+                UW.assign((size_t)4 * kWilkeRank * 16, 0.f);
+                for (int w = 0; w < 4; ++w) {
+                    for (int j = 0; j < K; ++j)
+                        for (int c = 0; c < 3; ++c) {
+                            const int m = w + 4 * c;
+                            VW[((size_t)w * Kp + j) * 4 + c] = (float)((m == 0 ? flip : 1.0) * V[(size_t)j * K + m]);
+                        }
+                    for (int m = 0; m < kWilkeRank; ++m)
+                        for (int a = 0; a < KW; ++a) {
+                            const int k = w * KW + a;
+                            UW[((size_t)w * kWilkeRank + m) * 16 + a] =
+                                k < K ? (float)((m == 0 ? flip : 1.0) * A[(size_t)k * K + m]) : (m == 0 ? 1.f : 0.f);
+                        }
+                }
+                d.wilke_rank = kWilkeRank;
+            }
+        }
         // eight species tiles of TS; tile pair (kt <= jt) number kt*8 - kt(kt-1)/2 + (jt - kt): [a][b][5], rows padded to RS
         size_t tix = 0;
         for (int kt = 0; kt < 8; ++kt)
@@ -217,7 +306,7 @@ extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const
                             c[0] = 1.f;
                     }
         if ((st = to_device(&d.small_p, small)) || (st = to_device(&d.thp, thp)) || (st = to_device(&d.h0p, h0p)) ||
-            (st = to_device(&d.BW, BW)) || (st = to_device(&d.dtile, dt))) {
+            (st = to_device(&d.BW, BW)) || (st = to_device(&d.dtile, dt)) || (st = to_device(&d.VW, VW)) || (st = to_device(&d.UW, UW))) {
             df_mech_destroy(mech);
             return st;
         }
@@ -245,6 +334,8 @@ extern "C" df_status df_mech_destroy(df_mech* mech) {
     cudaFree(d.thp);
     cudaFree(d.h0p);
     cudaFree(d.BW);
+    cudaFree(d.VW);
+    cudaFree(d.UW);
     cudaFree(d.dtile);
     delete mech->t9;
     delete mech->t19;

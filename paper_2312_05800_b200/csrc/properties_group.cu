@@ -102,7 +102,7 @@ constexpr int kSmallStride = 20;
 struct GroupSmem {   // byte offsets into the dynamic shared memory of a block
     int sX, sR, small, thp, h0p, BW, ring, scr, total;
 };
-__host__ __device__ inline GroupSmem group_smem(int Kp) {
+__host__ __device__ inline GroupSmem group_smem(int Kp, bool lr) {
     GroupSmem g;
     int o = 0;
     g.sX = o; o += Kp * 32 * 8;
@@ -110,7 +110,7 @@ __host__ __device__ inline GroupSmem group_smem(int Kp) {
     g.h0p = o; o += Kp * 2 * 8;
     g.small = o; o += Kp * kSmallStride * 4;
     g.thp = o; o += Kp * 12 * 4;
-    g.BW = o; o += 4 * Kp * 16 * 4;
+    g.BW = o; o += lr ? (4 * Kp * 4 + 4 * kWilkeRank * 16) * 4 : 4 * Kp * 16 * 4;   // factored: VW then UW
     g.ring = o; o += 4 * 2 * kTileFloatsMax * 4;   // per warp: two coefficient tiles
     g.scr = o; o += 4 * kScrSlots * 32 * 8;
     g.total = o;
@@ -120,7 +120,8 @@ __host__ __device__ inline GroupSmem group_smem(int Kp) {
 // KW: Wilke rows per warp = Kp / 4.  FULL: every group of the launch lies inside the field (the host launches the ragged
 // last group separately), so loads and stores are plain float2 accesses.  ALL: all five outputs are wanted (the solver's
 // call), so none of the per-species code is guarded by a runtime flag.
-template <int KW, bool FULL, bool ALL>
+// LR: Wilke's B in its factored form (MechDev::VW, UW).
+template <int KW, bool FULL, bool ALL, bool LR>
 __global__ void __launch_bounds__(kGT, 3)
 props_group_kernel(const __grid_constant__ MechDev md, long long g_first, long long g_end, long long n, long long ld, const float* __restrict__ Tg,
                    const float* __restrict__ pg, const float* __restrict__ Yg, float* __restrict__ cp_o,
@@ -128,7 +129,7 @@ props_group_kernel(const __grid_constant__ MechDev md, long long g_first, long l
     extern __shared__ __align__(16) unsigned char smem[];
     constexpr int Kp = 4 * KW, TS = KW / 2;   // eight species tiles of TS
     const int K = md.K;
-    const GroupSmem L = group_smem(Kp);
+    const GroupSmem L = group_smem(Kp, LR);
     f2* sX = reinterpret_cast<f2*>(smem + L.sX);
     f2* sR = reinterpret_cast<f2*>(smem + L.sR);
     const double* sH0 = reinterpret_cast<const double*>(smem + L.h0p);
@@ -145,8 +146,15 @@ props_group_kernel(const __grid_constant__ MechDev md, long long g_first, long l
         reinterpret_cast<float4*>(smem + L.small)[e] = __ldg(reinterpret_cast<const float4*>(md.small_p) + e);
     for (int e = tid; e < Kp * 12 / 4; e += kGT)
         reinterpret_cast<float4*>(smem + L.thp)[e] = __ldg(reinterpret_cast<const float4*>(md.thp) + e);
-    for (int e = tid; e < 4 * Kp * 16 / 4; e += kGT)
-        reinterpret_cast<float4*>(smem + L.BW)[e] = __ldg(reinterpret_cast<const float4*>(md.BW) + e);
+    if (LR) {
+        for (int e = tid; e < Kp * 4; e += kGT)
+            reinterpret_cast<float4*>(smem + L.BW)[e] = __ldg(reinterpret_cast<const float4*>(md.VW) + e);
+        for (int e = tid; e < kWilkeRank * 16; e += kGT)
+            reinterpret_cast<float4*>(smem + L.BW)[Kp * 4 + e] = __ldg(reinterpret_cast<const float4*>(md.UW) + e);
+    } else {
+        for (int e = tid; e < 4 * Kp * 16 / 4; e += kGT)
+            reinterpret_cast<float4*>(smem + L.BW)[e] = __ldg(reinterpret_cast<const float4*>(md.BW) + e);
+    }
     __syncthreads();
 
     const bool want_h = ALL || h_o, want_cp = ALL || cp_o, want_mu = ALL || mu_o, want_lam = ALL || lam_o, want_D = ALL || D_o;
@@ -311,9 +319,55 @@ props_group_kernel(const __grid_constant__ MechDev md, long long g_first, long l
                 gk[a] = rcp2(sR[(k0 + a) * 32 + lane]);
                 den[a] = bc(0.f);
             }
+            if (LR) {
+                // den_k = sum_j B_kj (x_j + 2 g_k x_j r_j + g_k^2 x_j r_j^2) with B = U diag(s) V^T cut after kWilkeRank terms
+                // (2e-7; B is a smooth function of W_k/W_j): first the three vectors projected on the V_m -- warp w takes the
+                // modes w, w + 4, w + 8 over all species --, then, after a barrier, the rows of this warp from the U_m:
+                // 6 r K packed FMAs per group instead of 3 K^2.
+                constexpr int NM = kWilkeRank / 4;
+                f2 tP[NM], tQ[NM], tR[NM];
+#pragma unroll
+                for (int c = 0; c < NM; ++c) tP[c] = tQ[c] = tR[c] = bc(0.f);
+                const float4* vw = reinterpret_cast<const float4*>(sBW) + (size_t)w * Kp;
+#pragma unroll 4
+                for (int j = 0; j < K; ++j) {
+                    const f2 xj = sX[j * 32 + lane], rj = sR[j * 32 + lane];
+                    const f2 xr = mul2(xj, rj), xrr = mul2(xr, rj);
+                    const float4 v = vw[j];
+                    const float vm[3] = {v.x, v.y, v.z};
+#pragma unroll
+                    for (int c = 0; c < NM; ++c) {
+                        tP[c] = fma2(xj, vm[c], tP[c]);
+                        tQ[c] = fma2(xr, vm[c], tQ[c]);
+                        tR[c] = fma2(xrr, vm[c], tR[c]);
+                    }
+                }
+                f2* sT = reinterpret_cast<f2*>(sRing);   // [mode][3][lane]: the ring is idle until the pair rounds
+#pragma unroll
+                for (int c = 0; c < NM; ++c) {
+                    const int m = w + 4 * c;
+                    sT[(3 * m) * 32 + lane] = tP[c];
+                    sT[(3 * m + 1) * 32 + lane] = add2(tQ[c], tQ[c]);
+                    sT[(3 * m + 2) * 32 + lane] = tR[c];
+                }
+                __syncthreads();
+                const float* uw = sBW + (size_t)4 * Kp * 4 + (size_t)w * kWilkeRank * 16;
+#pragma unroll 2
+                for (int m = 0; m < kWilkeRank; ++m) {
+                    const f2 p0 = sT[(3 * m) * 32 + lane], q2 = sT[(3 * m + 1) * 32 + lane], r2 = sT[(3 * m + 2) * 32 + lane];
+                    float U[16];
+#pragma unroll
+                    for (int q4 = 0; q4 < (KW + 3) / 4; ++q4) {
+                        const float4 v = *reinterpret_cast<const float4*>(uw + m * 16 + 4 * q4);
+                        U[4 * q4] = v.x; U[4 * q4 + 1] = v.y; U[4 * q4 + 2] = v.z; U[4 * q4 + 3] = v.w;
+                    }
+#pragma unroll
+                    for (int a = 0; a < KW; ++a) den[a] = fma2(fma2(gk[a], fma2(gk[a], r2, q2), p0), U[a], den[a]);
+                }
+            }
             const float* bw = sBW + (size_t)w * Kp * 16;
 #pragma unroll 2
-            for (int j = 0; j < K; ++j) {   // padding species have X_j = 0: skipped
+            for (int j = 0; j < (LR ? 0 : K); ++j) {   // padding species have X_j = 0: skipped
                 const f2 xj = sX[j * 32 + lane], rj = sR[j * 32 + lane];
                 const f2 xr = mul2(xj, rj);
                 const f2 b2 = add2(xr, xr), c = mul2(xr, rj);
@@ -436,34 +490,43 @@ props_group_kernel(const __grid_constant__ MechDev md, long long g_first, long l
     }
 }
 
-template <int KW, bool FULL, bool ALL>
+template <int KW, bool FULL, bool ALL, bool LR>
 df_status launch_one(const MechDev& md, long long g_first, long long g_end, long long n, long long ld, const float* T, const float* p,
                      const float* Y, float* cp, float* h, float* mu, float* lam, float* D, cudaStream_t s) {
-    const int smem = group_smem(4 * KW).total;
+    const int smem = group_smem(4 * KW, LR).total;
     static DfPerDevice smem_attr;
-    const df_status st = df_ensure_dyn_smem((const void*)props_group_kernel<KW, FULL, ALL>, smem, &smem_attr);
+    const df_status st = df_ensure_dyn_smem((const void*)props_group_kernel<KW, FULL, ALL, LR>, smem, &smem_attr);
     if (st != DF_OK) return st;
     const long long ngroups = g_end - g_first;
     const long long cap = (long long)df_device_sm_count() * 3 * 4;   // 3 resident blocks per SM, ~4 waves
     const long long blocks = ngroups < cap ? ngroups : cap;
-    props_group_kernel<KW, FULL, ALL><<<(unsigned)(blocks > 0 ? blocks : 1), kGT, smem, s>>>(md, g_first, g_end, n, ld, T, p, Y, cp, h, mu, lam, D);
+    props_group_kernel<KW, FULL, ALL, LR><<<(unsigned)(blocks > 0 ? blocks : 1), kGT, smem, s>>>(md, g_first, g_end, n, ld, T, p, Y, cp, h, mu, lam, D);
     DF_CUDA_TRY(cudaGetLastError());
     return DF_OK;
 }
 
 // the full groups in one launch, the ragged last group (if any) in a launch of its own
-template <int KW>
-df_status launch_kw(const MechDev& md, long long n, long long ld, const float* T, const float* p, const float* Y, float* cp,
+template <int KW, bool LR>
+df_status launch_lr(const MechDev& md, long long n, long long ld, const float* T, const float* p, const float* Y, float* cp,
                     float* h, float* mu, float* lam, float* D, cudaStream_t s) {
     const long long full_groups = n / kGroupCells, ngroups = (n + kGroupCells - 1) / kGroupCells;
     const bool all = cp && h && mu && lam && D;
     df_status st = DF_OK;
     if (full_groups > 0)
-        st = all ? launch_one<KW, true, true>(md, 0, full_groups, n, ld, T, p, Y, cp, h, mu, lam, D, s)
-                 : launch_one<KW, true, false>(md, 0, full_groups, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+        st = all ? launch_one<KW, true, true, LR>(md, 0, full_groups, n, ld, T, p, Y, cp, h, mu, lam, D, s)
+                 : launch_one<KW, true, false, LR>(md, 0, full_groups, n, ld, T, p, Y, cp, h, mu, lam, D, s);
     if (st == DF_OK && ngroups > full_groups)
-        st = launch_one<KW, false, false>(md, full_groups, ngroups, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+        st = launch_one<KW, false, false, LR>(md, full_groups, ngroups, n, ld, T, p, Y, cp, h, mu, lam, D, s);
     return st;
+}
+
+template <int KW>
+df_status launch_kw(const MechDev& md, long long n, long long ld, const float* T, const float* p, const float* Y, float* cp,
+                    float* h, float* mu, float* lam, float* D, cudaStream_t s) {
+    if constexpr (KW >= 8) {   // K > 28: the factored Wilke pays when the mechanism's B allows it (mech.cu)
+        if (md.wilke_rank == kWilkeRank) return launch_lr<KW, true>(md, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+    }
+    return launch_lr<KW, false>(md, n, ld, T, p, Y, cp, h, mu, lam, D, s);
 }
 
 }  // namespace
