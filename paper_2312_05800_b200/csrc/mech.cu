@@ -261,14 +261,18 @@ extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const
                 for (int j = 0; j < K; ++j) Bd[(size_t)k * K + j] = 1.0 / sqrt(8.0 * (1.0 + W[k] / W[j]));
             A = Bd;
             jacobi_svd(K, A, V, sv);   // A = U diag(s)
-            double worst = 0.0;
-            for (int k = 0; k < K; ++k)
-                for (int j = 0; j < K; ++j) {
-                    double acc = 0.0;
-                    for (int m = 0; m < kWilkeRank; ++m) acc += A[(size_t)k * K + m] * V[(size_t)j * K + m];
-                    worst = fmax(worst, fabs(acc / Bd[(size_t)k * K + j] - 1.0));
-                }
-            if (worst <= 2e-7) {
+            int rank = 0;
+            for (int r = 8; r <= kWilkeRank && !rank; r += 4) {   // the smallest of 8, 12 terms that reproduces every element to 2e-7
+                double worst = 0.0;
+                for (int k = 0; k < K; ++k)
+                    for (int j = 0; j < K; ++j) {
+                        double acc = 0.0;
+                        for (int m = 0; m < r; ++m) acc += A[(size_t)k * K + m] * V[(size_t)j * K + m];
+                        worst = fmax(worst, fabs(acc / Bd[(size_t)k * K + j] - 1.0));
+                    }
+                if (worst <= 2e-7) rank = r;
+            }
+            if (rank) {
                 // the leading pair of singular vectors of a positive matrix has one sign: make it +, so that the m = 0 term
                 // of a denominator is positive (the padding rows' denominators consist of it alone)
                 double sg = 0.0;
@@ -280,7 +284,7 @@ extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const
                     for (int j = 0; j < K; ++j)
                         for (int c = 0; c < 3; ++c) {
                             const int m = w + 4 * c;
-                            VW[((size_t)w * Kp + j) * 4 + c] = (float)((m == 0 ? flip : 1.0) * V[(size_t)j * K + m]);
+                            if (m < rank) VW[((size_t)w * Kp + j) * 4 + c] = (float)((m == 0 ? flip : 1.0) * V[(size_t)j * K + m]);
                         }
                     for (int m = 0; m < kWilkeRank; ++m)
                         for (int a = 0; a < KW; ++a) {
@@ -289,7 +293,7 @@ extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const
                                 k < K ? (float)((m == 0 ? flip : 1.0) * A[(size_t)k * K + m]) : (m == 0 ? 1.f : 0.f);
                         }
                 }
-                d.wilke_rank = kWilkeRank;
+                d.wilke_rank = rank;
             }
         }
         // eight species tiles of TS; tile pair (kt <= jt) number kt*8 - kt(kt-1)/2 + (jt - kt): [a][b][5], rows padded to RS

@@ -102,7 +102,7 @@ constexpr int kSmallStride = 20;
 struct GroupSmem {   // byte offsets into the dynamic shared memory of a block
     int sX, sR, small, thp, h0p, BW, ring, scr, total;
 };
-__host__ __device__ inline GroupSmem group_smem(int Kp, bool lr) {
+__host__ __device__ inline GroupSmem group_smem(int Kp, int wilke_rank) {
     GroupSmem g;
     int o = 0;
     g.sX = o; o += Kp * 32 * 8;
@@ -110,7 +110,7 @@ __host__ __device__ inline GroupSmem group_smem(int Kp, bool lr) {
     g.h0p = o; o += Kp * 2 * 8;
     g.small = o; o += Kp * kSmallStride * 4;
     g.thp = o; o += Kp * 12 * 4;
-    g.BW = o; o += lr ? (4 * Kp * 4 + 4 * kWilkeRank * 16) * 4 : 4 * Kp * 16 * 4;   // factored: VW then UW
+    g.BW = o; o += wilke_rank ? (4 * Kp * 4 + 4 * wilke_rank * 16) * 4 : 4 * Kp * 16 * 4;   // factored: VW then UW
     g.ring = o; o += 4 * 2 * kTileFloatsMax * 4;   // per warp: two coefficient tiles
     g.scr = o; o += 4 * kScrSlots * 32 * 8;
     g.total = o;
@@ -120,8 +120,8 @@ __host__ __device__ inline GroupSmem group_smem(int Kp, bool lr) {
 // KW: Wilke rows per warp = Kp / 4.  FULL: every group of the launch lies inside the field (the host launches the ragged
 // last group separately), so loads and stores are plain float2 accesses.  ALL: all five outputs are wanted (the solver's
 // call), so none of the per-species code is guarded by a runtime flag.
-// LR: Wilke's B in its factored form (MechDev::VW, UW).
-template <int KW, bool FULL, bool ALL, bool LR>
+// NM: 0, or a quarter of the number of terms of Wilke's B in its factored form (MechDev::VW, UW: 2 or 3 modes per warp).
+template <int KW, bool FULL, bool ALL, int NM>
 __global__ void __launch_bounds__(kGT, 3)
 props_group_kernel(const __grid_constant__ MechDev md, long long g_first, long long g_end, long long n, long long ld, const float* __restrict__ Tg,
                    const float* __restrict__ pg, const float* __restrict__ Yg, float* __restrict__ cp_o,
@@ -129,7 +129,9 @@ props_group_kernel(const __grid_constant__ MechDev md, long long g_first, long l
     extern __shared__ __align__(16) unsigned char smem[];
     constexpr int Kp = 4 * KW, TS = KW / 2;   // eight species tiles of TS
     const int K = md.K;
-    const GroupSmem L = group_smem(Kp, LR);
+    constexpr bool LR = NM > 0;
+    constexpr int kRank = 4 * NM;
+    const GroupSmem L = group_smem(Kp, kRank);
     f2* sX = reinterpret_cast<f2*>(smem + L.sX);
     f2* sR = reinterpret_cast<f2*>(smem + L.sR);
     const double* sH0 = reinterpret_cast<const double*>(smem + L.h0p);
@@ -149,8 +151,10 @@ props_group_kernel(const __grid_constant__ MechDev md, long long g_first, long l
     if (LR) {
         for (int e = tid; e < Kp * 4; e += kGT)
             reinterpret_cast<float4*>(smem + L.BW)[e] = __ldg(reinterpret_cast<const float4*>(md.VW) + e);
-        for (int e = tid; e < kWilkeRank * 16; e += kGT)
-            reinterpret_cast<float4*>(smem + L.BW)[Kp * 4 + e] = __ldg(reinterpret_cast<const float4*>(md.UW) + e);
+        for (int e = tid; e < 4 * kRank * 4; e += kGT) {   // UW[w][m < kRank][16], rows of kWilkeRank in global memory
+            const int ww = e / (kRank * 4), rest = e % (kRank * 4);
+            reinterpret_cast<float4*>(smem + L.BW)[Kp * 4 + e] = __ldg(reinterpret_cast<const float4*>(md.UW) + ww * kWilkeRank * 4 + rest);
+        }
     } else {
         for (int e = tid; e < 4 * Kp * 16 / 4; e += kGT)
             reinterpret_cast<float4*>(smem + L.BW)[e] = __ldg(reinterpret_cast<const float4*>(md.BW) + e);
@@ -319,12 +323,11 @@ props_group_kernel(const __grid_constant__ MechDev md, long long g_first, long l
                 gk[a] = rcp2(sR[(k0 + a) * 32 + lane]);
                 den[a] = bc(0.f);
             }
-            if (LR) {
-                // den_k = sum_j B_kj (x_j + 2 g_k x_j r_j + g_k^2 x_j r_j^2) with B = U diag(s) V^T cut after kWilkeRank terms
-                // (2e-7; B is a smooth function of W_k/W_j): first the three vectors projected on the V_m -- warp w takes the
+            if constexpr (LR) {
+                // den_k = sum_j B_kj (x_j + 2 g_k x_j r_j + g_k^2 x_j r_j^2) with B = U diag(s) V^T cut after kRank terms
+                // (kRank = 8 or 12 terms, 2e-7; B is a smooth function of W_k/W_j): first the three vectors projected on the V_m -- warp w takes the
                 // modes w, w + 4, w + 8 over all species --, then, after a barrier, the rows of this warp from the U_m:
                 // 6 r K packed FMAs per group instead of 3 K^2.
-                constexpr int NM = kWilkeRank / 4;
                 f2 tP[NM], tQ[NM], tR[NM];
 #pragma unroll
                 for (int c = 0; c < NM; ++c) tP[c] = tQ[c] = tR[c] = bc(0.f);
@@ -334,7 +337,7 @@ props_group_kernel(const __grid_constant__ MechDev md, long long g_first, long l
                     const f2 xj = sX[j * 32 + lane], rj = sR[j * 32 + lane];
                     const f2 xr = mul2(xj, rj), xrr = mul2(xr, rj);
                     const float4 v = vw[j];
-                    const float vm[3] = {v.x, v.y, v.z};
+                    const float vm[3] = {v.x, v.y, v.z};   // modes w, w + 4, w + 8
 #pragma unroll
                     for (int c = 0; c < NM; ++c) {
                         tP[c] = fma2(xj, vm[c], tP[c]);
@@ -351,9 +354,9 @@ props_group_kernel(const __grid_constant__ MechDev md, long long g_first, long l
                     sT[(3 * m + 2) * 32 + lane] = tR[c];
                 }
                 __syncthreads();
-                const float* uw = sBW + (size_t)4 * Kp * 4 + (size_t)w * kWilkeRank * 16;
+                const float* uw = sBW + (size_t)4 * Kp * 4 + (size_t)w * kRank * 16;
 #pragma unroll 2
-                for (int m = 0; m < kWilkeRank; ++m) {
+                for (int m = 0; m < kRank; ++m) {
                     const f2 p0 = sT[(3 * m) * 32 + lane], q2 = sT[(3 * m + 1) * 32 + lane], r2 = sT[(3 * m + 2) * 32 + lane];
                     float U[16];
 #pragma unroll
@@ -490,33 +493,33 @@ props_group_kernel(const __grid_constant__ MechDev md, long long g_first, long l
     }
 }
 
-template <int KW, bool FULL, bool ALL, bool LR>
+template <int KW, bool FULL, bool ALL, int NM>
 df_status launch_one(const MechDev& md, long long g_first, long long g_end, long long n, long long ld, const float* T, const float* p,
                      const float* Y, float* cp, float* h, float* mu, float* lam, float* D, cudaStream_t s) {
-    const int smem = group_smem(4 * KW, LR).total;
+    const int smem = group_smem(4 * KW, 4 * NM).total;
     static DfPerDevice smem_attr;
-    const df_status st = df_ensure_dyn_smem((const void*)props_group_kernel<KW, FULL, ALL, LR>, smem, &smem_attr);
+    const df_status st = df_ensure_dyn_smem((const void*)props_group_kernel<KW, FULL, ALL, NM>, smem, &smem_attr);
     if (st != DF_OK) return st;
     const long long ngroups = g_end - g_first;
     const long long cap = (long long)df_device_sm_count() * 3 * 4;   // 3 resident blocks per SM, ~4 waves
     const long long blocks = ngroups < cap ? ngroups : cap;
-    props_group_kernel<KW, FULL, ALL, LR><<<(unsigned)(blocks > 0 ? blocks : 1), kGT, smem, s>>>(md, g_first, g_end, n, ld, T, p, Y, cp, h, mu, lam, D);
+    props_group_kernel<KW, FULL, ALL, NM><<<(unsigned)(blocks > 0 ? blocks : 1), kGT, smem, s>>>(md, g_first, g_end, n, ld, T, p, Y, cp, h, mu, lam, D);
     DF_CUDA_TRY(cudaGetLastError());
     return DF_OK;
 }
 
 // the full groups in one launch, the ragged last group (if any) in a launch of its own
-template <int KW, bool LR>
+template <int KW, int NM>
 df_status launch_lr(const MechDev& md, long long n, long long ld, const float* T, const float* p, const float* Y, float* cp,
                     float* h, float* mu, float* lam, float* D, cudaStream_t s) {
     const long long full_groups = n / kGroupCells, ngroups = (n + kGroupCells - 1) / kGroupCells;
     const bool all = cp && h && mu && lam && D;
     df_status st = DF_OK;
     if (full_groups > 0)
-        st = all ? launch_one<KW, true, true, LR>(md, 0, full_groups, n, ld, T, p, Y, cp, h, mu, lam, D, s)
-                 : launch_one<KW, true, false, LR>(md, 0, full_groups, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+        st = all ? launch_one<KW, true, true, NM>(md, 0, full_groups, n, ld, T, p, Y, cp, h, mu, lam, D, s)
+                 : launch_one<KW, true, false, NM>(md, 0, full_groups, n, ld, T, p, Y, cp, h, mu, lam, D, s);
     if (st == DF_OK && ngroups > full_groups)
-        st = launch_one<KW, false, false, LR>(md, full_groups, ngroups, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+        st = launch_one<KW, false, false, NM>(md, full_groups, ngroups, n, ld, T, p, Y, cp, h, mu, lam, D, s);
     return st;
 }
 
@@ -524,9 +527,10 @@ template <int KW>
 df_status launch_kw(const MechDev& md, long long n, long long ld, const float* T, const float* p, const float* Y, float* cp,
                     float* h, float* mu, float* lam, float* D, cudaStream_t s) {
     if constexpr (KW >= 8) {   // K > 28: the factored Wilke pays when the mechanism's B allows it (mech.cu)
-        if (md.wilke_rank == kWilkeRank) return launch_lr<KW, true>(md, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+        if (md.wilke_rank == 8) return launch_lr<KW, 2>(md, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+        if (md.wilke_rank == 12) return launch_lr<KW, 3>(md, n, ld, T, p, Y, cp, h, mu, lam, D, s);
     }
-    return launch_lr<KW, false>(md, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+    return launch_lr<KW, 0>(md, n, ld, T, p, Y, cp, h, mu, lam, D, s);
 }
 
 }  // namespace

@@ -197,6 +197,19 @@ def test_properties_subset_outputs(B):
     assert helpers.rel_err(mu.cpu().numpy(), ref["mu"]).max() <= 1e-5
 
 
+@pytest.mark.parametrize("K,w_hi", [(40, 44.0), (40, 250.0), (61, 1200.0)])
+def test_properties_factored_wilke_weight_ranges(B, K, w_hi):
+    """The any-K kernel holds Wilke's B factored (8 or 12 terms, chosen at create from the molecular weights) or, when the
+    weights span too wide a range for 12 terms, in full: log-spaced weights 1 ... w_hi exercise the three cases."""
+    import dataclasses
+    from oracle import oracle
+    from paper_2312_05800_b200 import synth
+    mech = synth.make_mechanism(K, 900 + K)
+    mech = dataclasses.replace(mech, W=np.exp(np.linspace(0.0, np.log(w_hi), K)))
+    cells = synth.cells_stratified(K, 333, 901 + K, ld=336)
+    check_properties(B, mech, cells, oracle.Mech(mech), 333)
+
+
 @pytest.mark.parametrize("K,n,ld", [(24, 200, 200), (53, 131, 132)])
 def test_properties_subset_outputs_generic_K(B, K, n, ld):
     """The any-K kernel's instantiations for calls that want only some outputs, on full groups and a ragged last one."""
