@@ -81,6 +81,9 @@ struct PropTables {
     float invW[K], sqrtW[K];
     float visc[K][5], cond[K][5], ddiag[K][5];
     float B[K][K];
+    // Wilke's B factored, B_kj ~ sum_{m < wilke_rank} WU[k][m] WV[j][m] (WU carries the singular values); wilke_rank = 0: use B
+    float WV[K][8], WU[K][8];
+    int wilke_rank;
     float dpair[K * (K - 1) / 2 > 0 ? K * (K - 1) / 2 : 1][5];  // pairs (j<k) in row-major order of (j,k)
     MechScalars sc;
 };

@@ -91,7 +91,7 @@ struct HostTables {
 };
 
 template <int K>
-PropTables<K>* make_fixed(const HostTables& t) {
+PropTables<K>* make_fixed(const HostTables& t, const double* W) {
     PropTables<K>* p = new PropTables<K>;
     memset(p, 0, sizeof(*p));
     for (int k = 0; k < K; ++k) {
@@ -113,6 +113,30 @@ PropTables<K>* make_fixed(const HostTables& t) {
         for (int k = j + 1; k < K; ++k, ++idx)
             for (int m = 0; m < 5; ++m) p->dpair[idx][m] = t.dfull[(j * K + k) * 5 + m];
     p->sc = t.sc;
+    // factored Wilke (see MechDev::wilke_rank): the smallest of 7, 8 terms that reproduces every B_kj to 2e-7, if it is
+    // cheaper than the K x K table (2 r < K)
+    if (K > 16) {
+        std::vector<double> A((size_t)K * K), Bd((size_t)K * K), V, sv;
+        for (int k = 0; k < K; ++k)
+            for (int j = 0; j < K; ++j) Bd[(size_t)k * K + j] = 1.0 / sqrt(8.0 * (1.0 + W[k] / W[j]));
+        A = Bd;
+        jacobi_svd(K, A, V, sv);
+        for (int r = 7; r <= 8 && !p->wilke_rank; ++r) {
+            double worst = 0.0;
+            for (int k = 0; k < K; ++k)
+                for (int j = 0; j < K; ++j) {
+                    double acc = 0.0;
+                    for (int m = 0; m < r; ++m) acc += A[(size_t)k * K + m] * V[(size_t)j * K + m];
+                    worst = fmax(worst, fabs(acc / Bd[(size_t)k * K + j] - 1.0));
+                }
+            if (worst <= 2e-7) p->wilke_rank = r;
+        }
+        for (int k = 0; k < K; ++k)
+            for (int m = 0; m < p->wilke_rank; ++m) {
+                p->WU[k][m] = (float)A[(size_t)k * K + m];
+                p->WV[k][m] = (float)V[(size_t)k * K + m];
+            }
+    }
     return p;
 }
 
@@ -315,8 +339,8 @@ extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const
             return st;
         }
     }
-    if (K == 9) mech->t9 = make_fixed<9>(t);
-    if (K == 19) mech->t19 = make_fixed<19>(t);
+    if (K == 9) mech->t9 = make_fixed<9>(t, W);
+    if (K == 19) mech->t19 = make_fixed<19>(t, W);
     *out = mech;
     return DF_OK;
 }

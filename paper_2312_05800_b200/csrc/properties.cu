@@ -46,7 +46,8 @@ __device__ __forceinline__ f2 poly4_2(const float* c, f2 u) {
 // 19 % slower, 3 blocks (168 registers) 23 % slower
 // FULL: every thread of the launch has both of its cells inside the field (the host launches the ragged last block
 // separately), so loads and stores are plain float2 accesses without the two-path predicates.
-template <int K, bool TRANSPORT, bool FULL>
+// R: number of terms of Wilke's B in factored form (PropTables::WU, WV), 0 = the full table.
+template <int K, bool TRANSPORT, bool FULL, int R>
 __global__ void __launch_bounds__(kThreads, 4)
 props_fixed_kernel(const __grid_constant__ PropTables<K> tab, long long i_first, long long n, long long ld,
                    const float* __restrict__ Tg, const float* __restrict__ pg, const float* __restrict__ Yg,
@@ -118,7 +119,39 @@ props_fixed_kernel(const __grid_constant__ PropTables<K> tab, long long i_first,
     const f2 sqrtT = make_float2(sqrtf(T.x), sqrtf(T.y));
 
     // ---- Wilke viscosity ----------------------------------------------------------------------
-    if (mu_o) {
+    if (mu_o && R > 0) {
+        // B = sum_m WU[.][m] WV[.][m] (R terms, 2e-7: B is a smooth function of W_k/W_j, its singular values fall ~10x per
+        // term): den_k = sum_j B_kj (x_j + 2 g_k x_j r_j + g_k^2 x_j r_j^2), r = 1/g, is evaluated as three projections on the
+        // WV_m (3 R K packed FMAs) and K rows from the WU_m (3 R K) instead of 3 K^2; no square roots, X stays X.
+        constexpr int RR = R > 0 ? R : 1;
+        f2 tP[RR], tQ[RR], tR[RR];
+#pragma unroll
+        for (int m = 0; m < RR; ++m) tP[m] = tQ[m] = tR[m] = bc(0.f);
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const f2 rk = rcp2(poly4_2(tab.visc[k], u));
+            const f2 xr = mul2(X[k], rk), xrr = mul2(xr, rk);
+#pragma unroll
+            for (int m = 0; m < RR; ++m) {
+                tP[m] = fma2(X[k], tab.WV[k][m], tP[m]);
+                tQ[m] = fma2(xr, tab.WV[k][m], tQ[m]);
+                tR[m] = fma2(xrr, tab.WV[k][m], tR[m]);
+            }
+        }
+#pragma unroll
+        for (int m = 0; m < RR; ++m) tQ[m] = add2(tQ[m], tQ[m]);
+        f2 acc = bc(0.f);
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const f2 gk = poly4_2(tab.visc[k], u);
+            f2 den = bc(0.f);
+#pragma unroll
+            for (int m = 0; m < RR; ++m) den = fma2(fma2(gk, fma2(gk, tR[m], tQ[m]), tP[m]), tab.WU[k][m], den);
+            acc = fma2(mul2(mul2(X[k], tab.sqrtW[k]), mul2(gk, gk)), rcp2(den), acc);
+        }
+        st2(mu_o, mul2(sqrtT, acc));
+    }
+    if (mu_o && R == 0) {
         // x_j Phi_kj = B_kj (sqrt(x_j) + g_k sqrt(x_j)/g_j)^2: two per-species vectors (a_j = sqrt(x_j), b_j = a_j/g_j) and
         // 3 packed instructions per (k,j) -- the register footprint of the two-vector form at the instruction count of the
         // three-vector one.  X_j is rebuilt as a_j^2 afterwards (1 ulp; exact for x_j = 0).
@@ -199,22 +232,32 @@ props_fixed_kernel(const __grid_constant__ PropTables<K> tab, long long i_first,
     }
 }
 
-template <int K>
-df_status launch_fixed(const PropTables<K>* tab, long long n, long long ld, const float* T, const float* p,
-                       const float* Y, float* cp, float* h, float* mu, float* lam, float* D, cudaStream_t s) {
+template <int K, int R>
+df_status launch_fixed_r(const PropTables<K>* tab, long long n, long long ld, const float* T, const float* p,
+                         const float* Y, float* cp, float* h, float* mu, float* lam, float* D, cudaStream_t s) {
     constexpr long long per_block = 2 * kThreads;
     const long long full_blocks = n / per_block, tail_first = full_blocks * per_block;
     const bool transport = mu || lam || D;
     if (full_blocks > 0) {
-        if (transport) props_fixed_kernel<K, true, true><<<(unsigned)full_blocks, kThreads, 0, s>>>(*tab, 0, n, ld, T, p, Y, cp, h, mu, lam, D);
-        else props_fixed_kernel<K, false, true><<<(unsigned)full_blocks, kThreads, 0, s>>>(*tab, 0, n, ld, T, p, Y, cp, h, mu, lam, D);
+        if (transport) props_fixed_kernel<K, true, true, R><<<(unsigned)full_blocks, kThreads, 0, s>>>(*tab, 0, n, ld, T, p, Y, cp, h, mu, lam, D);
+        else props_fixed_kernel<K, false, true, 0><<<(unsigned)full_blocks, kThreads, 0, s>>>(*tab, 0, n, ld, T, p, Y, cp, h, mu, lam, D);
     }
     if (tail_first < n) {   // the ragged last block
-        if (transport) props_fixed_kernel<K, true, false><<<1, kThreads, 0, s>>>(*tab, tail_first, n, ld, T, p, Y, cp, h, mu, lam, D);
-        else props_fixed_kernel<K, false, false><<<1, kThreads, 0, s>>>(*tab, tail_first, n, ld, T, p, Y, cp, h, mu, lam, D);
+        if (transport) props_fixed_kernel<K, true, false, R><<<1, kThreads, 0, s>>>(*tab, tail_first, n, ld, T, p, Y, cp, h, mu, lam, D);
+        else props_fixed_kernel<K, false, false, 0><<<1, kThreads, 0, s>>>(*tab, tail_first, n, ld, T, p, Y, cp, h, mu, lam, D);
     }
     DF_CUDA_TRY(cudaGetLastError());
     return DF_OK;
+}
+
+template <int K>
+df_status launch_fixed(const PropTables<K>* tab, long long n, long long ld, const float* T, const float* p,
+                       const float* Y, float* cp, float* h, float* mu, float* lam, float* D, cudaStream_t s) {
+    if constexpr (K > 16) {   // the factored Wilke when the mechanism's B allows it (mech.cu: make_fixed)
+        if (tab->wilke_rank == 7) return launch_fixed_r<K, 7>(tab, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+        if (tab->wilke_rank == 8) return launch_fixed_r<K, 8>(tab, n, ld, T, p, Y, cp, h, mu, lam, D, s);
+    }
+    return launch_fixed_r<K, 0>(tab, n, ld, T, p, Y, cp, h, mu, lam, D, s);
 }
 
 }  // namespace
