@@ -64,7 +64,7 @@ struct MechDev {
     float* BW;       // [4][Kp][16]: BW[w][j][a] = B_{k,j} for k = w Kp/4 + a (Wilke rows of warp w; padding 1)
     // Wilke's B in factored form (properties_group.cu, K > 28): B = U diag(s) V^T truncated after wilke_rank = 8 or 12 terms -- B depends
     // on W_k/W_j only and is smooth in it, so its singular values fall by ~10x per term.  wilke_rank = 0: not usable (the
-    // truncation error of this mechanism's B exceeds 2e-7 element-wise, or K is too small to gain) -> the full table BW is used.
+    // truncation error of this mechanism's B exceeds 1e-6 element-wise -- a tenth of the 1e-5 tolerance of mu --, or K is too small to gain) -> the full table BW is used.
     int wilke_rank;
     float* VW;       // [4][Kp][4]:  VW[w][j][c] = V_{j, w + 4c} (modes of warp w; c = 3 and padding species: 0)
     float* UW;       // [4][kWilkeRank][16] (wilke_rank rows used): UW[w][m][a] = U_{k,m} s_m for k = w Kp/4 + a (padding rows: 1 for m = 0, else 0)

@@ -113,7 +113,7 @@ PropTables<K>* make_fixed(const HostTables& t, const double* W) {
         for (int k = j + 1; k < K; ++k, ++idx)
             for (int m = 0; m < 5; ++m) p->dpair[idx][m] = t.dfull[(j * K + k) * 5 + m];
     p->sc = t.sc;
-    // factored Wilke (see MechDev::wilke_rank): the smallest of 7, 8 terms that reproduces every B_kj to 2e-7, if it is
+    // factored Wilke (see MechDev::wilke_rank): the smallest of 7, 8 terms that reproduces every B_kj to 1e-6, if it is
     // cheaper than the K x K table (2 r < K)
     if (K > 16) {
         std::vector<double> A((size_t)K * K), Bd((size_t)K * K), V, sv;
@@ -129,7 +129,7 @@ PropTables<K>* make_fixed(const HostTables& t, const double* W) {
                     for (int m = 0; m < r; ++m) acc += A[(size_t)k * K + m] * V[(size_t)j * K + m];
                     worst = fmax(worst, fabs(acc / Bd[(size_t)k * K + j] - 1.0));
                 }
-            if (worst <= 2e-7) p->wilke_rank = r;
+            if (worst <= 1e-6) p->wilke_rank = r;
         }
         for (int k = 0; k < K; ++k)
             for (int m = 0; m < p->wilke_rank; ++m) {
@@ -277,7 +277,7 @@ extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const
                     if (k < K) BW[((size_t)w * Kp + j) * 16 + a] = t.wilkeB[(size_t)k * K + j];
                 }
         // Wilke's B factored (common.cuh): B = U diag(s) V^T from the fp64 weights, truncated after kWilkeRank terms, accepted
-        // when every element of the truncated product is within 2e-7 of B (relative) and the factored form is cheaper
+        // when every element of the truncated product is within 1e-6 of B (relative) and the factored form is cheaper
         std::vector<float> VW, UW;
         if (K > 28) {
             std::vector<double> A((size_t)K * K), Bd((size_t)K * K), V, sv;
@@ -286,7 +286,7 @@ extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const
             A = Bd;
             jacobi_svd(K, A, V, sv);   // A = U diag(s)
             int rank = 0;
-            for (int r = 8; r <= kWilkeRank && !rank; r += 4) {   // the smallest of 8, 12 terms that reproduces every element to 2e-7
+            for (int r = 8; r <= kWilkeRank && !rank; r += 4) {   // the smallest of 8, 12 terms that reproduces every element to 1e-6
                 double worst = 0.0;
                 for (int k = 0; k < K; ++k)
                     for (int j = 0; j < K; ++j) {
@@ -294,7 +294,7 @@ extern "C" df_status df_mech_create(df_mech** out, int K, const double* W, const
                         for (int m = 0; m < r; ++m) acc += A[(size_t)k * K + m] * V[(size_t)j * K + m];
                         worst = fmax(worst, fabs(acc / Bd[(size_t)k * K + j] - 1.0));
                     }
-                if (worst <= 2e-7) rank = r;
+                if (worst <= 1e-6) rank = r;
             }
             if (rank) {
                 // the leading pair of singular vectors of a positive matrix has one sign: make it +, so that the m = 0 term

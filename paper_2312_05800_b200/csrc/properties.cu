@@ -120,7 +120,7 @@ props_fixed_kernel(const __grid_constant__ PropTables<K> tab, long long i_first,
 
     // ---- Wilke viscosity ----------------------------------------------------------------------
     if (mu_o && R > 0) {
-        // B = sum_m WU[.][m] WV[.][m] (R terms, 2e-7: B is a smooth function of W_k/W_j, its singular values fall ~10x per
+        // B = sum_m WU[.][m] WV[.][m] (R terms, 1e-6: B is a smooth function of W_k/W_j, its singular values fall ~10x per
         // term): den_k = sum_j B_kj (x_j + 2 g_k x_j r_j + g_k^2 x_j r_j^2), r = 1/g, is evaluated as three projections on the
         // WV_m (3 R K packed FMAs) and K rows from the WU_m (3 R K) instead of 3 K^2; no square roots, X stays X.
         constexpr int RR = R > 0 ? R : 1;

@@ -325,7 +325,7 @@ props_group_kernel(const __grid_constant__ MechDev md, long long g_first, long l
             }
             if constexpr (LR) {
                 // den_k = sum_j B_kj (x_j + 2 g_k x_j r_j + g_k^2 x_j r_j^2) with B = U diag(s) V^T cut after kRank terms
-                // (kRank = 8 or 12 terms, 2e-7; B is a smooth function of W_k/W_j): first the three vectors projected on the V_m -- warp w takes the
+                // (kRank = 8 or 12 terms, 1e-6; B is a smooth function of W_k/W_j): first the three vectors projected on the V_m -- warp w takes the
                 // modes w, w + 4, w + 8 over all species --, then, after a barrier, the rows of this warp from the U_m:
                 // 6 r K packed FMAs per group instead of 3 K^2.
                 f2 tP[NM], tQ[NM], tR[NM];

@@ -197,10 +197,11 @@ def test_properties_subset_outputs(B):
     assert helpers.rel_err(mu.cpu().numpy(), ref["mu"]).max() <= 1e-5
 
 
-@pytest.mark.parametrize("K,w_hi", [(40, 44.0), (40, 250.0), (61, 1200.0)])
+@pytest.mark.parametrize("K,w_hi", [(40, 20.0), (40, 250.0), (61, 1200.0), (19, 20.0), (19, 44.0), (19, 400.0)])
 def test_properties_factored_wilke_weight_ranges(B, K, w_hi):
-    """The any-K kernel holds Wilke's B factored (8 or 12 terms, chosen at create from the molecular weights) or, when the
-    weights span too wide a range for 12 terms, in full: log-spaced weights 1 ... w_hi exercise the three cases."""
+    """The property kernels hold Wilke's B factored (any K: 8 or 12 terms; K = 19: 7 or 8 terms; chosen at create from the
+    molecular weights) or, when the weights span too wide a range, in full: log-spaced weights 1 ... w_hi exercise the three
+    cases of each kernel."""
     import dataclasses
     from oracle import oracle
     from paper_2312_05800_b200 import synth
