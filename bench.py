@@ -615,6 +615,12 @@ def run_gpu(args):
         "properties": alu_entry("props kernel (K=19)", props_flops(K), n, k_ms[1], fp32,
                                 {"ms_alone": alone_ms["properties"],
                                  "frac_alone": props_flops(K) * n / (alone_ms["properties"] * 1e-3) / 1e12 / fp32["measured"],
+                                 "frac_alone_vs_nominal": props_flops(K) * n / (alone_ms["properties"] * 1e-3) / 1e12 / fp32["nominal"],
+                                 # in the loop the kernel runs at the clock the MLP's power draw leaves (clocks.sm_mhz); the
+                                 # measured peak is a full-clock burst: the same fraction with the peak scaled to that clock
+                                 "frac_at_loop_clock": (props_flops(K) * n / (k_ms[1] * 1e-3) / 1e12 / fp32["measured"]
+                                                        * clocks["sm_max_mhz"] / clocks["sm_mhz"])
+                                 if clocks.get("sm_mhz") and clocks.get("sm_max_mhz") else None,
                                  "hbm_bytes_per_cell": 4 * (2 * K + 6),
                                  "traffic": ncu_traffic("props_fixed", None) if n == 2097152 else None}),
         "ann_bf16": dict(ann_roof, ms=k_ms[2], ms_alone=alone_ms["ann_bf16"], frac_alone_vs_burst=a_alone / pk["bf16"]),
