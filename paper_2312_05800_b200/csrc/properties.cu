@@ -4,7 +4,8 @@
 // design goal is FMA density, not bytes:
 //   * fixed-K kernels (K = 9, 19) take the whole species table as a __grid_constant__ parameter: fully
 //     unrolled, coefficients reach the FMAs through uniform registers (LDCU), all per-cell vectors in registers;
-//   * Wilke: Phi_kj = B_kj (1 + g_k/g_j)^2 with g = sqrt(mu)/(T W)^(1/4) and B_kj = [8 (1 + W_k/W_j)]^(-1/2) tabulated;
+//   * Wilke: Phi_kj = B_kj (1 + g_k/g_j)^2 with g = sqrt(mu)/(T W)^(1/4) and B_kj = [8 (1 + W_k/W_j)]^(-1/2) tabulated -- as a
+//     truncated singular-value factorisation when the mechanism's weights allow it (R terms: 6 R K instead of 3 K^2 FMAs);
 //   * binary diffusion uses each symmetric pair once (4 FFMA Horner + 1 MUFU.RCP + 2 FFMA);
 //   * the formation-enthalpy part of h is accumulated in fp64 (K DFMA), the sensible part in fp32.
 // Other K (e.g. 53) go to the any-K kernel in properties_group.cu.

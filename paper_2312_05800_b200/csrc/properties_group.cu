@@ -12,7 +12,9 @@
 //            and S_k are corrected by sum(x) at the end -- so nothing here waits for a sum over species)
 //   phase 3  Wilke: warp w owns rows k in [w Kp/4, (w+1) Kp/4) (accumulators in registers) and streams all j:
 //            den_k += B_kj (X_j + g_k (2 X_j r_j + g_k X_j r_j^2)) -- three FFMA2 per (k, j), B_kj from a table re-tiled
-//            per warp so that a row segment is four broadcast LDS.128
+//            per warp so that a row segment is four broadcast LDS.128.  When the mechanism's weights allow it (mech.cu) B is
+//            held factored, B = U diag(s) V^T cut after 8 or 12 terms: warp w projects the three vectors on the modes w, w + 4,
+//            w + 8, one barrier, then expands its rows -- 6 r K FMAs instead of 3 K^2
 //   phase 4  mixture-averaged diffusion: the Kp species form EIGHT tiles of TS = Kp/8, each symmetric pair of species is
 //            evaluated once (4 FFMA2 Horner, two MUFU.RCP, 2 FFMA2).  The 28 off-diagonal tile pairs are played as a
 //            round-robin tournament of 8 teams: 7 rounds x 4 pairs with pairwise disjoint tiles, one pair per warp, so
