@@ -163,7 +163,7 @@ def test_properties(B, cfg, n, ld):
     check_properties(B, mech, cells, om, n)
 
 
-@pytest.mark.parametrize("K", [1, 2, 3, 9, 19, 24])
+@pytest.mark.parametrize("K", [1, 2, 3, 9, 19, 24, 53])
 def test_properties_one_hot_and_generic_K(B, K):
     """Degenerate cells: pure species (A7 self-diffusion branch) and exact zeros, any K."""
     from oracle import oracle
