@@ -37,6 +37,11 @@ namespace {
 
 // ---- geometry ---------------------------------------------------------------------------------
 constexpr int kTileM = 128;
+// Registers by role (setmaxnreg acts on a warpgroup = four consecutive warps; the launch gives every thread 96): warps 0..3
+// (TMA producers, MMA issuers) keep 48, the three epilogue groups take 112 each -- 128 x (48 + 3 x 112 + 96) = 640 x 96.  The
+// epilogue's GELU chains are what the kernel waits for; with 112 registers ptxas keeps more of them in flight (6.05 -> 5.88 ms;
+// four groups of 88 or 96 registers: 5.95-5.99 ms).
+constexpr int kRegsIssue = 48, kRegsEpilogue = 112;
 constexpr int kGroups = 3;                     // epilogue groups of 4 warps (one warp per TMEM lane quarter)
 constexpr int kIssuer2Warp = 3;                // second layer-2/3 MMA issuer
 constexpr int kIoWarp = 4 + 4 * kGroups;       // four cell-I/O warps: next tile's features -> A0, this tile's D4 -> omega
@@ -290,8 +295,10 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    // register budget by role: kRegsIssue / kRegsEpilogue above (every warp of a warpgroup executes its setmaxnreg)
 
     if (warp == 0) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsIssue));
         // ================= TMA producers: two lanes of one warp, each with its own loop (the two sides of one divergent
         // branch make independent progress; 20 warps instead of 21 lifts the register cap from 80 to 96) =================
         // lane 0: weight ring
@@ -336,6 +343,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             }
         }
     } else if (warp == 2) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsIssue));
         // ================= layer-1 MMA issuer (this warp also owns the TMEM allocation) =================
         // Layer 1 has its own issuing warp so that neither issuer has more than two mbarrier round trips per
         // 32-column chunk: it runs ahead of layer 2 as far as the three D1 buffers allow.  Whole warp convergent,
@@ -366,6 +374,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             ++gs;  // the D4 accumulation of this tile (issued by warp 1) takes the next buffer of the ring
         }
     } else if (warp == 1 || warp == kIssuer2Warp) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsIssue));
         // ================= layer-2/3/4 MMA issuers (two warps, each convergent, one elected lane issues) ============
         // One warp needs ~700 cycles of its own instruction stream per 32-wide K stage (two mbarrier round trips,
         // four UTCHMMA, two UTCBAR, warp re-convergence) against ~460 cycles of tensor time, so the stages of the
@@ -469,6 +478,7 @@ ann_bf16_kernel(const __grid_constant__ KArgs a, const __grid_constant__ AnnNorm
             ++gs;
         }
     } else if (warp >= 4 && warp < 4 + 4 * kGroups) {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsEpilogue));
         // ================= epilogue warps: kGroups groups of four (one warp per TMEM lane quarter) =================
         // Group grp takes every kGroups-th layer-1 chunk (so several chunks are in flight), every kGroups-th
         // 16-column unit of the D2/D3 drains, and one 16-byte column chunk of the A0 feature tile.
