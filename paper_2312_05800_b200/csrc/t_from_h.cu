@@ -162,9 +162,13 @@ df_status launch_fixed(const df_mech* mech, long long n, long long ld, const flo
 }
 
 // ---- any K: the same algorithm with the tables in shared memory and a run-time species loop -----------------------
-__global__ void __launch_bounds__(kThreads, 4)
-t_from_h_kernel(int K, MechScalars sc, const double* __restrict__ th64, long long n, long long ld,
-                const float* __restrict__ h, const float* __restrict__ Y, float* __restrict__ T,
+// A block stages the tables once and walks over tiles of 256 cells (grid-stride).  FULL: every tile of the launch lies
+// inside the field (the host launches the ragged last tile separately): plain float2 accesses.
+constexpr int kGenericBlocks = 6;   // resident blocks per SM (85 registers): 4 (126 registers) and 5 measured 9-13 % slower, 8 the same
+template <bool FULL>
+__global__ void __launch_bounds__(kThreads, kGenericBlocks)
+t_from_h_kernel(int K, MechScalars sc, const double* __restrict__ th64, long long tile_first, long long tile_end, long long n,
+                long long ld, const float* __restrict__ h, const float* __restrict__ Y, float* __restrict__ T,
                 float* __restrict__ cp_out, int* __restrict__ n_unconv) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double* sHi = reinterpret_cast<double*>(smem_raw);                              // [K][6] high range
@@ -176,50 +180,53 @@ t_from_h_kernel(int K, MechScalars sc, const double* __restrict__ th64, long lon
         sD[k * 8 + m] = (float)(th64[(k * 2) * 6 + m] - hi);
     }
     __syncthreads();
-    const long long i = ((long long)blockIdx.x * kThreads + threadIdx.x) * 2;
-    if (i >= n) return;
-    const bool two = i + 1 < n;
-    auto ld2 = [&](const float* p) -> float2 {
-        if (two) return __ldg(reinterpret_cast<const float2*>(p + i));
-        const float v = __ldg(p + i);
-        return make_float2(v, v);
-    };
-    double A[6], Bc[6];
-    float2 d[6];
-#pragma unroll
-    for (int m = 0; m < 6; ++m) {
-        A[m] = Bc[m] = 0.0;
-        d[m] = make_float2(0.f, 0.f);
-    }
-#pragma unroll 8
-    for (int k = 0; k < K; ++k) {   // unrolled: eight rows of loads in flight per thread
-        const float2 y = ld2(Y + (size_t)k * ld);
-        const double ya = (double)y.x, yb = (double)y.y;
-        const double2 h01 = *reinterpret_cast<const double2*>(sHi + k * 6), h23 = *reinterpret_cast<const double2*>(sHi + k * 6 + 2),
-                      h45 = *reinterpret_cast<const double2*>(sHi + k * 6 + 4);
-        const float4 d03 = *reinterpret_cast<const float4*>(sD + k * 8);
-        const float2 d45 = *reinterpret_cast<const float2*>(sD + k * 8 + 4);
-        const double hc[6] = {h01.x, h01.y, h23.x, h23.y, h45.x, h45.y};
-        const float dc[6] = {d03.x, d03.y, d03.z, d03.w, d45.x, d45.y};
+    int bad = 0;
+    for (long long tile = tile_first + blockIdx.x; tile < tile_end; tile += gridDim.x) {
+        const long long i = (tile * kThreads + threadIdx.x) * 2;
+        if (!FULL && i >= n) break;
+        const bool two = FULL || i + 1 < n;
+        auto ld2 = [&](const float* p) -> float2 {
+            if (two) return __ldg(reinterpret_cast<const float2*>(p + i));
+            const float v = __ldg(p + i);
+            return make_float2(v, v);
+        };
+        double A[6], Bc[6];
+        float2 d[6];
 #pragma unroll
         for (int m = 0; m < 6; ++m) {
-            A[m] = fma(ya, hc[m], A[m]);
-            Bc[m] = fma(yb, hc[m], Bc[m]);
-            d[m] = __ffma2_rn(y, make_float2(dc[m], dc[m]), d[m]);
+            A[m] = Bc[m] = 0.0;
+            d[m] = make_float2(0.f, 0.f);
         }
-    }
-    const float2 hin = ld2(h);
-    float2 tg;
-    if (two) tg = *reinterpret_cast<const float2*>(T + i);
-    else tg = make_float2(T[i], T[i]);
-    float2 Tout, cpv;
-    const int bad = newton_pair(sc, A, Bc, d, hin, tg, two, Tout, cpv);
-    if (two) {
-        *reinterpret_cast<float2*>(T + i) = Tout;
-        if (cp_out) *reinterpret_cast<float2*>(cp_out + i) = cpv;
-    } else {
-        T[i] = Tout.x;
-        if (cp_out) cp_out[i] = cpv.x;
+#pragma unroll 8
+        for (int k = 0; k < K; ++k) {   // unrolled: eight rows of loads in flight per thread
+            const float2 y = ld2(Y + (size_t)k * ld);
+            const double ya = (double)y.x, yb = (double)y.y;
+            const double2 h01 = *reinterpret_cast<const double2*>(sHi + k * 6), h23 = *reinterpret_cast<const double2*>(sHi + k * 6 + 2),
+                          h45 = *reinterpret_cast<const double2*>(sHi + k * 6 + 4);
+            const float4 d03 = *reinterpret_cast<const float4*>(sD + k * 8);
+            const float2 d45 = *reinterpret_cast<const float2*>(sD + k * 8 + 4);
+            const double hc[6] = {h01.x, h01.y, h23.x, h23.y, h45.x, h45.y};
+            const float dc[6] = {d03.x, d03.y, d03.z, d03.w, d45.x, d45.y};
+#pragma unroll
+            for (int m = 0; m < 6; ++m) {
+                A[m] = fma(ya, hc[m], A[m]);
+                Bc[m] = fma(yb, hc[m], Bc[m]);
+                d[m] = __ffma2_rn(y, make_float2(dc[m], dc[m]), d[m]);
+            }
+        }
+        const float2 hin = ld2(h);
+        float2 tg;
+        if (two) tg = *reinterpret_cast<const float2*>(T + i);
+        else tg = make_float2(T[i], T[i]);
+        float2 Tout, cpv;
+        bad += newton_pair(sc, A, Bc, d, hin, tg, two, Tout, cpv);
+        if (two) {
+            *reinterpret_cast<float2*>(T + i) = Tout;
+            if (cp_out) *reinterpret_cast<float2*>(cp_out + i) = cpv;
+        } else {
+            T[i] = Tout.x;
+            if (cp_out) cp_out[i] = cpv.x;
+        }
     }
     if (n_unconv && bad) atomicAdd(n_unconv, bad);
 }
@@ -232,10 +239,15 @@ df_status launch_T_from_h(const df_mech* mech, long long n, long long ld, const 
     if (K == 19) return launch_fixed<19>(mech, n, ld, h, Y, T, cp, n_unconv, s);
     if (K == 9) return launch_fixed<9>(mech, n, ld, h, Y, T, cp, n_unconv, s);
     const size_t smem = (size_t)K * (6 * sizeof(double) + 8 * sizeof(float));
-    const long long per_block = (long long)kThreads * 2;
-    const long long blocks = (n + per_block - 1) / per_block;
-    if (blocks > 0x7fffffffLL) return df_set_error(DF_ERR_UNSUPPORTED, "df_thermo_T_from_h: n_cells too large");
-    t_from_h_kernel<<<(unsigned)blocks, kThreads, smem, s>>>(K, mech->dev.sc, mech->dev.th64, n, ld, h, Y, T, cp, n_unconv);
+    const long long per_tile = (long long)kThreads * 2;
+    const long long full_tiles = n / per_tile, tiles = (n + per_tile - 1) / per_tile;
+    if (full_tiles > 0) {   // a few waves of resident blocks, each walking over its tiles
+        const long long cap = (long long)df_device_sm_count() * kGenericBlocks * 8;
+        const long long blocks = full_tiles < cap ? full_tiles : cap;
+        t_from_h_kernel<true><<<(unsigned)blocks, kThreads, smem, s>>>(K, mech->dev.sc, mech->dev.th64, 0, full_tiles, n, ld, h, Y, T, cp, n_unconv);
+    }
+    if (tiles > full_tiles)
+        t_from_h_kernel<false><<<1, kThreads, smem, s>>>(K, mech->dev.sc, mech->dev.th64, full_tiles, tiles, n, ld, h, Y, T, cp, n_unconv);
     DF_CUDA_TRY(cudaGetLastError());
     return DF_OK;
 }
