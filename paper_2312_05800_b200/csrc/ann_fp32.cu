@@ -2,8 +2,9 @@
 // 11 -> 64 -> 64 -> 9).  Tensor cores cannot meet the 1e-5 tolerance of this path, so it is plain
 // FFMA.  A block owns 32 cells; lane = cell, and the eight warps split every layer's outputs (warp j takes outputs
 // 8j .. 8j+7, then +64, ...: a cell's serial chain is an eighth of the layer), activations ping-pong through shared
-// memory ([feature][cell], conflict-free), weights W^T[in][out] are read warp-uniformly through the read-only path as
-// float4.  Exact erf GELU (A13).  The configuration is launch/latency-bound (4096 cells), so what counts is the length
+// memory ([feature][cell], conflict-free), weights W^T[in][out] are fetched a layer ahead into shared memory with cp.async
+// (all loads of a layer in flight at once; read from global memory each one was an L2 round trip on the chain: 36 -> 15 us)
+// and read warp-uniformly as float4.  Exact erf GELU (A13).  The configuration is launch/latency-bound (4096 cells), so what counts is the length
 // of the per-cell dependency chain, not throughput.
 #include "ann_common.cuh"
 
@@ -21,6 +22,7 @@ struct Fp32Net {
     const float* WT[kMaxLayers];  // [in][out_pad]
     const float* b[kMaxLayers];   // [out_pad]
     int max_dim;
+    int stage_floats;   // > 0: every layer's W^T and bias fit a shared-memory buffer of this many floats (two of them: double-buffered)
 };
 
 __global__ void __launch_bounds__(kThreads)
@@ -31,6 +33,20 @@ ann_fp32_kernel(Fp32Net net, AnnNorm nm, int K, const float* __restrict__ invW, 
     const int c = threadIdx.x & 31, j = threadIdx.x >> 5;
     float* act0 = sm;
     float* act1 = sm + (size_t)net.max_dim * kCells;
+    float* wbuf = act1 + (size_t)net.max_dim * kCells;   // 2 x stage_floats: layer l's W^T then its bias, staged with cp.async
+    // A weight is read once per block, so from global memory every read is an L2 round trip on the cell's dependency chain;
+    // the whole layer is fetched with all loads in flight at once instead, one layer ahead of its use.
+    auto stage = [&](int l) {
+        if (net.stage_floats == 0 || l >= net.n_layers) return;
+        float* dst = wbuf + (size_t)(l & 1) * net.stage_floats;
+        const int nw = net.dims[l] * net.out_pad[l], nb = net.out_pad[l];
+        for (int e = threadIdx.x * 4; e < nw; e += kThreads * 4)
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst + e)), "l"(net.WT[l] + e) : "memory");
+        for (int e = threadIdx.x * 4; e < nb; e += kThreads * 4)
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst + nw + e)), "l"(net.b[l] + e) : "memory");
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    stage(0);
     const long long i_raw = (long long)blockIdx.x * kCells + c;
     const bool valid = i_raw < n;
     const long long i = valid ? i_raw : 0;   // every thread stays for the barriers; cells past the end are not stored
@@ -43,6 +59,7 @@ ann_fp32_kernel(Fp32Net net, AnnNorm nm, int K, const float* __restrict__ invW, 
         else x = ann_feature_Y(__ldg(Yg + (size_t)(f - 2) * ld + i), nm.lambda, nm.inv_lambda, nm.x_mean[f], nm.x_inv_std[f]);
         act0[f * kCells + c] = x;
     }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
     __syncthreads();
 
     float* in = act0;
@@ -50,18 +67,22 @@ ann_fp32_kernel(Fp32Net net, AnnNorm nm, int K, const float* __restrict__ invW, 
     for (int l = 0; l < net.n_layers; ++l) {
         const int din = net.dims[l], dout = net.dims[l + 1], op = net.out_pad[l];
         const bool last = (l + 1 == net.n_layers);
+        stage(l + 1);
+        const bool staged = net.stage_floats > 0;
+        const float* wl = staged ? wbuf + (size_t)(l & 1) * net.stage_floats : net.WT[l];
+        const float* bl = staged ? wl + din * op : net.b[l];
         for (int o = j * 8; o < dout; o += 8 * kSplit) {
             float acc[8];
-            const float4 b0 = __ldg(reinterpret_cast<const float4*>(net.b[l] + o));
-            const float4 b1 = __ldg(reinterpret_cast<const float4*>(net.b[l] + o + 4));
+            const float4 b0 = *reinterpret_cast<const float4*>(bl + o);
+            const float4 b1 = *reinterpret_cast<const float4*>(bl + o + 4);
             acc[0] = b0.x; acc[1] = b0.y; acc[2] = b0.z; acc[3] = b0.w;
             acc[4] = b1.x; acc[5] = b1.y; acc[6] = b1.z; acc[7] = b1.w;
-            const float* w = net.WT[l] + o;
+            const float* w = wl + o;
 #pragma unroll 4
             for (int ii = 0; ii < din; ++ii) {
                 const float a = in[ii * kCells + c];
-                const float4 w0 = __ldg(reinterpret_cast<const float4*>(w + (size_t)ii * op));
-                const float4 w1 = __ldg(reinterpret_cast<const float4*>(w + (size_t)ii * op + 4));
+                const float4 w0 = *reinterpret_cast<const float4*>(w + (size_t)ii * op);
+                const float4 w1 = *reinterpret_cast<const float4*>(w + (size_t)ii * op + 4);
                 acc[0] = fmaf(a, w0.x, acc[0]); acc[1] = fmaf(a, w0.y, acc[1]);
                 acc[2] = fmaf(a, w0.z, acc[2]); acc[3] = fmaf(a, w0.w, acc[3]);
                 acc[4] = fmaf(a, w1.x, acc[4]); acc[5] = fmaf(a, w1.y, acc[5]);
@@ -71,6 +92,7 @@ ann_fp32_kernel(Fp32Net net, AnnNorm nm, int K, const float* __restrict__ invW, 
             for (int q = 0; q < 8; ++q)
                 if (o + q < dout) out[(o + q) * kCells + c] = last ? acc[q] : gelu_erf(acc[q]);
         }
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncthreads();
         float* tmp = in; in = out; out = tmp;
     }
@@ -118,7 +140,18 @@ df_status launch_ann_fp32(const df_ann* ann, const df_mech* mech, long long n, l
         net.WT[l] = ann->w32 + ann->w32_off[l];
         net.b[l] = ann->w32 + ann->b32_off[l];
     }
-    const size_t smem = (size_t)2 * net.max_dim * kCells * sizeof(float);
+    // stage the weights in shared memory when every layer (W^T + bias) fits 16 K floats and is 16-byte aligned
+    int stage_floats = 0;
+    bool can_stage = true;
+    for (int l = 0; l < ann->n_layers; ++l) {
+        const int fl = ann->dims[l] * ann->out_pad[l] + ann->out_pad[l];
+        if (fl > stage_floats) stage_floats = fl;
+        if (ann->w32_off[l] % 4 || ann->b32_off[l] % 4 || ann->out_pad[l] % 4) can_stage = false;
+    }
+    if (!can_stage || stage_floats > 16384) stage_floats = 0;
+    stage_floats = (stage_floats + 3) / 4 * 4;
+    net.stage_floats = stage_floats;
+    const size_t smem = ((size_t)2 * net.max_dim * kCells + (size_t)2 * stage_floats) * sizeof(float);
     static DfPerDevice smem_attr;
     const df_status st = df_ensure_dyn_smem((const void*)ann_fp32_kernel, 200 * 1024, &smem_attr);
     if (st != DF_OK) return st;
