@@ -297,6 +297,17 @@ def test_ann_source_fp32_ragged_and_degenerate(B):
     check_source(B, mech, ann, cells, 1003, 1e-5, tag="fp32_ragged_degenerate")
 
 
+@pytest.mark.parametrize("hidden", [[256, 200], [40], [24, 24, 24, 24, 24]])
+def test_ann_source_fp32_other_shapes(B, hidden):
+    """The fp32 path stages a layer's weights in shared memory when every layer fits (16 K floats); [256, 200] does not and
+    reads them from global memory; one hidden layer and five hidden layers exercise the double buffering."""
+    from paper_2312_05800_b200 import synth
+    mech = synth.make_mechanism(9, 41)
+    ann = synth.make_ann(9, hidden, 0, 42)
+    cells = synth.cells_dirichlet(9, 333, 43, ld=336)
+    check_source(B, mech, ann, cells, 333, 1e-5, tag="fp32_shapes_" + "_".join(map(str, hidden)))
+
+
 def test_ann_K_mismatch(B):
     from paper_2312_05800_b200 import synth
     mech9 = B.Mech(synth.make_mechanism(9, 1))
