@@ -39,8 +39,8 @@ namespace {
 constexpr int kTileM = 128;
 // Registers by role (setmaxnreg acts on a warpgroup = four consecutive warps; the launch gives every thread 96): warps 0..3
 // (TMA producers, MMA issuers) keep 48, the three epilogue groups take 112 each -- 128 x (48 + 3 x 112 + 96) = 640 x 96.  The
-// epilogue's GELU chains are what the kernel waits for; with 112 registers ptxas keeps more of them in flight (6.05 -> 5.88 ms;
-// four groups of 88 or 96 registers: 5.95-5.99 ms).
+// epilogue's GELU chains are what the kernel waits for; with 112 registers ptxas keeps more of them in flight (A/B on one box: 6.05 -> 5.88 ms,
+// on another 6.14 -> 6.07; four groups of 88 or 96 registers: 5.95-5.99 ms on the first).
 constexpr int kRegsIssue = 48, kRegsEpilogue = 112;
 constexpr int kGroups = 3;                     // epilogue groups of 4 warps (one warp per TMEM lane quarter)
 constexpr int kIssuer2Warp = 3;                // second layer-2/3 MMA issuer
